@@ -1,0 +1,135 @@
+/*
+ * lcs.h -- C ABI of liblcs_b200: the particle hot path of LCS.jl (arxiv/paper_2604_11008) on one
+ * NVIDIA B200 (sm_100a).  Lagrangian step (trilinear gather, drag + gravity advance, 27-way
+ * classification) followed by the prefix-scan particle communication among P = Px*Py*Pz virtual
+ * subdomains held in one GPU's HBM.
+ *
+ * Citations: PAPER.md:<line> is /root/reference/PAPER.md (the only reference file); "DESIGN R-n"
+ * is a numbered reading in DESIGN.md section 3 where the paper is silent or ambiguous.
+ *
+ * Conventions
+ *  - Box: periodic cube [0, L)^3, L = 2*pi as the double 0x401921FB54442D18 (PAPER.md:47, L0 = 1).
+ *  - Fluid: three N^3 fp64 arrays u,v,w at cell centres ((i+1/2)dx, ...), flat index
+ *    i + N*(j + N*k), x fastest (DESIGN R-8).
+ *  - Subdomain s = px + Px*(py + Py*pz); destination code c = (dx+1) + 3*(dy+1) + 9*(dz+1),
+ *    d* in {-1,0,+1}, 13 = stay (DESIGN R-13).
+ *  - Particle state: 8 SoA arrays x,y,z,vx,vy,vz,d (fp64) and id (int64)  (PAPER.md:150-162 lists
+ *    17 Float64 arrays for two RK2 stages; a single stage needs these 8, DESIGN R-2).
+ *  - Every d_* pointer is DEVICE memory owned by the caller, 16-byte aligned.  h_* pointers are
+ *    HOST memory (pinned for full speed).  The library never allocates device memory: it carves
+ *    the caller's workspace.  All calls enqueue on the handle's CUDA stream and return without
+ *    synchronising unless stated.
+ *  - Return value: 0 = LCS_OK, negative = error found on the host at call time.  Errors found on
+ *    the device are sticky in a status word that lcs_get_status reads (capacity overflow, a
+ *    particle that moved more than one subdomain or became non-finite, an input position outside
+ *    [0,L)).  After a sticky error memory safety still holds, particle contents are unspecified
+ *    and every further call returns that code.  (The paper is silent on errors: DESIGN R-16/17.)
+ */
+#ifndef LCS_B200_H
+#define LCS_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LCS_OK                0
+#define LCS_ERR_INVALID_ARG  (-1)
+#define LCS_ERR_STATE        (-2)
+#define LCS_ERR_CUDA         (-3)
+#define LCS_ERR_CAPACITY     (-4)   /* sticky: a receiver slab or a send region overflowed        */
+#define LCS_ERR_JUMP         (-5)   /* sticky: displacement > one subdomain, or non-finite        */
+#define LCS_ERR_RANGE        (-6)   /* sticky: lcs_set_particles saw a position outside [0, L)     */
+
+#define LCS_STAY_CODE 13
+
+typedef struct lcs_handle lcs_t;    /* opaque, host memory, owned by the library */
+
+/* Physical parameters, copied at create. */
+typedef struct {
+    double  nu;             /* kinematic viscosity, 1.5e-5 m^2/s                     */
+    double  rho_ratio;      /* rho_p / rho: 843 in PAPER.md:57, 1000 in BASELINE.json's configs     */
+    double  g[3];           /* gravity; (0,0,0) reproduces Eq. 6, DESIGN R-4          */
+    int64_t send_capacity;  /* migrant slots per subdomain send region; 0 = capacity (never full)  */
+} lcs_params;
+
+/* Bytes of device workspace lcs_create needs; 0 if the arguments are invalid. */
+size_t lcs_workspace_bytes(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params* prm);
+
+/* Create a handle.  N: fluid grid points per axis (>= 2, divisible by Px, Py and Pz);
+ * capacity: particle slots per subdomain slab (rounded up internally to a multiple of 2 is NOT
+ * done: it must be even, so slab bases stay 16-byte aligned); d_workspace: device block of at
+ * least lcs_workspace_bytes(), 256-byte aligned, borrowed until lcs_destroy; cuda_stream: a
+ * cudaStream_t (NULL = legacy default stream). */
+int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params* prm,
+               void* d_workspace, size_t workspace_bytes, void* cuda_stream, lcs_t** out);
+int lcs_destroy(lcs_t* h);
+
+/* Fluid velocity on the N^3 cell centres.  The three pointers are borrowed read-only (zero-copy)
+ * until the next lcs_set_fluid or lcs_destroy.  PAPER.md:64. */
+int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* d_w);
+
+/* Load n particles given in any order; they are binned stably (input order kept inside each
+ * slab) into the subdomain that contains them, all codes = stay.  Copies.  Positions must lie in
+ * [0, L) (else sticky LCS_ERR_RANGE); a slab that would exceed capacity -> sticky LCS_ERR_CAPACITY.
+ * PAPER.md:47 (3-D decomposition), DESIGN R-12. */
+int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y, const double* d_z,
+                      const double* d_vx, const double* d_vy, const double* d_vz,
+                      const double* d_diam, const int64_t* d_id);
+
+/* a1-a4: per particle, interpolate U at X (trilinear), advance V then X under
+ * dV/dt = -(V-U)/tau_p + g, dX/dt = V with U frozen over dt (Eq. 5-6, f = 1;
+ * exponential integrator, DESIGN R-1), wrap into the box, classify into one of 27 destinations
+ * ("mask computation") and count per (subdomain, destination).  In place. */
+int lcs_particle_step(lcs_t* h, double dt);
+
+/* a5-a8: prefix-scan particle communication among the virtual
+ * subdomains, consuming the codes of the last lcs_particle_step: exclusive prefix scan of the
+ * per-(subdomain, destination) indicator (single-pass decoupled look-back), stable pack of the
+ * migrants, in-place stable compaction of the stayers, append in fixed order: receiver r holds
+ * its stayers in original order, then incoming segments by (source s, code c, source slot)
+ * ascending (DESIGN R-12).  LCS_ERR_STATE if no lcs_particle_step preceded it. */
+int lcs_migrate(lcs_t* h);
+
+/* lcs_particle_step followed by lcs_migrate in one pass that reads and writes each particle
+ * once; the result is bit-identical to the two calls. */
+int lcs_step_fused(lcs_t* h, double dt);
+
+/* Per-subdomain particle counts, P int64 values, device pointer. */
+int lcs_get_counts(lcs_t* h, int64_t* d_counts);
+
+/* Packed copy-out: subdomain 0's particles in slot order, then subdomain 1's, ...  Each array
+ * needs room for the current total (lcs_get_status gives it; <= P*capacity).  Any of the data
+ * pointers may be NULL to skip that field. */
+int lcs_get_particles(lcs_t* h, int64_t* d_counts, double* d_x, double* d_y, double* d_z,
+                      double* d_vx, double* d_vy, double* d_vz, double* d_diam, int64_t* d_id);
+
+/* Destination codes of the last lcs_particle_step in the same packed order (uint8, 13 after a
+ * migrate); the P*27 count table (int64, row s, column c).  Test / diagnostic accessors. */
+int lcs_get_codes(lcs_t* h, uint8_t* d_codes);
+int lcs_get_count_table(lcs_t* h, int64_t* d_table);
+
+/* Synchronises the stream and reads the status word.  Any out pointer may be NULL.
+ * Returns the sticky error (0 if none). */
+int lcs_get_status(lcs_t* h, int* sticky_error, int64_t* n_total, int64_t* n_migrated_last);
+
+/* End-to-end convenience with HOST buffers (what a CPU-resident caller pays; cf. the paper's
+ * CPU-delegated path): copies n particles host->device, bins them, runs
+ * lcs_step_fused(dt), copies the packed result and the P counts device->host, synchronises.
+ * h_in / h_out: 8 host pointers each in the order x,y,z,vx,vy,vz,d,id (8 bytes per element;
+ * h_out arrays need room for n).  d_staging: device scratch of at least 64*n + 8*P bytes. */
+int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8], void* const h_out[8],
+                        int64_t* h_counts, void* d_staging, size_t staging_bytes);
+
+/* Number of kernels this library has launched on the handle since create (for bench accounting). */
+int64_t lcs_kernel_launches(lcs_t* h);
+
+/* Library build information: "lcs_b200 <version> sm_100a". */
+const char* lcs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LCS_B200_H */

@@ -209,6 +209,7 @@ int orc_set_particles(orc_t *o, int64_t n, const double *x, const double *y, con
         o->id[slot] = id[p];
         o->code[slot] = ORC_STAY;
     }
+    for (int64_t s = 0; s < o->P; ++s) o->cnt[s * 27 + ORC_STAY] = o->count[s];   /* all codes = stay */
     return ORC_OK;
 }
 

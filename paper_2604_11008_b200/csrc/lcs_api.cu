@@ -1,0 +1,348 @@
+// lcs_api.cu -- the C ABI of include/lcs.h: argument checks, workspace carving, kernel launches.
+// No device allocation happens here (the caller's workspace is carved); every call enqueues on the
+// handle's stream.  Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -fmad=false.
+#include "../../include/lcs.h"
+#include "lcs_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace lcs;
+
+struct lcs_handle {
+    Geom G;
+    Slabs S, Snd;
+    Tables T;
+    cudaStream_t stream;
+    const double *fu, *fv, *fw;
+    int64_t* prefix;          // [P+1] scratch for packed copy-out
+    void* pool;               // send pool base (also scratch of lcs_set_particles)
+    size_t pool_bytes;
+    uint32_t epoch;
+    bool pushed;              // codes + count table describe a push that has not been migrated
+    bool have_particles;
+    int sticky;               // last sticky error seen by lcs_get_status
+    int64_t launches;
+};
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {
+    size_t slab_f[7], slab_id, slab_code;
+    size_t pool, pool_bytes;
+    size_t count, cnt, recv_off, new_count, desc, tile_excl, tile_cnt, misc, prefix;
+    size_t total;
+    int tiles_per_sub;
+    int64_t send_cap;
+};
+
+bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* prm)
+{
+    if (!prm) return false;
+    if (N < 2 || N > (1 << 20) || Px < 1 || Py < 1 || Pz < 1) return false;
+    if (N % Px || N % Py || N % Pz) return false;
+    const int64_t P = (int64_t)Px * Py * Pz;
+    if (P > 8192) return false;                          // grid.y and shared-histogram limits
+    if (cap < 2 || (cap & 1)) return false;               // even: slab bases stay 16-byte aligned
+    if (cap > 0x7fffffff) return false;
+    if (prm->send_capacity < 0 || (prm->send_capacity & 1) || prm->send_capacity > cap) return false;
+    if (!(prm->nu > 0.0) || !(prm->rho_ratio > 0.0)) return false;
+    if (!std::isfinite(prm->g[0]) || !std::isfinite(prm->g[1]) || !std::isfinite(prm->g[2])) return false;
+    return true;
+}
+
+Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* prm)
+{
+    (void)N;
+    Layout L;
+    const size_t P = (size_t)Px * Py * Pz;
+    const size_t slots = P * (size_t)cap;
+    L.send_cap = prm->send_capacity ? prm->send_capacity : cap;
+    L.tiles_per_sub = (int)((cap + kTile - 1) / kTile);
+    const size_t ntiles = P * (size_t)L.tiles_per_sub;
+    size_t off = 0;
+    for (int a = 0; a < 7; ++a) { L.slab_f[a] = off; off = align_up(off + slots * 8); }
+    L.slab_id = off;   off = align_up(off + slots * 8);
+    L.slab_code = off; off = align_up(off + slots);
+    // send pool: 8 arrays of P*send_cap slots; doubles as lcs_set_particles scratch
+    const size_t send_bytes = 8 * align_up(P * (size_t)L.send_cap * 8);
+    const size_t set_tiles = (slots + kSetTile - 1) / kSetTile;
+    const size_t set_bytes = align_up(slots * 4) + align_up(set_tiles * P * 4);
+    L.pool = off; L.pool_bytes = send_bytes > set_bytes ? send_bytes : set_bytes;
+    off = align_up(off + L.pool_bytes);
+    L.count = off;     off = align_up(off + P * 4);
+    L.cnt = off;       off = align_up(off + P * 32 * 4);
+    L.recv_off = off;  off = align_up(off + P * 32 * 4);
+    L.new_count = off; off = align_up(off + P * 4);
+    L.desc = off;      off = align_up(off + ntiles * 32 * 8);
+    L.tile_excl = off; off = align_up(off + ntiles * 32 * 4);
+    L.tile_cnt = off;  off = align_up(off + ntiles * 32 * 4);
+    L.misc = off;      off = align_up(off + 256);
+    L.prefix = off;    off = align_up(off + (P + 1) * 8);
+    L.total = off;
+    return L;
+}
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+inline int check_launch(lcs_t* h, int n = 1)
+{
+    h->launches += n;
+    return cudaPeekAtLastError() == cudaSuccess ? LCS_OK : LCS_ERR_CUDA;
+}
+
+int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
+{
+    const Geom& G = h->G;
+    const unsigned ntiles = (unsigned)G.P * (unsigned)G.tiles_per_sub;
+    h->epoch = (h->epoch + 1u) & 0x3fffffffu;
+    if (h->epoch == 0u) h->epoch = 1u;
+    if (fused)
+        k_tile_pass<true><<<ntiles, kBlock, 0, h->stream>>>(G, h->S, h->Snd, h->T, h->fu, h->fv, h->fw, dt, h->epoch, 0ull);
+    else
+        k_tile_pass<false><<<ntiles, kBlock, 0, h->stream>>>(G, h->S, h->Snd, h->T, h->fu, h->fv, h->fw, dt, h->epoch, 0ull);
+    k_table<<<1, 256, 0, h->stream>>>(G, h->T);
+    k_unpack<<<dim3(G.tiles_per_sub, G.P), kUnpackBlock, 0, h->stream>>>(G, h->S, h->Snd, h->T);
+    k_commit_counts<<<(G.P + 255) / 256, 256, 0, h->stream>>>(G, h->T);
+    h->pushed = false;
+    return check_launch(h, 4);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* lcs_version(void) { return "lcs_b200 0.1 sm_100a"; }
+
+size_t lcs_workspace_bytes(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params* prm)
+{
+    if (!valid_args(N, Px, Py, Pz, capacity, prm)) return 0;
+    return make_layout(N, Px, Py, Pz, capacity, prm).total;
+}
+
+int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params* prm, void* d_workspace,
+               size_t workspace_bytes, void* cuda_stream, lcs_t** out)
+{
+    if (!out) return LCS_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!valid_args(N, Px, Py, Pz, capacity, prm) || !d_workspace) return LCS_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(d_workspace) % kAlign) return LCS_ERR_INVALID_ARG;
+    const Layout L = make_layout(N, Px, Py, Pz, capacity, prm);
+    if (workspace_bytes < L.total) return LCS_ERR_INVALID_ARG;
+    lcs_t* h = new (std::nothrow) lcs_handle();
+    if (!h) return LCS_ERR_CUDA;
+    std::memset(h, 0, sizeof(*h));
+    Geom& G = h->G;
+    G.N = N; G.Px = Px; G.Py = Py; G.Pz = Pz; G.P = Px * Py * Pz;
+    G.nx = N / Px; G.ny = N / Py; G.nz = N / Pz;
+    G.tiles_per_sub = L.tiles_per_sub;
+    G.cap = capacity; G.send_cap = L.send_cap;
+    // all doubles are computed once on the host and passed as data (rule R6)
+    G.L = 6.283185307179586;                      // 2*pi*L0, L0 = 1
+    G.inv_dx = (double)N / G.L;
+    G.K_tau = prm->rho_ratio / (18.0 * prm->nu);  // tau_p = K_tau * d^2
+    G.L_below = std::nextafter(G.L, 0.0);
+    G.gx = prm->g[0]; G.gy = prm->g[1]; G.gz = prm->g[2];
+    char* w = static_cast<char*>(d_workspace);
+    const size_t P = (size_t)G.P;
+    for (int a = 0; a < 7; ++a) h->S.f[a] = reinterpret_cast<double*>(w + L.slab_f[a]);
+    h->S.id = reinterpret_cast<int64_t*>(w + L.slab_id);
+    h->S.code = reinterpret_cast<uint8_t*>(w + L.slab_code);
+    h->pool = w + L.pool; h->pool_bytes = L.pool_bytes;
+    const size_t send_arr = align_up(P * (size_t)L.send_cap * 8);
+    for (int a = 0; a < 7; ++a) h->Snd.f[a] = reinterpret_cast<double*>(w + L.pool + a * send_arr);
+    h->Snd.id = reinterpret_cast<int64_t*>(w + L.pool + 7 * send_arr);
+    h->Snd.code = nullptr;
+    h->T.count = reinterpret_cast<uint32_t*>(w + L.count);
+    h->T.cnt = reinterpret_cast<uint32_t*>(w + L.cnt);
+    h->T.recv_off = reinterpret_cast<uint32_t*>(w + L.recv_off);
+    h->T.new_count = reinterpret_cast<uint32_t*>(w + L.new_count);
+    h->T.desc = reinterpret_cast<uint64_t*>(w + L.desc);
+    h->T.tile_excl = reinterpret_cast<uint32_t*>(w + L.tile_excl);
+    h->T.tile_cnt = reinterpret_cast<uint32_t*>(w + L.tile_cnt);
+    h->T.ticket = reinterpret_cast<unsigned int*>(w + L.misc);
+    h->T.status = reinterpret_cast<int*>(w + L.misc + 16);
+    h->T.n_migrated = reinterpret_cast<unsigned long long*>(w + L.misc + 32);
+    h->T.n_total = reinterpret_cast<unsigned long long*>(w + L.misc + 48);
+    h->prefix = reinterpret_cast<int64_t*>(w + L.prefix);
+    h->stream = static_cast<cudaStream_t>(cuda_stream);
+    // tables start at zero (epoch 0 is never published; counts empty)
+    if (cudaMemsetAsync(w + L.count, 0, L.total - L.count, h->stream) != cudaSuccess) { delete h; return LCS_ERR_CUDA; }
+    *out = h;
+    return LCS_OK;
+}
+
+int lcs_destroy(lcs_t* h)
+{
+    if (!h) return LCS_ERR_INVALID_ARG;
+    cudaStreamSynchronize(h->stream);
+    delete h;
+    return LCS_OK;
+}
+
+int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* d_w)
+{
+    if (!h || !d_u || !d_v || !d_w) return LCS_ERR_INVALID_ARG;
+    if (!aligned16(d_u) || !aligned16(d_v) || !aligned16(d_w)) return LCS_ERR_INVALID_ARG;
+    h->fu = d_u; h->fv = d_v; h->fw = d_w;
+    return LCS_OK;
+}
+
+int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y, const double* d_z,
+                      const double* d_vx, const double* d_vy, const double* d_vz, const double* d_diam,
+                      const int64_t* d_id)
+{
+    if (!h || n < 0) return LCS_ERR_INVALID_ARG;
+    const Geom& G = h->G;
+    if (n > (int64_t)G.P * G.cap) return LCS_ERR_INVALID_ARG;
+    if (n > 0 && (!d_x || !d_y || !d_z || !d_vx || !d_vy || !d_vz || !d_diam || !d_id)) return LCS_ERR_INVALID_ARG;
+    // a fresh particle set clears the sticky error
+    h->sticky = 0;
+    h->pushed = false;
+    h->have_particles = true;
+    cudaMemsetAsync(h->T.status, 0, sizeof(int), h->stream);
+    cudaMemsetAsync(h->T.n_migrated, 0, sizeof(unsigned long long), h->stream);
+    const int ntiles = (int)((n + kSetTile - 1) / kSetTile);
+    int32_t* owner = static_cast<int32_t*>(h->pool);
+    uint32_t* tilehist = reinterpret_cast<uint32_t*>(static_cast<char*>(h->pool) + align_up((size_t)G.P * (size_t)G.cap * 4));
+    if (ntiles > 0)
+        k_set_owner<<<ntiles, 256, (size_t)G.P * 4, h->stream>>>(G, h->T, n, d_x, d_y, d_z, owner, tilehist);
+    k_set_scan<<<(G.P + 127) / 128, 128, 0, h->stream>>>(G, h->T, ntiles, tilehist, n);
+    if (ntiles > 0) {
+        int wpb = (int)(32768 / ((size_t)G.P * 4));
+        wpb = wpb < 1 ? 1 : (wpb > 4 ? 4 : wpb);
+        InPtrs I;
+        I.f[0] = d_x; I.f[1] = d_y; I.f[2] = d_z; I.f[3] = d_vx; I.f[4] = d_vy; I.f[5] = d_vz; I.f[6] = d_diam;
+        I.id = d_id;
+        k_set_scatter<<<(ntiles + wpb - 1) / wpb, 32 * wpb, (size_t)wpb * G.P * 4, h->stream>>>(G, h->S, n, I, owner,
+                                                                                                 tilehist, wpb);
+    }
+    return check_launch(h, ntiles > 0 ? 3 : 1);
+}
+
+int lcs_particle_step(lcs_t* h, double dt)
+{
+    if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
+    if (!h->fu || !h->have_particles) return LCS_ERR_STATE;
+    if (h->sticky) return h->sticky;
+    const Geom& G = h->G;
+    cudaMemsetAsync(h->T.cnt, 0, (size_t)G.P * 32 * 4, h->stream);
+    k_push<<<dim3(G.tiles_per_sub, G.P), kBlock, 0, h->stream>>>(G, h->S, h->T, h->fu, h->fv, h->fw, dt);
+    h->pushed = true;
+    return check_launch(h);
+}
+
+int lcs_migrate(lcs_t* h)
+{
+    if (!h) return LCS_ERR_INVALID_ARG;
+    if (!h->pushed) return LCS_ERR_STATE;
+    if (h->sticky) return h->sticky;
+    return enqueue_tile_pass(h, false, 0.0);
+}
+
+int lcs_step_fused(lcs_t* h, double dt)
+{
+    if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
+    if (!h->fu || !h->have_particles) return LCS_ERR_STATE;
+    if (h->sticky) return h->sticky;
+    return enqueue_tile_pass(h, true, dt);
+}
+
+int lcs_get_counts(lcs_t* h, int64_t* d_counts)
+{
+    if (!h || !d_counts) return LCS_ERR_INVALID_ARG;
+    k_counts_out<<<1, 256, 0, h->stream>>>(h->G, h->T, d_counts, nullptr);
+    return check_launch(h);
+}
+
+static int copy_out(lcs_t* h, int64_t* d_counts, OutPtrs O)
+{
+    const Geom& G = h->G;
+    k_counts_out<<<1, 256, 0, h->stream>>>(G, h->T, d_counts, h->prefix);
+    k_copy_out<<<dim3(G.tiles_per_sub, G.P), kBlock, 0, h->stream>>>(G, h->S, h->T, h->prefix, O, h->pushed ? 1 : 0);
+    return check_launch(h, 2);
+}
+
+int lcs_get_particles(lcs_t* h, int64_t* d_counts, double* d_x, double* d_y, double* d_z, double* d_vx,
+                      double* d_vy, double* d_vz, double* d_diam, int64_t* d_id)
+{
+    if (!h) return LCS_ERR_INVALID_ARG;
+    OutPtrs O;
+    O.f[0] = d_x; O.f[1] = d_y; O.f[2] = d_z; O.f[3] = d_vx; O.f[4] = d_vy; O.f[5] = d_vz; O.f[6] = d_diam;
+    O.id = d_id; O.code = nullptr;
+    return copy_out(h, d_counts, O);
+}
+
+int lcs_get_codes(lcs_t* h, uint8_t* d_codes)
+{
+    if (!h || !d_codes) return LCS_ERR_INVALID_ARG;
+    OutPtrs O;
+    for (int a = 0; a < 7; ++a) O.f[a] = nullptr;
+    O.id = nullptr; O.code = d_codes;
+    return copy_out(h, nullptr, O);
+}
+
+int lcs_get_count_table(lcs_t* h, int64_t* d_table)
+{
+    if (!h || !d_table) return LCS_ERR_INVALID_ARG;
+    const int n = h->G.P * kNC;
+    k_table_out<<<(n + 255) / 256, 256, 0, h->stream>>>(h->G, h->T, d_table, h->pushed ? 1 : 0);
+    return check_launch(h);
+}
+
+int lcs_get_status(lcs_t* h, int* sticky_error, int64_t* n_total, int64_t* n_migrated_last)
+{
+    if (!h) return LCS_ERR_INVALID_ARG;
+    struct { int status; unsigned long long mig, tot; } host;
+    if (cudaMemcpyAsync(&host.status, h->T.status, sizeof(int), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaMemcpyAsync(&host.mig, h->T.n_migrated, 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaMemcpyAsync(&host.tot, h->T.n_total, 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaStreamSynchronize(h->stream) != cudaSuccess) {
+        return LCS_ERR_CUDA;
+    }
+    h->sticky = host.status;
+    if (sticky_error) *sticky_error = host.status;
+    if (n_total) *n_total = (int64_t)host.tot;
+    if (n_migrated_last) *n_migrated_last = (int64_t)host.mig;
+    return host.status;
+}
+
+int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8], void* const h_out[8],
+                        int64_t* h_counts, void* d_staging, size_t staging_bytes)
+{
+    if (!h || !h_in || !h_out || !h_counts || !d_staging || n < 0) return LCS_ERR_INVALID_ARG;
+    const size_t arr = align_up((size_t)n * 8);
+    if (staging_bytes < 8 * arr + align_up((size_t)h->G.P * 8)) return LCS_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(d_staging) % kAlign) return LCS_ERR_INVALID_ARG;
+    char* st = static_cast<char*>(d_staging);
+    for (int a = 0; a < 8; ++a) {
+        if (!h_in[a] || !h_out[a]) return LCS_ERR_INVALID_ARG;
+        if (cudaMemcpyAsync(st + a * arr, h_in[a], (size_t)n * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+            return LCS_ERR_CUDA;
+    }
+    double* f[7];
+    for (int a = 0; a < 7; ++a) f[a] = reinterpret_cast<double*>(st + a * arr);
+    int64_t* ids = reinterpret_cast<int64_t*>(st + 7 * arr);
+    int64_t* d_counts = reinterpret_cast<int64_t*>(st + 8 * arr);
+    int rc = lcs_set_particles(h, n, f[0], f[1], f[2], f[3], f[4], f[5], f[6], ids);
+    if (rc) return rc;
+    rc = lcs_step_fused(h, dt);
+    if (rc) return rc;
+    rc = lcs_get_particles(h, d_counts, f[0], f[1], f[2], f[3], f[4], f[5], f[6], ids);
+    if (rc) return rc;
+    for (int a = 0; a < 8; ++a)
+        if (cudaMemcpyAsync(h_out[a], st + a * arr, (size_t)n * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
+            return LCS_ERR_CUDA;
+    if (cudaMemcpyAsync(h_counts, d_counts, (size_t)h->G.P * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
+        return LCS_ERR_CUDA;
+    return lcs_get_status(h, nullptr, nullptr, nullptr);
+}
+
+int64_t lcs_kernel_launches(lcs_t* h) { return h ? h->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,282 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the oracle, element by element on
+the same seeded inputs.  Bit-exact for ids / order / counts / codes; |dx| <= 1e-12*L and
+|dv| <= 1e-12*max(|v|,1) for state (north_star) -- and, because the push is specified to be
+bit-reproducible, the maximum ulp distance is asserted to be 0 as well."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+L = 6.283185307179586
+F7 = ("x", "y", "z", "vx", "vy", "vz", "d")
+F8 = F7 + ("id",)
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("a CUDA device is required for -m gpu tests (no CPU fallback exists)")
+    return torch
+
+
+def to_dev(torch, arrs):
+    return {k: torch.from_numpy(np.ascontiguousarray(v)).cuda() for k, v in arrs.items()}
+
+
+def to_np(d):
+    return {k: v.cpu().numpy() for k, v in d.items()}
+
+
+def ulps(a, b):
+    return int(np.max(np.abs(a.view(np.int64) - b.view(np.int64)))) if a.size else 0
+
+
+def assert_state_close(got, want, tag=""):
+    for k in ("x", "y", "z"):
+        d = np.abs(got[k] - want[k])
+        assert d.size == 0 or np.max(d) <= 1e-12 * L, (tag, k, np.max(d))
+    for k in ("vx", "vy", "vz"):
+        d = np.abs(got[k] - want[k])
+        assert d.size == 0 or np.all(d <= 1e-12 * np.maximum(np.abs(want[k]), 1.0)), (tag, k)
+    for k in F7:
+        assert ulps(got[k], want[k]) == 0, (tag, k, "ulp distance", ulps(got[k], want[k]))
+
+
+def make_pair(torch, oracle_lib, N, P, cap, fluid, parts, g=(0.0, 0.0, 0.0), rho=1000.0, send_capacity=0):
+    from paper_2604_11008_b200 import LCS
+    o = oracle_lib.Oracle(N, *P, cap, g=g, rho_ratio=rho)
+    o.set_fluid(*fluid)
+    rc = o.set_particles(*(parts[k] for k in F8))
+    dev = LCS(N, *P, cap, g=g, rho_ratio=rho, send_capacity=send_capacity)
+    df = [torch.from_numpy(np.ascontiguousarray(f, dtype=np.float64)).cuda() for f in fluid]
+    dev.set_fluid(*df)
+    dp = to_dev(torch, parts)
+    dev.set_particles(*(dp[k] for k in F8))
+    return o, dev, rc
+
+
+def random_parts(rng, n, vmax, d=1.0):
+    X = rng.random((3, n)) * L
+    X = np.minimum(X, np.nextafter(L, 0.0))
+    V = (rng.random((3, n)) * 2 - 1) * np.asarray(vmax).reshape(-1, 1)
+    return {"x": X[0], "y": X[1], "z": X[2], "vx": V[0], "vy": V[1], "vz": V[2],
+            "d": np.full(n, d) if np.isscalar(d) else d, "id": rng.permutation(n).astype(np.int64) + 7}
+
+
+def compare_packed(dev, o, tag=""):
+    got = to_np(dev.get_particles())
+    want = o.get_particles()
+    assert np.array_equal(got["counts"], want["counts"]), tag
+    assert np.array_equal(got["id"], want["id"]), tag
+    assert np.array_equal(got["d"], want["d"]), tag
+    assert_state_close(got, want, tag)
+    return got, want
+
+
+# ------------------------------------------------------------------------------------------------
+def test_set_particles_bins_stably(torch_cuda, oracle_lib):
+    rng = np.random.default_rng(0)
+    N, P = 16, (2, 3, 2)
+    N = 24
+    for n in (0, 1, 2, 511, 513, 5000, 20011):
+        parts = random_parts(rng, n, [1, 1, 1])
+        z = np.zeros(N ** 3)
+        o, dev, rc = make_pair(torch_cuda, oracle_lib, N, P, 4096, (z, z, z), parts)
+        assert rc == 0
+        st = dev.get_status()
+        assert st[0] == 0 and st[1] == n
+        compare_packed(dev, o, f"n={n}")
+        assert np.all(dev.get_codes().cpu().numpy() == 13)
+        tab = dev.get_count_table().cpu().numpy()
+        assert np.array_equal(tab, o.cnt_table())
+        dev.close()
+
+
+@pytest.mark.parametrize("name", ["Tiny"])
+def test_config_lockstep_P1_and_free_running_P2(torch_cuda, oracle_lib, name):
+    from workloads import gen
+    cfg = gen.get_config(name)
+    wl = gen.make_workload(cfg)
+    fluid = [wl[k].numpy() for k in "uvw"]
+    parts = {k: v.numpy() for k, v in wl["particles"].items()}
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, cfg["N"], cfg["P"], cfg["capacity"], fluid, parts, g=cfg["g"])
+    assert rc == 0
+    o_free = oracle_lib.Oracle(cfg["N"], *cfg["P"], cfg["capacity"], g=cfg["g"])
+    o_free.set_fluid(*fluid)
+    o_free.set_particles(*(parts[k] for k in F8))
+    for step in range(cfg["steps"]):
+        # P1: both start from the same state
+        dev.particle_step(cfg["dt"])
+        assert o.push(cfg["dt"]) == 0
+        got, want = compare_packed(dev, o, f"push {step}")
+        codes = dev.get_codes().cpu().numpy()
+        assert np.array_equal(codes, want["code"])
+        assert np.array_equal(dev.get_count_table().cpu().numpy(), o.cnt_table())
+        # oracle migrate on the GPU's post-push arrays must equal the GPU's migrate bit for bit
+        o2 = oracle_lib.Oracle(cfg["N"], *cfg["P"], cfg["capacity"], g=cfg["g"])
+        o2.load_packed(got["counts"], *(got[k] for k in F8), codes)
+        assert o2.migrate() == 0
+        dev.migrate()
+        e, n_tot, n_mig = dev.get_status()
+        assert e == 0 and n_tot == cfg["n"] and n_mig == o2.n_migrated_last
+        g2 = to_np(dev.get_particles())
+        w2 = o2.get_particles()
+        for k in F8 + ("counts",):
+            assert np.array_equal(g2[k], w2[k]), (step, k)
+        assert o.migrate() == 0
+        assert o_free.step(cfg["dt"]) == 0
+    # P2: the free-running oracle ends in the same state as the GPU
+    compare_packed(dev, o_free, "free running")
+    dev.close()
+
+
+@pytest.mark.parametrize("P,N", [((2, 2, 2), 16), ((3, 3, 3), 24), ((1, 2, 3), 12), ((1, 1, 1), 8), ((4, 2, 1), 16)])
+def test_fused_and_unfused_match_oracle_ballistic(torch_cuda, oracle_lib, P, N):
+    rng = np.random.default_rng(P[0] * 100 + N)
+    nP = P[0] * P[1] * P[2]
+    n = 3000 * nP + 17
+    Ls = np.array([L / P[0], L / P[1], L / P[2]])
+    parts = random_parts(rng, n, 0.45 * Ls)
+    z = np.zeros(N ** 3)
+    cap = 2 * (int(1.5 * n / nP) // 2 + 200)
+    o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, cap, (z, z, z), parts)
+    _, dev2, _ = make_pair(torch_cuda, oracle_lib, N, P, cap, (z, z, z), parts)
+    for step in range(3):
+        assert o.step(0.7) == 0
+        dev.step_fused(0.7)
+        dev2.particle_step(0.7)
+        dev2.migrate()
+        e, n_tot, n_mig = dev.get_status()
+        assert (e, n_tot, n_mig) == (0, n, o.n_migrated_last)
+        assert dev2.get_status() == (0, n, o.n_migrated_last)
+        compare_packed(dev, o, f"fused step {step}")
+        compare_packed(dev2, o, f"unfused step {step}")
+    dev.close(); dev2.close()
+
+
+def test_all_27_codes_hand_placed(torch_cuda, oracle_lib):
+    for P in [(3, 3, 3), (2, 2, 2), (1, 2, 3), (1, 1, 1)]:
+        N = 24
+        Ls = [L / P[0], L / P[1], L / P[2]]
+        X, V, want_code = [], [], []
+        for s in range(P[0] * P[1] * P[2]):
+            pc = (s % P[0], (s // P[0]) % P[1], s // (P[0] * P[1]))
+            for c in range(27):
+                dd = (c % 3 - 1, (c // 3) % 3 - 1, c // 9 - 1)
+                X.append([(pc[a] + 0.5) * Ls[a] for a in range(3)])
+                V.append([dd[a] * 0.75 * Ls[a] for a in range(3)])
+                want_code.append(c)
+        X, V = np.array(X).T, np.array(V).T
+        n = X.shape[1]
+        parts = {"x": X[0], "y": X[1], "z": X[2], "vx": V[0], "vy": V[1], "vz": V[2],
+                 "d": np.full(n, 1.0), "id": np.arange(n, dtype=np.int64)}
+        z = np.zeros(N ** 3)
+        o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, 64, (z, z, z), parts)
+        dev.particle_step(1.0)
+        codes = dev.get_codes().cpu().numpy()
+        assert np.array_equal(codes, np.array(want_code, dtype=np.uint8))
+        assert np.all(dev.get_count_table().cpu().numpy() == 1)
+        dev.migrate()
+        assert o.step(1.0) == 0
+        compare_packed(dev, o, str(P))
+        dev.close()
+
+
+def test_edge_cases(torch_cuda, oracle_lib):
+    N, P = 16, (2, 2, 2)
+    z = np.zeros(N ** 3)
+    rng = np.random.default_rng(5)
+    # zero migrants, then everybody migrates (+x), odd counts and ragged tiles
+    for vx, n in ((0.0, 4097), (L / 2, 4097), (L / 2, 3)):
+        parts = random_parts(rng, n, [0, 0, 0])
+        parts["vx"][:] = vx
+        o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, 2048, (z, z, z), parts)
+        for _ in range(2):
+            dev.step_fused(1.0)
+            assert o.step(1.0) == 0
+        assert dev.get_status() == (0, n, n if vx else 0)
+        compare_packed(dev, o)
+        dev.close()
+    # empty box
+    parts = random_parts(rng, 0, [0, 0, 0])
+    o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, 64, (z, z, z), parts)
+    dev.step_fused(1.0)
+    dev.particle_step(1.0); dev.migrate()
+    assert dev.get_status() == (0, 0, 0)
+    dev.close()
+
+
+def test_sticky_errors(torch_cuda, oracle_lib):
+    from paper_2604_11008_b200 import LCS, LcsError, LCS_ERR_CAPACITY, LCS_ERR_JUMP, LCS_ERR_RANGE, LCS_ERR_STATE
+    N, P = 16, (4, 4, 4)
+    z = np.zeros(N ** 3)
+    one = lambda **kw: {**{"x": np.array([1.0]), "y": np.array([1.0]), "z": np.array([1.0]), "vx": np.array([0.0]),
+                           "vy": np.array([0.0]), "vz": np.array([0.0]), "d": np.array([1.0]),
+                           "id": np.array([0], dtype=np.int64)}, **kw}
+    # jump: more than one subdomain in one step
+    o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, 16, (z, z, z), one(vx=np.array([L / 4 * 1.6])))
+    dev.step_fused(1.0)
+    assert dev.get_status()[0] == LCS_ERR_JUMP and o.step(1.0) == oracle_lib.ERR_JUMP
+    with pytest.raises(LcsError):
+        dev.step_fused(1.0)
+    dev.close()
+    # non-finite
+    o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, 16, (z, z, z), one(vx=np.array([np.nan])))
+    dev.particle_step(1.0)
+    assert dev.get_status()[0] == LCS_ERR_JUMP
+    dev.close()
+    # range
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, N, P, 16, (z, z, z), one(x=np.array([L])))
+    assert rc == oracle_lib.ERR_RANGE and dev.get_status()[0] == LCS_ERR_RANGE
+    dev.close()
+    # capacity at set_particles and at migrate
+    n = 10
+    parts = {"x": np.concatenate([np.full(5, 1.0), np.full(5, 4.0)]), "y": np.ones(n), "z": np.ones(n),
+             "vx": np.concatenate([np.full(5, 3.0), np.zeros(5)]), "vy": np.zeros(n), "vz": np.zeros(n),
+             "d": np.ones(n), "id": np.arange(n, dtype=np.int64)}
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, 8, (2, 1, 1), 6, (np.zeros(512),) * 3, parts)
+    assert rc == 0
+    dev.step_fused(1.0)
+    assert dev.get_status()[0] == LCS_ERR_CAPACITY and o.step(1.0) == oracle_lib.ERR_CAPACITY
+    dev.close()
+    crowded = dict(parts, x=np.concatenate([np.full(8, 1.0), np.full(2, 4.0)]))   # 8 > 6 in slab 0
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, 8, (2, 1, 1), 6, (np.zeros(512),) * 3, crowded)
+    assert rc == oracle_lib.ERR_CAPACITY and dev.get_status()[0] == LCS_ERR_CAPACITY
+    dev.close()
+    with pytest.raises(LcsError):      # more particles than slots is a host-side argument error
+        make_pair(torch_cuda, oracle_lib, 8, (2, 1, 1), 4, (np.zeros(512),) * 3, parts)
+    # send region overflow: 5 migrants, send_capacity 4
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, 8, (2, 1, 1), 16, (np.zeros(512),) * 3, parts, send_capacity=4)
+    dev.step_fused(1.0)
+    assert dev.get_status()[0] == LCS_ERR_CAPACITY
+    dev.close()
+    # migrate without a step; invalid arguments
+    o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, 16, (z, z, z), one())
+    with pytest.raises(LcsError) as ei:
+        dev.migrate()
+    assert ei.value.code == LCS_ERR_STATE
+    dev.close()
+    with pytest.raises(LcsError):
+        LCS(15, 2, 2, 2, 16)          # N not divisible
+    with pytest.raises(LcsError):
+        LCS(16, 2, 2, 2, 15)          # odd capacity
+
+
+def test_medium_shape_sample(torch_cuda, oracle_lib):
+    """Medium's recipe (gravity on, 4x4x4, 128^3 field, lognormal radii) at 1/8 of the particles."""
+    from workloads import gen
+    cfg = gen.scaled_config(gen.get_config("Medium"), n=262144)
+    wl = gen.make_workload(cfg, device="cuda")
+    fluid = [wl[k].cpu().numpy() for k in "uvw"]
+    parts = {k: v.cpu().numpy() for k, v in wl["particles"].items()}
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, cfg["N"], cfg["P"], cfg["capacity"], fluid, parts, g=cfg["g"])
+    assert rc == 0
+    for step in range(5):
+        dev.step_fused(cfg["dt"])
+        assert o.step(cfg["dt"]) == 0
+        assert dev.get_status() == (0, cfg["n"], o.n_migrated_last)
+    compare_packed(dev, o, "medium sample")
+    frac = o.n_migrated_last / cfg["n"]
+    assert 0.02 < frac < 0.09
+    dev.close()
