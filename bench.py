@@ -1,0 +1,311 @@
+#!/usr/bin/env python
+"""bench.py -- particles/s of the fused push + prefix-scan migrate step (BASELINE.json's metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload Large] [--impl reference]
+
+One "step" = one lcs_step_fused over all resident particles of the workload (all of SURVEY.md
+section 8(a): gather, advance, classify, count, scan, pack, compaction, unpack).  At N > 1 every
+rank owns an independent periodic box of the same workload (weak scaling, no data-path collective;
+DESIGN.md section 8).  Prints ONE JSON line on rank 0.
+
+--impl reference times the oracle (oracle/, the plain sequential CPU statement of the same path)
+on a bounded sample of the same workload on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "particles/s (fused push + prefix-scan migrate step)"
+F8 = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
+
+
+def measured_peak_hbm():
+    """(GB/s, source): MEASURED_PEAKS.json if present, else the fallback of B200_PROFILING.md."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            t = [c.strip() for c in line.split(",")]
+            if len(t) < 7:
+                continue
+            try:
+                sm.append(float(t[0])); mx.append(float(t[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, t[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(np.max(mx)), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def pick_device():
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return torch, rank, world, local
+
+
+def build_workload(name, device):
+    from workloads import gen
+    cfg = gen.get_config(name)
+    wl = gen.make_workload(cfg, device=device)
+    return cfg, wl
+
+
+def oracle_sample_rate(cfg, wl, stride, steps, torch):
+    """Oracle (as it stands, single thread) on every `stride`-th particle of the workload with the
+    full fluid field; -> (particles/s, seconds per step, sample size)."""
+    from oracle import oracle as orc
+    fluid = [wl[k].cpu().numpy() for k in "uvw"]
+    parts = {k: wl["particles"][k][::stride].contiguous().cpu().numpy() for k in F8}
+    n_s = parts["id"].size
+    P = cfg["P"][0] * cfg["P"][1] * cfg["P"][2]
+    cap = int(max(64, 2 * np.ceil(1.5 * n_s / P / 2) + 64))
+    if cfg.get("clumps"):
+        cap = int(max(cap, 2 * np.ceil(cfg["capacity"] / stride * 1.5 / 2) + 64))
+    o = orc.Oracle(cfg["N"], *cfg["P"], cap, g=cfg["g"])
+    o.set_fluid(*fluid)
+    rc = o.set_particles(*(parts[k] for k in F8))
+    if rc:
+        raise RuntimeError(f"oracle set_particles -> {rc}")
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        rc = o.step(cfg["dt"])
+        if rc:
+            raise RuntimeError(f"oracle step -> {rc}")
+    dt = time.perf_counter() - t0
+    o.close()
+    return n_s * steps / dt, dt / steps, n_s
+
+
+def run_reference(args):
+    torch, rank, world, local = pick_device()
+    if rank != 0:
+        return 0
+    dev = "cuda:0" if torch.cuda.is_available() else "cpu"   # the harness may synthesise inputs on a GPU
+    cfg, wl = build_workload(args.workload, dev)
+    stride = max(1, cfg["n"] // args.ref_sample)
+    # untimed warm-up then K timed steps, each a bounded sample of the workload
+    oracle_sample_rate(cfg, wl, stride * 8, max(1, min(args.warmup, 1)), torch)
+    rate, sec, n_s = oracle_sample_rate(cfg, wl, stride, args.steps, torch)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": "particles/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "N": cfg["N"], "P": cfg["P"], "particles": cfg["n"], "dt": cfg["dt"]},
+        "cpu_baseline": {"value": rate, "unit": "particles/s", "cores": 1, "kind": "oracle",
+                         "sample": f"every {stride}th particle of {cfg['name']} ({n_s} particles, full {cfg['N']}^3 field), "
+                                   f"{args.steps} steps, single thread"},
+        "e2e": {"value": rate, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_cuda(args):
+    torch, rank, world, local = pick_device()
+    if not torch.cuda.is_available():
+        print("bench.py: no CUDA device; the CUDA path has no CPU fallback", file=sys.stderr)
+        return 2
+    from paper_2604_11008_b200 import LCS
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    cfg, wl = build_workload(args.workload, dev)
+    n, N = cfg["n"], cfg["N"]
+    P = cfg["P"][0] * cfg["P"][1] * cfg["P"][2]
+    lcs = LCS(N, *cfg["P"], cfg["capacity"], g=cfg["g"], device=dev)
+    lcs.set_fluid(wl["u"], wl["v"], wl["w"])
+    parts = wl["particles"]
+    lcs.set_particles(*(parts[k] for k in F8))
+    err, n_tot, _ = lcs.get_status()
+    if err or n_tot != n:
+        print(f"bench.py: set_particles failed: status {err}, total {n_tot}", file=sys.stderr)
+        return 3
+    dt = cfg["dt"]
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        lcs.step_fused(dt)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    launches0 = lcs.kernel_launches
+    lcs.profile_begin(args.steps)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        lcs.step_fused(dt)
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    prof = lcs.profile_end()
+    launches = lcs.kernel_launches - launches0
+    clocks = sampler.stop() if sampler else None
+    err, n_tot, n_mig = lcs.get_status()
+    if err or n_tot != n:
+        print(f"bench.py: step failed: sticky status {err}, total {n_tot}", file=sys.stderr)
+        return 3
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * n * args.steps / (ms_total * 1e-3)
+    m = n_mig / n
+
+    # ---- end to end through the host-buffer entry point (rank-local, then max over ranks) ----------
+    e2e = None
+    if args.e2e_steps > 0:
+        state = lcs.get_particles(n)
+        h_in = {k: torch.empty(n, dtype=state[k].dtype, pin_memory=True) for k in F8}
+        h_out = {k: torch.empty(n, dtype=state[k].dtype, pin_memory=True) for k in F8}
+        h_counts = torch.empty(P, dtype=torch.int64, pin_memory=True)
+        for k in F8:
+            h_in[k].copy_(state[k])
+        del state
+        staging = torch.empty(64 * n + 8 * P + 16384, dtype=torch.uint8, device=dev)
+        lcs.step_fused_host(dt, h_in, h_out, h_counts, staging)       # warm-up
+        barrier()
+        t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+        t0.record()
+        src, dst = h_in, h_out
+        for _ in range(args.e2e_steps):
+            lcs.step_fused_host(dt, src, dst, h_counts, staging)      # synchronises: result is on the host
+            src, dst = dst, src
+        t1.record()
+        barrier()
+        ms_e2e = t0.elapsed_time(t1)
+        if dist is not None:
+            t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e2e = float(t.item())
+        assert int(h_counts.sum()) == n
+        e2e = {"value": world * n * args.e2e_steps / (ms_e2e * 1e-3), "unit": "particles/s",
+               "h2d_bytes_per_step": 64 * n, "d2h_bytes_per_step": 64 * n + 8 * P,
+               "steps": args.e2e_steps, "ms_per_step": ms_e2e / args.e2e_steps,
+               "call": "lcs_step_fused_host (pinned host particle arrays in/out; fluid field resident)"}
+        del staging, h_in, h_out
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (k_tile_pass<fused>) ---------------------------------------
+    peak, peak_src = measured_peak_hbm()
+    alg_bytes = 128.0 * n + 24.0 * N ** 3            # R64 + W64 per particle + the compulsory grid read
+    tile_ms = prof["tile_pass_ms"] / max(prof["steps"], 1)
+    achieved = alg_bytes / (tile_ms * 1e-3) / 1e9
+    step_bytes = n * (128.0 + 128.0 * m) + 24.0 * N ** 3
+    roofline = {"bound": "hbm", "kernel": "k_tile_pass<fused>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": args.traffic_bytes, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": tile_ms,
+                "kernel_share_of_step": tile_ms / ms_step,
+                "table_ms": prof["table_ms"] / max(prof["steps"], 1),
+                "unpack_ms": prof["unpack_ms"] / max(prof["steps"], 1),
+                "step_algorithmic_GBps": step_bytes / (ms_step * 1e-3) / 1e9,
+                "step_frac_of_measured_peak": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
+                "step_frac_of_nominal_8TBps": step_bytes / (ms_step * 1e-3) / 1e9 / 8000.0}
+
+    # ---- the oracle on the host cores, bounded sample ---------------------------------------------
+    cpu = None
+    if args.cpu_sample > 0:
+        stride = max(1, n // args.cpu_sample)
+        rate, sec, n_s = oracle_sample_rate(cfg, wl, stride, 2, torch)
+        cpu = {"value": rate, "unit": "particles/s", "cores": 1, "kind": "oracle",
+               "sample": f"every {stride}th particle of {cfg['name']} ({n_s} particles, full {N}^3 field), 2 steps, "
+                         f"single thread of {os.cpu_count()} host cores"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "N": N, "P": cfg["P"], "particles_per_gpu": n, "capacity": cfg["capacity"],
+                   "dt": dt, "migrant_fraction_last_step": m, "l2": "inputs larger than L2 (no flush)",
+                   "parallelism": "independent box per GPU" if world > 1 else "single GPU"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="Large")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-sample", type=int, default=1 << 22, help="particles in the oracle's timed sample (0 = skip)")
+    ap.add_argument("--ref-sample", type=int, default=1 << 21, help="--impl reference: particles per timed step")
+    ap.add_argument("--traffic-bytes", type=float, default=None,
+                    help="ncu dram bytes per launch of the dominant kernel (from profiles/), reported as roofline.traffic")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

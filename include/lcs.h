@@ -67,8 +67,9 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
                void* d_workspace, size_t workspace_bytes, void* cuda_stream, lcs_t** out);
 int lcs_destroy(lcs_t* h);
 
-/* Fluid velocity on the N^3 cell centres.  The three pointers are borrowed read-only (zero-copy)
- * until the next lcs_set_fluid or lcs_destroy.  PAPER.md:64. */
+/* Fluid velocity on the N^3 cell centres.  The three arrays are read once, at call
+ * time in stream order, and repacked into the workspace as one 32-byte (u,v,w,0) record per cell
+ * (one L2 sector per stencil corner); the caller may reuse them once the call's work has run. */
 int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* d_w);
 
 /* Load n particles given in any order; they are binned stably (input order kept inside each
@@ -122,6 +123,15 @@ int lcs_get_status(lcs_t* h, int* sticky_error, int64_t* n_total, int64_t* n_mig
  * h_out arrays need room for n).  d_staging: device scratch of at least 64*n + 8*P bytes. */
 int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8], void* const h_out[8],
                         int64_t* h_counts, void* d_staging, size_t staging_bytes);
+
+/* Optional per-kernel timing for benchmarks.  lcs_profile_begin creates CUDA events (no device
+ * memory) and makes every following lcs_step_fused / lcs_migrate record four of them on the
+ * handle's stream: before the tile pass, after it, after the table scan, after unpack + commit.
+ * At most max_steps steps are recorded; later steps run untimed.  lcs_profile_end synchronises the
+ * stream, returns the summed durations in milliseconds and the number of recorded steps, and
+ * destroys the events.  Any out pointer may be NULL. */
+int lcs_profile_begin(lcs_t* h, int max_steps);
+int lcs_profile_end(lcs_t* h, double* ms_tile_pass, double* ms_table, double* ms_unpack, int* n_steps);
 
 /* Number of kernels this library has launched on the handle since create (for bench accounting). */
 int64_t lcs_kernel_launches(lcs_t* h);

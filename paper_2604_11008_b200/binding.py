@@ -12,7 +12,7 @@ EXPORTED_SYMBOLS = (
     "lcs_workspace_bytes", "lcs_create", "lcs_destroy", "lcs_set_fluid", "lcs_set_particles",
     "lcs_particle_step", "lcs_migrate", "lcs_step_fused", "lcs_get_counts", "lcs_get_particles",
     "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_step_fused_host",
-    "lcs_kernel_launches", "lcs_version")
+    "lcs_profile_begin", "lcs_profile_end", "lcs_kernel_launches", "lcs_version")
 
 FIELDS = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
 
@@ -65,6 +65,8 @@ def load_library(build_if_missing: bool = True):
     L.lcs_get_count_table.argtypes = [vp, vp]
     L.lcs_get_status.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(i64), C.POINTER(i64)]
     L.lcs_step_fused_host.argtypes = [vp, dbl, i64, C.POINTER(vp), C.POINTER(vp), vp, vp, C.c_size_t]
+    L.lcs_profile_begin.argtypes = [vp, C.c_int]
+    L.lcs_profile_end.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl), C.POINTER(C.c_int)]
     L.lcs_kernel_launches.restype = i64
     L.lcs_kernel_launches.argtypes = [vp]
     _lib = L
@@ -201,6 +203,15 @@ class LCS:
         rc = self._L.lcs_step_fused_host(self._h, float(dt), n, pin, pout, C.c_void_p(h_counts.data_ptr()),
                                          C.c_void_p(sp), sbytes)
         self._chk("lcs_step_fused_host", rc)
+
+    def profile_begin(self, max_steps):
+        self._chk("lcs_profile_begin", self._L.lcs_profile_begin(self._h, int(max_steps)))
+
+    def profile_end(self):
+        """-> dict(tile_pass_ms, table_ms, unpack_ms, steps): summed CUDA-event durations."""
+        a, b, c, n = C.c_double(), C.c_double(), C.c_double(), C.c_int()
+        self._chk("lcs_profile_end", self._L.lcs_profile_end(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(n)))
+        return {"tile_pass_ms": a.value, "table_ms": b.value, "unpack_ms": c.value, "steps": n.value}
 
     @property
     def kernel_launches(self):

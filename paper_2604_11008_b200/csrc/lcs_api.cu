@@ -7,7 +7,9 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
 #include <new>
+#include <vector>
 
 using namespace lcs;
 
@@ -16,7 +18,8 @@ struct lcs_handle {
     Slabs S, Snd;
     Tables T;
     cudaStream_t stream;
-    const double *fu, *fv, *fw;
+    double* fluid4;           // [N^3][4] repacked fluid (u,v,w,0), in the workspace
+    bool have_fluid;
     int64_t* prefix;          // [P+1] scratch for packed copy-out
     void* pool;               // send pool base (also scratch of lcs_set_particles)
     size_t pool_bytes;
@@ -25,6 +28,9 @@ struct lcs_handle {
     bool have_particles;
     int sticky;               // last sticky error seen by lcs_get_status
     int64_t launches;
+    std::vector<cudaEvent_t>* prof;   // 4 events per recorded step, or null
+    int prof_steps, prof_max;
+    int grid_fused, grid_pack;         // persistent grid sizes of the tile pass
 };
 
 namespace {
@@ -34,8 +40,8 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t slab_f[7], slab_id, slab_code;
-    size_t pool, pool_bytes;
-    size_t count, cnt, recv_off, new_count, desc, tile_excl, tile_cnt, misc, prefix;
+    size_t pool, pool_bytes, fluid4;
+    size_t count, cnt, recv_off, new_count, desc, tile_start, tile_excl, tile_cnt, misc, prefix;
     size_t total;
     int tiles_per_sub;
     int64_t send_cap;
@@ -58,7 +64,6 @@ bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* pr
 
 Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* prm)
 {
-    (void)N;
     Layout L;
     const size_t P = (size_t)Px * Py * Pz;
     const size_t slots = P * (size_t)cap;
@@ -75,11 +80,13 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     const size_t set_bytes = align_up(slots * 4) + align_up(set_tiles * P * 4);
     L.pool = off; L.pool_bytes = send_bytes > set_bytes ? send_bytes : set_bytes;
     off = align_up(off + L.pool_bytes);
+    L.fluid4 = off;    off = align_up(off + (size_t)N * N * N * 32);
     L.count = off;     off = align_up(off + P * 4);
     L.cnt = off;       off = align_up(off + P * 32 * 4);
     L.recv_off = off;  off = align_up(off + P * 32 * 4);
     L.new_count = off; off = align_up(off + P * 4);
-    L.desc = off;      off = align_up(off + ntiles * 32 * 8);
+    L.desc = off;      off = align_up(off + ntiles * 2 * 8);
+    L.tile_start = off; off = align_up(off + (P + 1) * 4);
     L.tile_excl = off; off = align_up(off + ntiles * 32 * 4);
     L.tile_cnt = off;  off = align_up(off + ntiles * 32 * 4);
     L.misc = off;      off = align_up(off + 256);
@@ -87,6 +94,8 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     L.total = off;
     return L;
 }
+
+inline size_t tile_pass_smem(int P) { return 2 * sizeof(TileBuf) + (size_t)(P + 1) * sizeof(uint32_t); }
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -99,18 +108,25 @@ inline int check_launch(lcs_t* h, int n = 1)
 int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
 {
     const Geom& G = h->G;
-    const unsigned ntiles = (unsigned)G.P * (unsigned)G.tiles_per_sub;
     h->epoch = (h->epoch + 1u) & 0x3fffffffu;
     if (h->epoch == 0u) h->epoch = 1u;
+    const bool rec = h->prof && h->prof_steps < h->prof_max;
+    cudaEvent_t* ev = rec ? h->prof->data() + 4 * h->prof_steps : nullptr;
+    if (rec) cudaEventRecord(ev[0], h->stream);
+    const size_t smem = tile_pass_smem(G.P);
     if (fused)
-        k_tile_pass<true><<<ntiles, kBlock, 0, h->stream>>>(G, h->S, h->Snd, h->T, h->fu, h->fv, h->fw, dt, h->epoch, 0ull);
+        k_tile_pass<true><<<h->grid_fused, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch, 0ull);
     else
-        k_tile_pass<false><<<ntiles, kBlock, 0, h->stream>>>(G, h->S, h->Snd, h->T, h->fu, h->fv, h->fw, dt, h->epoch, 0ull);
+        k_tile_pass<false><<<h->grid_pack, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch, 0ull);
+    if (rec) cudaEventRecord(ev[1], h->stream);
+    k_code_scan<<<G.P, 256, 0, h->stream>>>(G, h->T);
     k_table<<<1, 256, 0, h->stream>>>(G, h->T);
+    if (rec) cudaEventRecord(ev[2], h->stream);
     k_unpack<<<dim3(G.tiles_per_sub, G.P), kUnpackBlock, 0, h->stream>>>(G, h->S, h->Snd, h->T);
-    k_commit_counts<<<(G.P + 255) / 256, 256, 0, h->stream>>>(G, h->T);
+    k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, 1);
+    if (rec) { cudaEventRecord(ev[3], h->stream); ++h->prof_steps; }
     h->pushed = false;
-    return check_launch(h, 4);
+    return check_launch(h, 5);
 }
 
 }  // namespace
@@ -136,7 +152,7 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     if (workspace_bytes < L.total) return LCS_ERR_INVALID_ARG;
     lcs_t* h = new (std::nothrow) lcs_handle();
     if (!h) return LCS_ERR_CUDA;
-    std::memset(h, 0, sizeof(*h));
+    std::memset(static_cast<void*>(h), 0, sizeof(*h));
     Geom& G = h->G;
     G.N = N; G.Px = Px; G.Py = Py; G.Pz = Pz; G.P = Px * Py * Pz;
     G.nx = N / Px; G.ny = N / Py; G.nz = N / Pz;
@@ -158,11 +174,13 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     for (int a = 0; a < 7; ++a) h->Snd.f[a] = reinterpret_cast<double*>(w + L.pool + a * send_arr);
     h->Snd.id = reinterpret_cast<int64_t*>(w + L.pool + 7 * send_arr);
     h->Snd.code = nullptr;
+    h->fluid4 = reinterpret_cast<double*>(w + L.fluid4);
     h->T.count = reinterpret_cast<uint32_t*>(w + L.count);
     h->T.cnt = reinterpret_cast<uint32_t*>(w + L.cnt);
     h->T.recv_off = reinterpret_cast<uint32_t*>(w + L.recv_off);
     h->T.new_count = reinterpret_cast<uint32_t*>(w + L.new_count);
     h->T.desc = reinterpret_cast<uint64_t*>(w + L.desc);
+    h->T.tile_start = reinterpret_cast<uint32_t*>(w + L.tile_start);
     h->T.tile_excl = reinterpret_cast<uint32_t*>(w + L.tile_excl);
     h->T.tile_cnt = reinterpret_cast<uint32_t*>(w + L.tile_cnt);
     h->T.ticket = reinterpret_cast<unsigned int*>(w + L.misc);
@@ -171,6 +189,20 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     h->T.n_total = reinterpret_cast<unsigned long long*>(w + L.misc + 48);
     h->prefix = reinterpret_cast<int64_t*>(w + L.prefix);
     h->stream = static_cast<cudaStream_t>(cuda_stream);
+    {   // persistent grids: one wave of resident CTAs
+        int dev = 0, sms = 0, occ_f = 0, occ_p = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const size_t smem = tile_pass_smem(G.P);
+        cudaFuncSetAttribute(k_tile_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(k_tile_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_tile_pass<true>, kBlock, smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, k_tile_pass<false>, kBlock, smem);
+        if (sms < 1) sms = 148;
+        const long long max_tiles = (long long)G.P * G.tiles_per_sub;
+        h->grid_fused = (int)std::min<long long>(max_tiles, (long long)sms * (occ_f > 0 ? occ_f : 1));
+        h->grid_pack = (int)std::min<long long>(max_tiles, (long long)sms * (occ_p > 0 ? occ_p : 1));
+    }
     // tables start at zero (epoch 0 is never published; counts empty)
     if (cudaMemsetAsync(w + L.count, 0, L.total - L.count, h->stream) != cudaSuccess) { delete h; return LCS_ERR_CUDA; }
     *out = h;
@@ -181,6 +213,7 @@ int lcs_destroy(lcs_t* h)
 {
     if (!h) return LCS_ERR_INVALID_ARG;
     cudaStreamSynchronize(h->stream);
+    if (h->prof) lcs_profile_end(h, nullptr, nullptr, nullptr, nullptr);
     delete h;
     return LCS_OK;
 }
@@ -189,8 +222,11 @@ int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* 
 {
     if (!h || !d_u || !d_v || !d_w) return LCS_ERR_INVALID_ARG;
     if (!aligned16(d_u) || !aligned16(d_v) || !aligned16(d_w)) return LCS_ERR_INVALID_ARG;
-    h->fu = d_u; h->fv = d_v; h->fw = d_w;
-    return LCS_OK;
+    const size_t ncell = (size_t)h->G.N * h->G.N * h->G.N;
+    const unsigned blocks = (unsigned)std::min<size_t>((ncell + 255) / 256, 148u * 16u);
+    k_repack_fluid<<<blocks, 256, 0, h->stream>>>(ncell, d_u, d_v, d_w, h->fluid4);
+    h->have_fluid = true;
+    return check_launch(h);
 }
 
 int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y, const double* d_z,
@@ -213,6 +249,7 @@ int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y,
     if (ntiles > 0)
         k_set_owner<<<ntiles, 256, (size_t)G.P * 4, h->stream>>>(G, h->T, n, d_x, d_y, d_z, owner, tilehist);
     k_set_scan<<<(G.P + 127) / 128, 128, 0, h->stream>>>(G, h->T, ntiles, tilehist, n);
+    k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, 0);
     if (ntiles > 0) {
         int wpb = (int)(32768 / ((size_t)G.P * 4));
         wpb = wpb < 1 ? 1 : (wpb > 4 ? 4 : wpb);
@@ -222,17 +259,17 @@ int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y,
         k_set_scatter<<<(ntiles + wpb - 1) / wpb, 32 * wpb, (size_t)wpb * G.P * 4, h->stream>>>(G, h->S, n, I, owner,
                                                                                                  tilehist, wpb);
     }
-    return check_launch(h, ntiles > 0 ? 3 : 1);
+    return check_launch(h, ntiles > 0 ? 4 : 2);
 }
 
 int lcs_particle_step(lcs_t* h, double dt)
 {
     if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
-    if (!h->fu || !h->have_particles) return LCS_ERR_STATE;
+    if (!h->have_fluid || !h->have_particles) return LCS_ERR_STATE;
     if (h->sticky) return h->sticky;
     const Geom& G = h->G;
     cudaMemsetAsync(h->T.cnt, 0, (size_t)G.P * 32 * 4, h->stream);
-    k_push<<<dim3(G.tiles_per_sub, G.P), kBlock, 0, h->stream>>>(G, h->S, h->T, h->fu, h->fv, h->fw, dt);
+    k_push<<<dim3(G.tiles_per_sub, G.P), kBlock, 0, h->stream>>>(G, h->S, h->T, h->fluid4, dt);
     h->pushed = true;
     return check_launch(h);
 }
@@ -248,7 +285,7 @@ int lcs_migrate(lcs_t* h)
 int lcs_step_fused(lcs_t* h, double dt)
 {
     if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
-    if (!h->fu || !h->have_particles) return LCS_ERR_STATE;
+    if (!h->have_fluid || !h->have_particles) return LCS_ERR_STATE;
     if (h->sticky) return h->sticky;
     return enqueue_tile_pass(h, true, dt);
 }
@@ -341,6 +378,39 @@ int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8
     if (cudaMemcpyAsync(h_counts, d_counts, (size_t)h->G.P * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
         return LCS_ERR_CUDA;
     return lcs_get_status(h, nullptr, nullptr, nullptr);
+}
+
+int lcs_profile_begin(lcs_t* h, int max_steps)
+{
+    if (!h || max_steps < 1 || max_steps > 4096) return LCS_ERR_INVALID_ARG;
+    if (h->prof) lcs_profile_end(h, nullptr, nullptr, nullptr, nullptr);
+    h->prof = new (std::nothrow) std::vector<cudaEvent_t>(4 * (size_t)max_steps);
+    if (!h->prof) return LCS_ERR_CUDA;
+    for (auto& e : *h->prof)
+        if (cudaEventCreate(&e) != cudaSuccess) return LCS_ERR_CUDA;
+    h->prof_steps = 0; h->prof_max = max_steps;
+    return LCS_OK;
+}
+
+int lcs_profile_end(lcs_t* h, double* ms_tile_pass, double* ms_table, double* ms_unpack, int* n_steps)
+{
+    if (!h || !h->prof) return LCS_ERR_STATE;
+    int rc = cudaStreamSynchronize(h->stream) == cudaSuccess ? LCS_OK : LCS_ERR_CUDA;
+    double acc[3] = {0.0, 0.0, 0.0};
+    for (int i = 0; i < h->prof_steps && rc == LCS_OK; ++i)
+        for (int k = 0; k < 3; ++k) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, (*h->prof)[4 * i + k], (*h->prof)[4 * i + k + 1]) != cudaSuccess) rc = LCS_ERR_CUDA;
+            acc[k] += ms;
+        }
+    if (ms_tile_pass) *ms_tile_pass = acc[0];
+    if (ms_table) *ms_table = acc[1];
+    if (ms_unpack) *ms_unpack = acc[2];
+    if (n_steps) *n_steps = h->prof_steps;
+    for (auto& e : *h->prof) cudaEventDestroy(e);
+    delete h->prof;
+    h->prof = nullptr; h->prof_steps = 0; h->prof_max = 0;
+    return rc;
 }
 
 int64_t lcs_kernel_launches(lcs_t* h) { return h ? h->launches : 0; }

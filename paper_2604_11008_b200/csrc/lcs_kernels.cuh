@@ -8,7 +8,14 @@
 
 namespace lcs {
 
-constexpr int kBlock = 256;            // threads per tile CTA
+#ifndef LCS_BLOCK
+#define LCS_BLOCK 256
+#endif
+#ifndef LCS_MIN_BLOCKS
+#define LCS_MIN_BLOCKS 2
+#endif
+constexpr int kBlock = LCS_BLOCK;      // threads per tile CTA
+constexpr int kMinBlocks = LCS_MIN_BLOCKS;   // CTAs per SM the tile pass is compiled for
 constexpr int kIpt = 2;                // particles per thread = one 128-bit load per field
 constexpr int kTile = kBlock * kIpt;   // particles per tile
 constexpr int kWarps = kBlock / 32;
@@ -36,7 +43,8 @@ struct Tables {
     uint32_t* cnt;                     // [P*32] per-(s,c) totals of the last step (27 used per row)
     uint32_t* recv_off;                // [P*32] slot in the receiver slab where segment (s,c) starts
     uint32_t* new_count;               // [P]
-    uint64_t* desc;                    // [P*tiles_per_sub*32] look-back descriptors
+    uint64_t* desc;                    // [P*tiles_per_sub*2] look-back descriptors: (stay, migrant) words
+    uint32_t* tile_start;              // [P+1] compact prefix of non-empty tiles per subdomain
     uint32_t* tile_excl;               // [P*tiles_per_sub*32] exclusive per-code prefix of each tile
     uint32_t* tile_cnt;                // [P*tiles_per_sub*32] per-code count of each tile
     unsigned int* ticket;              // tile ticket counter
@@ -113,16 +121,16 @@ __device__ __forceinline__ Axis stencil_axis(double a, double inv_dx, int N)
 
 __device__ __forceinline__ double lerp(double p, double q, double f) { return fma(f, q - p, p); }
 
-__device__ __forceinline__ double tri(const double* __restrict__ F, size_t r00, size_t r10, size_t r01,
-                                      size_t r11, int i0, int i1, double fx, double fy, double fz)
+// Fluid is held as one 32-byte record per cell: (u, v, w, 0) -- one L2 sector and one 256-bit load per
+// stencil corner instead of three scattered 8-byte loads.
+struct alignas(32) Cell { double u, v, w, pad; };
+
+__device__ __forceinline__ Cell ld_cell(const double* __restrict__ F4, size_t cell)
 {
-    const double a0 = __ldg(F + r00 + i0), a1 = __ldg(F + r00 + i1);
-    const double b0 = __ldg(F + r10 + i0), b1 = __ldg(F + r10 + i1);
-    const double c0 = __ldg(F + r01 + i0), c1 = __ldg(F + r01 + i1);
-    const double d0 = __ldg(F + r11 + i0), d1 = __ldg(F + r11 + i1);
-    const double c00 = lerp(a0, a1, fx), c10 = lerp(b0, b1, fx);
-    const double c01 = lerp(c0, c1, fx), c11 = lerp(d0, d1, fx);
-    return lerp(lerp(c00, c10, fy), lerp(c01, c11, fy), fz);
+    Cell r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
+                 : "=d"(r.u), "=d"(r.v), "=d"(r.w), "=d"(r.pad) : "l"(F4 + 4 * cell));
+    return r;
 }
 
 struct Particle { double x, y, z, vx, vy, vz, d; };
@@ -153,9 +161,8 @@ __device__ __forceinline__ int advance_axis(double& a, double& v, double U, doub
 }
 
 // a1-a3 for one particle.  Returns the destination code.
-__device__ __forceinline__ int push_particle(Particle& p, const double* __restrict__ u, const double* __restrict__ v,
-                                             const double* __restrict__ w, const Geom& G, const SubBox& B, double dt,
-                                             bool& jump)
+__device__ __forceinline__ int push_particle(Particle& p, const double* __restrict__ F4, const Geom& G,
+                                             const SubBox& B, double dt, bool& jump)
 {
     const Axis sx = stencil_axis(p.x, G.inv_dx, G.N);
     const Axis sy = stencil_axis(p.y, G.inv_dx, G.N);
@@ -163,9 +170,20 @@ __device__ __forceinline__ int push_particle(Particle& p, const double* __restri
     const size_t Ns = (size_t)G.N;
     const size_t r00 = Ns * (sy.i0 + Ns * sz.i0), r10 = Ns * (sy.i1 + Ns * sz.i0);
     const size_t r01 = Ns * (sy.i0 + Ns * sz.i1), r11 = Ns * (sy.i1 + Ns * sz.i1);
-    const double Ux = tri(u, r00, r10, r01, r11, sx.i0, sx.i1, sx.f, sy.f, sz.f);
-    const double Uy = tri(v, r00, r10, r01, r11, sx.i0, sx.i1, sx.f, sy.f, sz.f);
-    const double Uz = tri(w, r00, r10, r01, r11, sx.i0, sx.i1, sx.f, sy.f, sz.f);
+    double Ux, Uy, Uz;
+    {
+        const Cell a0 = ld_cell(F4, r00 + sx.i0), a1 = ld_cell(F4, r00 + sx.i1);
+        const Cell b0 = ld_cell(F4, r10 + sx.i0), b1 = ld_cell(F4, r10 + sx.i1);
+        const Cell c0 = ld_cell(F4, r01 + sx.i0), c1 = ld_cell(F4, r01 + sx.i1);
+        const Cell d0 = ld_cell(F4, r11 + sx.i0), d1 = ld_cell(F4, r11 + sx.i1);
+        // same lerp order as the definition: x, then y, then z
+        Ux = lerp(lerp(lerp(a0.u, a1.u, sx.f), lerp(b0.u, b1.u, sx.f), sy.f),
+                  lerp(lerp(c0.u, c1.u, sx.f), lerp(d0.u, d1.u, sx.f), sy.f), sz.f);
+        Uy = lerp(lerp(lerp(a0.v, a1.v, sx.f), lerp(b0.v, b1.v, sx.f), sy.f),
+                  lerp(lerp(c0.v, c1.v, sx.f), lerp(d0.v, d1.v, sx.f), sy.f), sz.f);
+        Uz = lerp(lerp(lerp(a0.w, a1.w, sx.f), lerp(b0.w, b1.w, sx.f), sy.f),
+                  lerp(lerp(c0.w, c1.w, sx.f), lerp(d0.w, d1.w, sx.f), sy.f), sz.f);
+    }
     const double tau = (G.K_tau * p.d) * p.d;     // tau_p = (rho_p/rho) d^2 / (18 nu)
     const double zz = dt / tau;
     const double alpha = exp_neg(zz);
@@ -224,11 +242,23 @@ __device__ __forceinline__ unsigned code_mask(const RowBallots& r, int c)
 }
 
 // ---------------------------------------------------------------------------------------------
+// K0: lcs_set_fluid -- repack the three x-fastest arrays into one (u,v,w,0) record per cell
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_repack_fluid(size_t ncell, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
+               double* __restrict__ F4)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncell; i += (size_t)gridDim.x * blockDim.x) {
+        const double4 r = make_double4(__ldcs(u + i), __ldcs(v + i), __ldcs(w + i), 0.0);
+        *reinterpret_cast<double4*>(F4 + 4 * i) = r;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // K1: unfused push (a1-a4).  One CTA per (subdomain, tile); in place; codes + count table.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kBlock)
-k_push(Geom G, Slabs S, Tables T, const double* __restrict__ fu, const double* __restrict__ fv,
-       const double* __restrict__ fw, double dt)
+k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
 {
     const int s = blockIdx.y;
     const int t = blockIdx.x;
@@ -250,8 +280,8 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ fu, const double* _
         for (int a = 0; a < 7; ++a) q[a] = ld_stream2(S.f[a] + base);
         Particle p0{q[0].x, q[1].x, q[2].x, q[3].x, q[4].x, q[5].x, q[6].x};
         Particle p1{q[0].y, q[1].y, q[2].y, q[3].y, q[4].y, q[5].y, q[6].y};
-        c0 = push_particle(p0, fu, fv, fw, G, B, dt, jump);
-        if (v1) c1 = push_particle(p1, fu, fv, fw, G, B, dt, jump);
+        c0 = push_particle(p0, F4, G, B, dt, jump);
+        if (v1) c1 = push_particle(p1, F4, G, B, dt, jump);
         double2 o;
         o = make_double2(p0.x, p1.x);   __stcs(reinterpret_cast<double2*>(S.f[0] + base), o);
         o = make_double2(p0.y, p1.y);   __stcs(reinterpret_cast<double2*>(S.f[1] + base), o);
@@ -276,151 +306,291 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ fu, const double* _
 
 // ---------------------------------------------------------------------------------------------
 // K2: tile pass of the migration (a5-a7), optionally with the push fused in front (a1-a4).
-//   - per-code stable ranks by single-pass decoupled look-back over the tiles of one subdomain,
-//     carried as a 27-vector (lane c of warp 0 owns code c);
-//   - stayers written in place at their compacted slot;
-//   - migrants written to the subdomain's send region, grouped by code inside the tile's chunk.
-// Tiles take their index from an atomic ticket so every predecessor is resident or finished.
+//   Persistent CTAs; each takes tiles from an atomic ticket (so every predecessor of a tile is
+//   resident or finished) and maps the ticket to (subdomain, tile) through the compact prefix
+//   tile_start[] (empty tiles never get a ticket).  Per tile:
+//   - in-tile per-code stable ranks from warp ballots (lane c owns code c);
+//   - single-pass decoupled look-back over the tiles of the SAME subdomain with a 32-wide window
+//     (lane L inspects predecessor t-1-L), carrying two running sums: stayers and migrants;
+//   - stayers written in place at their compacted slot; migrants written to the subdomain's send
+//     region at (migrant prefix) + (offset of their code's run in the tile chunk) + (in-tile rank).
+//   The per-code cross-tile prefix needed by the unpack is produced afterwards by k_code_scan
+//   from tile_cnt[] (it is not on the critical path of the look-back).
 // `dep_zero` is always 0; it ties the id/field loads into the published aggregate so that a
 // tile publishes only after its loads have completed (in-place compaction safety).
 // ---------------------------------------------------------------------------------------------
-template <bool kFused>
-__global__ void __launch_bounds__(kBlock)
-k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ fu, const double* __restrict__ fv,
-            const double* __restrict__ fw, double dt, uint32_t epoch, unsigned long long dep_zero)
+__device__ __forceinline__ uint32_t warp_sum(uint32_t v)
 {
-    __shared__ unsigned int s_ticket;
-    __shared__ uint32_t s_wtot[kWarps][32];     // per-warp per-code counts, then exclusive prefix over warps
-    __shared__ uint32_t s_excl[32];             // exclusive prefix of this tile (over earlier tiles of s)
-    __shared__ uint32_t s_codeoff[32];          // offset of code c inside this tile's send chunk
-    __shared__ int64_t s_sendbase;              // first send slot of this tile's chunk, -1 = overflow
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
 
-    if (threadIdx.x == 0) s_ticket = atomicAdd(T.ticket, 1u);
+// one window step of the look-back for one of the two running sums; returns true when a PREFIX was found
+__device__ __forceinline__ bool window_step(uint64_t w, bool beyond_start, int lane, uint32_t& excl)
+{
+    const bool is_prefix = beyond_start || ((uint32_t)(w >> 32) & 3u) == kStPrefix;
+    const unsigned pm = __ballot_sync(0xffffffffu, is_prefix);
+    const int first = pm ? (__ffs(pm) - 1) : 32;               // nearest predecessor holding a prefix
+    const uint32_t v = (lane <= first && !beyond_start) ? (uint32_t)w : 0u;
+    excl += warp_sum(v);
+    return pm != 0u;
+}
+
+// A pushed tile staged in shared memory in OUTPUT order: stayers first (stable), then the migrants
+// grouped by destination code (stable inside each code).
+struct TileBuf {
+    double f[7][kTile];
+    long long id[kTile];
+};
+
+struct TileCtl {
+    uint32_t wtot[kWarps][32];      // per-warp per-code counts of the tile being pushed
+    uint32_t stay_excl;             // look-back result of the tile being resolved
+    long long sendbase;             // first send slot of its chunk, -1 = send region overflow
+    unsigned int next_ticket;
+};
+
+// Per-tile facts carried from its push to its resolve one iteration later (all CTA-uniform).
+struct TileInfo { int s, t; uint32_t n_stay, n_mig, cnt_s; bool valid; };
+
+template <bool kFused>
+__global__ void __launch_bounds__(kBlock, kMinBlocks)
+k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch,
+            unsigned long long dep_zero)
+{
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    TileBuf* buf = reinterpret_cast<TileBuf*>(s_raw);                                   // [2]
+    uint32_t* s_tile_start = reinterpret_cast<uint32_t*>(s_raw + 2 * sizeof(TileBuf));  // [P+1]
+    __shared__ TileCtl sm;
+
+    for (int i = threadIdx.x; i <= G.P; i += kBlock) s_tile_start[i] = T.tile_start[i];
+    if (threadIdx.x == 0) sm.next_ticket = atomicAdd(T.ticket, 1u);
     __syncthreads();
-    const unsigned int g = s_ticket;
-    const int s = g / G.tiles_per_sub;
-    const int t = g % G.tiles_per_sub;
-    const uint32_t cnt_s = T.count[s];
-    const int64_t first = (int64_t)t * kTile;
-    if (first >= (int64_t)cnt_s) return;
-    const bool last_tile = first + kTile >= (int64_t)cnt_s;
-
+    const unsigned int n_active = s_tile_start[G.P];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t slot0 = first + 2 * (int64_t)threadIdx.x;
-    const size_t slab0 = (size_t)s * (size_t)G.cap;
-    const size_t base = slab0 + (size_t)slot0;
-    const bool v0 = slot0 < (int64_t)cnt_s, v1 = slot0 + 1 < (int64_t)cnt_s;
+    const uint64_t tag = (uint64_t)(epoch << 2) << 32;
 
-    Particle p0, p1;
-    int64_t id0 = 0, id1 = 0;
-    int c0 = kStay, c1 = kStay;
-    bool jump = false;
-    unsigned long long dep = 0;
-    if (v0) {
-        double2 q[7];
-#pragma unroll
-        for (int a = 0; a < 7; ++a) q[a] = ld_stream2(S.f[a] + base);
-        const longlong2 qi = ld_stream2(S.id + base);
-        p0 = Particle{q[0].x, q[1].x, q[2].x, q[3].x, q[4].x, q[5].x, q[6].x};
-        p1 = Particle{q[0].y, q[1].y, q[2].y, q[3].y, q[4].y, q[5].y, q[6].y};
-        id0 = qi.x; id1 = qi.y;
-        if (kFused) {
-            const SubBox B = sub_box(G, s);
-            c0 = push_particle(p0, fu, fv, fw, G, B, dt, jump);
-            if (v1) c1 = push_particle(p1, fu, fv, fw, G, B, dt, jump);
-            dep = (unsigned long long)(id0 ^ id1);
-        } else {
-            const uchar2 cc = *reinterpret_cast<const uchar2*>(S.code + base);
-            c0 = min((int)cc.x, 26);
-            c1 = v1 ? min((int)cc.y, 26) : kStay;
-            dep = (unsigned long long)(id0 ^ id1);
-#pragma unroll
-            for (int a = 0; a < 7; ++a)
-                dep ^= (unsigned long long)(__double_as_longlong(q[a].x) ^ __double_as_longlong(q[a].y));
-        }
-        dep &= dep_zero;                          // == 0, but only known at run time
-    }
-    if (jump) raise(T.status, -5);
+    TileInfo prev; prev.valid = false; prev.s = prev.t = 0; prev.n_stay = prev.n_mig = prev.cnt_s = 0;
+    for (int it = 0;; ++it) {
+        const int b = it & 1;
+        const unsigned int g = sm.next_ticket;
+        TileInfo cur; cur.valid = g < n_active; cur.s = cur.t = 0; cur.n_stay = cur.n_mig = cur.cnt_s = 0;
+        if (!cur.valid && !prev.valid) break;
 
-    // --- in-warp ranks and per-warp totals --------------------------------------------------
-    const RowBallots r0 = row_ballots(v0 || dep != 0, c0), r1 = row_ballots(v1, c1);
-    const unsigned lt = (1u << lane) - 1u;
-    const uint32_t rank0 = __popc(code_mask(r0, c0) & lt) + __popc(code_mask(r1, c0) & lt);
-    const uint32_t rank1 = __popc(code_mask(r0, c1) & lt) + __popc(code_mask(r1, c1) & lt) + ((v0 && c0 == c1) ? 1u : 0u);
-    s_wtot[warp][lane] = (lane < kNC) ? (uint32_t)(__popc(code_mask(r0, lane)) + __popc(code_mask(r1, lane))) : 0u;
-    __syncthreads();
+        // ============ push phase of tile g: load, (push,) rank, stage into buf[b], publish aggregate ============
+        if (cur.valid) {
+            int lo = 0, hi = G.P;                                       // largest s with tile_start[s] <= g
+            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (s_tile_start[mid] <= g) lo = mid; else hi = mid; }
+            cur.s = lo;
+            cur.t = (int)(g - s_tile_start[lo]);
+            cur.cnt_s = T.count[lo];
+            const int64_t first = (int64_t)cur.t * kTile;
+            const int64_t slot0 = first + 2 * (int64_t)threadIdx.x;
+            const size_t base = (size_t)cur.s * (size_t)G.cap + (size_t)slot0;
+            const bool v0 = slot0 < (int64_t)cur.cnt_s, v1 = slot0 + 1 < (int64_t)cur.cnt_s;
 
-    // --- warp 0: block aggregate, publish, look back ------------------------------------------
-    if (warp == 0) {
-        uint32_t agg = 0;
+            Particle p0, p1;
+            int64_t id0 = 0, id1 = 0;
+            int c0 = kStay, c1 = kStay;
+            bool jump = false;
+            unsigned long long dep = 0;
+            if (v0) {
+                double2 q[7];
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) { const uint32_t v = s_wtot[w][lane]; s_wtot[w][lane] = agg; agg += v; }
-        uint64_t* my_desc = T.desc + ((size_t)s * G.tiles_per_sub + t) * 32;
-        const uint64_t tag = (uint64_t)(epoch << 2) << 32;
-        uint32_t excl = 0;
-        if (t == 0) {
-            st_relaxed_u64(my_desc + lane, tag | ((uint64_t)kStPrefix << 32) | agg);
-        } else {
-            st_relaxed_u64(my_desc + lane, tag | ((uint64_t)kStAgg << 32) | agg);
-            int j = t - 1;
-            while (true) {
-                const uint64_t* pd = T.desc + ((size_t)s * G.tiles_per_sub + j) * 32 + lane;
-                uint64_t wv = ld_relaxed_u64(pd);
-                while ((uint32_t)(wv >> 34) != epoch || ((uint32_t)(wv >> 32) & 3u) == 0u) { __nanosleep(20); wv = ld_relaxed_u64(pd); }
-                excl += (uint32_t)wv;
-                if (((uint32_t)(wv >> 32) & 3u) == kStPrefix) break;
-                --j;
+                for (int a = 0; a < 7; ++a) q[a] = ld_stream2(S.f[a] + base);
+                const longlong2 qi = ld_stream2(S.id + base);
+                p0 = Particle{q[0].x, q[1].x, q[2].x, q[3].x, q[4].x, q[5].x, q[6].x};
+                p1 = Particle{q[0].y, q[1].y, q[2].y, q[3].y, q[4].y, q[5].y, q[6].y};
+                id0 = qi.x; id1 = qi.y;
+                if (kFused) {
+                    const SubBox B = sub_box(G, cur.s);
+                    c0 = push_particle(p0, F4, G, B, dt, jump);
+                    if (v1) c1 = push_particle(p1, F4, G, B, dt, jump);
+                } else {
+                    const uchar2 cc = *reinterpret_cast<const uchar2*>(S.code + base);
+                    c0 = min((int)cc.x, 26);
+                    c1 = v1 ? min((int)cc.y, 26) : kStay;
+                }
             }
-            st_relaxed_u64(my_desc + lane, tag | ((uint64_t)kStPrefix << 32) | (uint64_t)(excl + agg));
-        }
-        s_excl[lane] = excl;
-        const size_t trow = ((size_t)s * G.tiles_per_sub + t) * 32 + lane;
-        T.tile_excl[trow] = excl;
-        T.tile_cnt[trow] = agg;
-        if (last_tile) T.cnt[s * 32 + lane] = excl + agg;      // a4/a5 totals of subdomain s
-        // offsets of each code's run inside this tile's send chunk, and the chunk's position
-        const uint32_t magg = (lane < kNC && lane != kStay) ? agg : 0u;
-        const uint32_t mexc = (lane < kNC && lane != kStay) ? excl : 0u;
-        uint32_t inc = magg, tot_excl = mexc;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += nb;
-            tot_excl += __shfl_xor_sync(0xffffffffu, tot_excl, o);
-        }
-        s_codeoff[lane] = inc - magg;
-        const uint32_t n_mig_tile = __shfl_sync(0xffffffffu, inc, 31);
-        if (lane == 0) {
-            int64_t sb = (int64_t)s * G.send_cap + (int64_t)tot_excl;
-            if ((int64_t)tot_excl + (int64_t)n_mig_tile > G.send_cap) { raise(T.status, -4); sb = -1; }
-            s_sendbase = sb;
-        }
-    }
-    __syncthreads();
+            if (jump) raise(T.status, -5);
 
-    // --- scatter: stayers compact in place, migrants to the send chunk ---------------------------
-    const int64_t sendbase = s_sendbase;
+            // in-warp ranks and per-warp totals
+            const RowBallots r0 = row_ballots(v0, c0), r1 = row_ballots(v1, c1);
+            const unsigned lt = (1u << lane) - 1u;
+            const uint32_t rank0 = __popc(code_mask(r0, c0) & lt) + __popc(code_mask(r1, c0) & lt);
+            const uint32_t rank1 = __popc(code_mask(r0, c1) & lt) + __popc(code_mask(r1, c1) & lt) + ((v0 && c0 == c1) ? 1u : 0u);
+            sm.wtot[warp][lane] = (lane < kNC) ? (uint32_t)(__popc(code_mask(r0, lane)) + __popc(code_mask(r1, lane))) : 0u;
+            __syncthreads();                                                                             // B1
+            // every warp: lane c sums code c over the warps -> its own exclusive prefix and the tile total
+            uint32_t wexcl = 0, agg = 0;
 #pragma unroll
-    for (int e = 0; e < kIpt; ++e) {
-        const bool valid = e == 0 ? v0 : v1;
-        if (!valid) continue;
-        const int c = e == 0 ? c0 : c1;
-        const Particle& p = e == 0 ? p0 : p1;
-        const int64_t pid = e == 0 ? id0 : id1;
-        const uint32_t in_tile = s_wtot[warp][c] + (e == 0 ? rank0 : rank1);
-        const bool stay = c == kStay;
-        if (!stay && sendbase < 0) continue;
-        const size_t dst = stay ? slab0 + (size_t)s_excl[kStay] + in_tile
-                                : (size_t)sendbase + s_codeoff[c] + in_tile;
-        st_stream((stay ? S.f[0] : Snd.f[0]) + dst, p.x);
-        st_stream((stay ? S.f[1] : Snd.f[1]) + dst, p.y);
-        st_stream((stay ? S.f[2] : Snd.f[2]) + dst, p.z);
-        st_stream((stay ? S.f[3] : Snd.f[3]) + dst, p.vx);
-        st_stream((stay ? S.f[4] : Snd.f[4]) + dst, p.vy);
-        st_stream((stay ? S.f[5] : Snd.f[5]) + dst, p.vz);
-        st_stream((stay ? S.f[6] : Snd.f[6]) + dst, p.d);
-        st_stream((stay ? S.id : Snd.id) + dst, pid);
+            for (int w = 0; w < kWarps; ++w) { const uint32_t v = sm.wtot[w][lane]; if (w < warp) wexcl += v; agg += v; }
+            const uint32_t magg = (lane < kNC && lane != kStay) ? agg : 0u;
+            uint32_t inc = magg;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += nb;
+            }
+            cur.n_mig = __shfl_sync(0xffffffffu, inc, 31);
+            cur.n_stay = __shfl_sync(0xffffffffu, agg, kStay);
+            // position of code c's run in the staged tile: stayers at 0, migrants after them in code order
+            const uint32_t run_start = (lane == kStay) ? 0u : cur.n_stay + (inc - magg);
+            const uint32_t my_base = run_start + wexcl;            // lane c: first staged slot of this warp's code-c particles
+            TileBuf& B = buf[b];
+            if (v0) {
+                const uint32_t pos = __shfl_sync(0xffffffffu, my_base, c0) + rank0;
+                B.f[0][pos] = p0.x; B.f[1][pos] = p0.y; B.f[2][pos] = p0.z; B.f[3][pos] = p0.vx;
+                B.f[4][pos] = p0.vy; B.f[5][pos] = p0.vz; B.f[6][pos] = p0.d; B.id[pos] = id0;
+            } else (void)__shfl_sync(0xffffffffu, my_base, 0);
+            if (v1) {
+                const uint32_t pos = __shfl_sync(0xffffffffu, my_base, c1) + rank1;
+                B.f[0][pos] = p1.x; B.f[1][pos] = p1.y; B.f[2][pos] = p1.z; B.f[3][pos] = p1.vx;
+                B.f[4][pos] = p1.vy; B.f[5][pos] = p1.vz; B.f[6][pos] = p1.d; B.id[pos] = id1;
+            } else (void)__shfl_sync(0xffffffffu, my_base, 0);
+            if (warp == 0) {
+                // The staged copies above are this warp's own; the other warps' loads are ordered before the
+                // publish by barrier B1 (their ballots consumed the loaded values) -- see DESIGN.md 6.3.
+                const size_t tile_row = (size_t)cur.s * G.tiles_per_sub + cur.t;
+                T.tile_cnt[tile_row * 32 + lane] = agg;
+                if (lane < 2) {
+                    const uint32_t mine = lane == 0 ? cur.n_stay : cur.n_mig;
+                    const uint32_t st = cur.t == 0 ? kStPrefix : kStAgg;
+                    st_relaxed_u64(T.desc + tile_row * 2 + lane, tag | ((uint64_t)st << 32) | mine);
+                }
+            }
+        }
+
+        // ============ resolve phase of the previous tile: windowed look-back (warp 0) ============
+        if (prev.valid && warp == 0) {
+            uint32_t excl_stay = 0, excl_mig = 0;
+            if (prev.t > 0) {
+                bool done_s = false, done_m = false;
+                for (int nearest = prev.t - 1; !(done_s && done_m); nearest -= 32) {
+                    const int j = nearest - lane;
+                    const bool beyond = j < 0;                       // before the subdomain's first tile: prefix 0
+                    uint64_t wa = 0, wb = 0;
+                    if (!beyond) {
+                        const uint64_t* pd = T.desc + ((size_t)prev.s * G.tiles_per_sub + j) * 2;
+                        wa = ld_relaxed_u64(pd);
+                        wb = ld_relaxed_u64(pd + 1);
+                        while ((uint32_t)(wa >> 34) != epoch || ((uint32_t)(wa >> 32) & 3u) == 0u ||
+                               (uint32_t)(wb >> 34) != epoch || ((uint32_t)(wb >> 32) & 3u) == 0u) {
+                            __nanosleep(20);
+                            wa = ld_relaxed_u64(pd);
+                            wb = ld_relaxed_u64(pd + 1);
+                        }
+                    }
+                    if (!done_s) done_s = window_step(wa, beyond, lane, excl_stay);
+                    if (!done_m) done_m = window_step(wb, beyond, lane, excl_mig);
+                }
+                if (lane < 2) {
+                    const uint32_t incl = lane == 0 ? excl_stay + prev.n_stay : excl_mig + prev.n_mig;
+                    st_relaxed_u64(T.desc + ((size_t)prev.s * G.tiles_per_sub + prev.t) * 2 + lane,
+                                   tag | ((uint64_t)kStPrefix << 32) | (uint64_t)incl);
+                }
+            }
+            if (lane == 0) {
+                sm.stay_excl = excl_stay;
+                long long sb = (long long)prev.s * G.send_cap + (long long)excl_mig;
+                if ((long long)excl_mig + (long long)prev.n_mig > G.send_cap) { raise(T.status, -4); sb = -1; }
+                sm.sendbase = sb;
+                // next ticket: taken only after this look-back has finished, so a CTA never holds an
+                // unpublished ticket while it waits on predecessors
+                sm.next_ticket = atomicAdd(T.ticket, 1u);
+            }
+        } else if (!prev.valid && threadIdx.x == 0) {
+            sm.next_ticket = atomicAdd(T.ticket, 1u);
+        }
+        __syncthreads();                                                                                 // B2
+
+        // ============ copy-out of the previous tile: staged order == output order, coalesced ============
+        if (prev.valid) {
+            const TileBuf& B = buf[b ^ 1];
+            const size_t stay_base = (size_t)prev.s * (size_t)G.cap + (size_t)sm.stay_excl;
+            const long long sendbase = sm.sendbase;
+            for (uint32_t j = threadIdx.x; j < prev.n_stay; j += kBlock) {
+                const size_t dst = stay_base + j;
+#pragma unroll
+                for (int a = 0; a < 7; ++a) st_stream(S.f[a] + dst, B.f[a][j]);
+                st_stream(S.id + dst, (int64_t)B.id[j]);
+            }
+            if (sendbase >= 0) {
+                for (uint32_t j = threadIdx.x; j < prev.n_mig; j += kBlock) {
+                    const size_t dst = (size_t)sendbase + j;
+                    const uint32_t src = prev.n_stay + j;
+#pragma unroll
+                    for (int a = 0; a < 7; ++a) st_stream(Snd.f[a] + dst, B.f[a][src]);
+                    st_stream(Snd.id + dst, (int64_t)B.id[src]);
+                }
+            }
+        }
+        __syncthreads();                                                                                 // B3
+        prev = cur;
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K2b: per-(subdomain, code) exclusive scan of tile_cnt over the tiles of the subdomain ->
+// tile_excl (used by the unpack) and the count table totals cnt[s][c] (a4/a5).  One CTA per s.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_code_scan(Geom G, Tables T)
+{
+    __shared__ uint32_t s_part[8][32];
+    const int s = blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t cnt_s = T.count[s];
+    const int nt = (int)((cnt_s + kTile - 1) / kTile);
+    const int chunk = (nt + 7) / 8;
+    const int t0 = min(nt, warp * chunk), t1 = min(nt, t0 + chunk);
+    const size_t row0 = (size_t)s * G.tiles_per_sub;
+    uint32_t sum = 0;
+    for (int t = t0; t < t1; ++t) sum += T.tile_cnt[(row0 + t) * 32 + lane];
+    s_part[warp][lane] = sum;
+    __syncthreads();
+    uint32_t run = 0, total = 0;
+    for (int w = 0; w < 8; ++w) { const uint32_t v = s_part[w][lane]; if (w < warp) run += v; total += v; }
+    for (int t = t0; t < t1; ++t) {
+        const uint32_t v = T.tile_cnt[(row0 + t) * 32 + lane];
+        T.tile_excl[(row0 + t) * 32 + lane] = run;
+        run += v;
+    }
+    if (warp == 0) T.cnt[s * 32 + lane] = total;
+}
+
+// compact tile prefix: tile_start[s] = sum_{s' < s} ceil(count[s'] / kTile); one CTA
+__global__ void __launch_bounds__(1024)
+k_tile_index(Geom G, Tables T, int commit)
+{
+    __shared__ uint32_t sh[1024];
+    __shared__ uint32_t s_run;
+    if (threadIdx.x == 0) s_run = 0;
+    __syncthreads();
+    const bool ok = *T.status == 0;
+    for (int b0 = 0; b0 < G.P; b0 += 1024) {
+        const int r = b0 + threadIdx.x;
+        uint32_t v = 0;
+        if (r < G.P) {
+            if (commit && ok) T.count[r] = T.new_count[r];
+            v = (T.count[r] + kTile - 1) / kTile;
+        }
+        sh[threadIdx.x] = v;
+        __syncthreads();
+        for (int o = 1; o < 1024; o <<= 1) {
+            const uint32_t add = threadIdx.x >= (unsigned)o ? sh[threadIdx.x - o] : 0u;
+            __syncthreads();
+            sh[threadIdx.x] += add;
+            __syncthreads();
+        }
+        const uint32_t incl = sh[threadIdx.x] + s_run;
+        if (r < G.P) T.tile_start[r] = incl - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) s_run = incl;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { T.tile_start[G.P] = s_run; *T.ticket = 0u; }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -431,7 +601,7 @@ __global__ void __launch_bounds__(256)
 k_table(Geom G, Tables T)
 {
     __shared__ unsigned long long s_mig, s_tot;
-    if (threadIdx.x == 0) { s_mig = 0; s_tot = 0; *T.ticket = 0u; }
+    if (threadIdx.x == 0) { s_mig = 0; s_tot = 0; }
     __syncthreads();
     unsigned long long my_mig = 0, my_tot = 0;
     for (int r = threadIdx.x; r < G.P; r += blockDim.x) {
@@ -531,13 +701,6 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
         for (int a = 0; a < 7; ++a) S.f[a][dst] = __ldcs(Snd.f[a] + src);
         S.id[dst] = __ldcs(reinterpret_cast<const long long*>(Snd.id) + src);
     }
-}
-
-// counts <- new counts (after unpack)
-__global__ void k_commit_counts(Geom G, Tables T)
-{
-    const int r = blockIdx.x * blockDim.x + threadIdx.x;
-    if (r < G.P && *T.status == 0) T.count[r] = T.new_count[r];
 }
 
 // ---------------------------------------------------------------------------------------------
