@@ -41,16 +41,16 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
     size_t slab_f[7], slab_id, slab_code;
     size_t pool, pool_bytes, fluid4;
-    size_t count, cnt, recv_off, new_count, desc, tile_start, tile_excl, tile_cnt, misc, prefix;
+    size_t count, cnt, recv_off, new_count, desc, gdesc, tile_start, tile_cnt, group_excl, misc, prefix;
     size_t total;
-    int tiles_per_sub;
+    int tiles_per_sub, groups_per_sub, lbgroups_per_sub;
     int64_t send_cap;
 };
 
 bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* prm)
 {
     if (!prm) return false;
-    if (N < 2 || N > (1 << 20) || Px < 1 || Py < 1 || Pz < 1) return false;
+    if (N < 2 || N > 1625 || Px < 1 || Py < 1 || Pz < 1) return false;
     if (N % Px || N % Py || N % Pz) return false;
     const int64_t P = (int64_t)Px * Py * Pz;
     if (P > 8192) return false;                          // grid.y and shared-histogram limits
@@ -69,6 +69,8 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     const size_t slots = P * (size_t)cap;
     L.send_cap = prm->send_capacity ? prm->send_capacity : cap;
     L.tiles_per_sub = (int)((cap + kTile - 1) / kTile);
+    L.groups_per_sub = (L.tiles_per_sub + kGroup - 1) / kGroup;
+    L.lbgroups_per_sub = (L.tiles_per_sub + 31) / 32;
     const size_t ntiles = P * (size_t)L.tiles_per_sub;
     size_t off = 0;
     for (int a = 0; a < 7; ++a) { L.slab_f[a] = off; off = align_up(off + slots * 8); }
@@ -86,16 +88,20 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     L.recv_off = off;  off = align_up(off + P * 32 * 4);
     L.new_count = off; off = align_up(off + P * 4);
     L.desc = off;      off = align_up(off + ntiles * 2 * 8);
+    L.gdesc = off;     off = align_up(off + P * (size_t)L.lbgroups_per_sub * 2 * 8);
     L.tile_start = off; off = align_up(off + (P + 1) * 4);
-    L.tile_excl = off; off = align_up(off + ntiles * 32 * 4);
-    L.tile_cnt = off;  off = align_up(off + ntiles * 32 * 4);
+    L.tile_cnt = off;  off = align_up(off + ntiles * 32);
+    L.group_excl = off; off = align_up(off + P * (size_t)L.groups_per_sub * 32 * 4);
     L.misc = off;      off = align_up(off + 256);
     L.prefix = off;    off = align_up(off + (P + 1) * 8);
     L.total = off;
     return L;
 }
 
-inline size_t tile_pass_smem(int P) { return 2 * sizeof(TileBuf) + (size_t)(P + 1) * sizeof(uint32_t); }
+inline size_t tile_pass_smem(int P)
+{
+    return kWarps * sizeof(WarpStage) + (P <= kTileStartSmemMax ? (size_t)(P + 1) * sizeof(uint32_t) : 0);
+}
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -115,14 +121,14 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
     if (rec) cudaEventRecord(ev[0], h->stream);
     const size_t smem = tile_pass_smem(G.P);
     if (fused)
-        k_tile_pass<true><<<h->grid_fused, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch, 0ull);
+        k_tile_pass<true><<<h->grid_fused, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch);
     else
-        k_tile_pass<false><<<h->grid_pack, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch, 0ull);
+        k_tile_pass<false><<<h->grid_pack, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch);
     if (rec) cudaEventRecord(ev[1], h->stream);
     k_code_scan<<<G.P, 256, 0, h->stream>>>(G, h->T);
     k_table<<<1, 256, 0, h->stream>>>(G, h->T);
     if (rec) cudaEventRecord(ev[2], h->stream);
-    k_unpack<<<dim3(G.tiles_per_sub, G.P), kUnpackBlock, 0, h->stream>>>(G, h->S, h->Snd, h->T);
+    k_unpack<<<dim3((G.groups_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, h->S, h->Snd, h->T);
     k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, 1);
     if (rec) { cudaEventRecord(ev[3], h->stream); ++h->prof_steps; }
     h->pushed = false;
@@ -157,6 +163,8 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     G.N = N; G.Px = Px; G.Py = Py; G.Pz = Pz; G.P = Px * Py * Pz;
     G.nx = N / Px; G.ny = N / Py; G.nz = N / Pz;
     G.tiles_per_sub = L.tiles_per_sub;
+    G.groups_per_sub = L.groups_per_sub;
+    G.lbgroups_per_sub = L.lbgroups_per_sub;
     G.cap = capacity; G.send_cap = L.send_cap;
     // all doubles are computed once on the host and passed as data (rule R6)
     G.L = 6.283185307179586;                      // 2*pi*L0, L0 = 1
@@ -180,9 +188,10 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     h->T.recv_off = reinterpret_cast<uint32_t*>(w + L.recv_off);
     h->T.new_count = reinterpret_cast<uint32_t*>(w + L.new_count);
     h->T.desc = reinterpret_cast<uint64_t*>(w + L.desc);
+    h->T.gdesc = reinterpret_cast<uint64_t*>(w + L.gdesc);
     h->T.tile_start = reinterpret_cast<uint32_t*>(w + L.tile_start);
-    h->T.tile_excl = reinterpret_cast<uint32_t*>(w + L.tile_excl);
-    h->T.tile_cnt = reinterpret_cast<uint32_t*>(w + L.tile_cnt);
+    h->T.tile_cnt = reinterpret_cast<uint8_t*>(w + L.tile_cnt);
+    h->T.group_excl = reinterpret_cast<uint32_t*>(w + L.group_excl);
     h->T.ticket = reinterpret_cast<unsigned int*>(w + L.misc);
     h->T.status = reinterpret_cast<int*>(w + L.misc + 16);
     h->T.n_migrated = reinterpret_cast<unsigned long long*>(w + L.misc + 32);
@@ -199,7 +208,7 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_tile_pass<true>, kBlock, smem);
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, k_tile_pass<false>, kBlock, smem);
         if (sms < 1) sms = 148;
-        const long long max_tiles = (long long)G.P * G.tiles_per_sub;
+        const long long max_tiles = ((long long)G.P * G.tiles_per_sub + kWarps - 1) / kWarps;
         h->grid_fused = (int)std::min<long long>(max_tiles, (long long)sms * (occ_f > 0 ? occ_f : 1));
         h->grid_pack = (int)std::min<long long>(max_tiles, (long long)sms * (occ_p > 0 ? occ_p : 1));
     }
@@ -222,9 +231,8 @@ int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* 
 {
     if (!h || !d_u || !d_v || !d_w) return LCS_ERR_INVALID_ARG;
     if (!aligned16(d_u) || !aligned16(d_v) || !aligned16(d_w)) return LCS_ERR_INVALID_ARG;
-    const size_t ncell = (size_t)h->G.N * h->G.N * h->G.N;
-    const unsigned blocks = (unsigned)std::min<size_t>((ncell + 255) / 256, 148u * 16u);
-    k_repack_fluid<<<blocks, 256, 0, h->stream>>>(ncell, d_u, d_v, d_w, h->fluid4);
+    const int N = h->G.N, tiles = (N + 31) / 32;
+    k_repack_fluid<<<dim3(tiles * tiles, N), 256, 0, h->stream>>>(N, d_u, d_v, d_w, h->fluid4);
     h->have_fluid = true;
     return check_launch(h);
 }
@@ -269,7 +277,7 @@ int lcs_particle_step(lcs_t* h, double dt)
     if (h->sticky) return h->sticky;
     const Geom& G = h->G;
     cudaMemsetAsync(h->T.cnt, 0, (size_t)G.P * 32 * 4, h->stream);
-    k_push<<<dim3(G.tiles_per_sub, G.P), kBlock, 0, h->stream>>>(G, h->S, h->T, h->fluid4, dt);
+    k_push<<<dim3((G.tiles_per_sub + kWarps - 1) / kWarps, G.P), kBlock, 0, h->stream>>>(G, h->S, h->T, h->fluid4, dt);
     h->pushed = true;
     return check_launch(h);
 }
@@ -301,7 +309,7 @@ static int copy_out(lcs_t* h, int64_t* d_counts, OutPtrs O)
 {
     const Geom& G = h->G;
     k_counts_out<<<1, 256, 0, h->stream>>>(G, h->T, d_counts, h->prefix);
-    k_copy_out<<<dim3(G.tiles_per_sub, G.P), kBlock, 0, h->stream>>>(G, h->S, h->T, h->prefix, O, h->pushed ? 1 : 0);
+    k_copy_out<<<dim3((unsigned)((G.cap + kCopyTile - 1) / kCopyTile), G.P), 256, 0, h->stream>>>(G, h->S, h->T, h->prefix, O, h->pushed ? 1 : 0);
     return check_launch(h, 2);
 }
 

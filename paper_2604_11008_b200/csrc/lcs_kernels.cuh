@@ -2,6 +2,13 @@
 // DESIGN.md section 6 for the kernel-by-kernel description.  Compiled with -fmad=false: a fused
 // multiply-add happens only where fma() is written, so the push is bit-reproducible (DESIGN.md
 // section 4, rules R1-R7).
+//
+// Execution model of the hot kernel (k_tile_pass): WARP-AUTONOMOUS tiles.  A tile is 128
+// consecutive slots of one subdomain slab (4 rows of 32 lanes).  Every warp of a persistent grid
+// takes tiles from an atomic ticket and runs the whole path for its tile with warp-level
+// primitives only (ballot / shuffle / popc, a private shared-memory staging area, no block
+// barrier): the 24 resident warps of an SM drift apart in phase, so the DRAM stream, the L2
+// gather, the fp64 arithmetic, the look-back and the write-out of different tiles overlap.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -12,22 +19,26 @@ namespace lcs {
 #define LCS_BLOCK 256
 #endif
 #ifndef LCS_MIN_BLOCKS
-#define LCS_MIN_BLOCKS 2
+#define LCS_MIN_BLOCKS 3
 #endif
-constexpr int kBlock = LCS_BLOCK;      // threads per tile CTA
+constexpr int kBlock = LCS_BLOCK;            // threads per CTA of the tile pass
 constexpr int kMinBlocks = LCS_MIN_BLOCKS;   // CTAs per SM the tile pass is compiled for
-constexpr int kIpt = 2;                // particles per thread = one 128-bit load per field
-constexpr int kTile = kBlock * kIpt;   // particles per tile
 constexpr int kWarps = kBlock / 32;
+constexpr int kRows = 4;                     // rows (particles per lane) of a warp tile
+constexpr int kTile = 32 * kRows;            // particles per tile
 constexpr int kStay = 13;
-constexpr int kNC = 27;                // destination codes
+constexpr int kNC = 27;                      // destination codes
+constexpr int kInvalid = 31;                 // code of a lane beyond the slab's count
+constexpr int kGroup = 16;                   // tiles per unpack warp
+constexpr int kTileStartSmemMax = 2048;      // tile_start[] is mirrored in shared memory up to this P
 
-// Decoupled look-back descriptor word: [ epoch:30 | state:2 | value:32 ]
-constexpr uint32_t kStAgg = 1u, kStPrefix = 2u;
+// Look-back descriptor word: [ epoch:30 | valid:2 | value:32 ]
 
 struct Geom {
     int N, Px, Py, Pz, P, nx, ny, nz;
     int tiles_per_sub;                 // ceil(cap / kTile)
+    int groups_per_sub;                // ceil(tiles_per_sub / kGroup)
+    int lbgroups_per_sub;              // ceil(tiles_per_sub / 32): look-back groups
     int64_t cap, send_cap;
     double inv_dx, K_tau, L, L_below, gx, gy, gz;
 };
@@ -43,10 +54,11 @@ struct Tables {
     uint32_t* cnt;                     // [P*32] per-(s,c) totals of the last step (27 used per row)
     uint32_t* recv_off;                // [P*32] slot in the receiver slab where segment (s,c) starts
     uint32_t* new_count;               // [P]
-    uint64_t* desc;                    // [P*tiles_per_sub*2] look-back descriptors: (stay, migrant) words
+    uint64_t* desc;                    // [P*tiles_per_sub*2] tile aggregates: (stay, migrant) words
+    uint64_t* gdesc;                   // [P*lbgroups_per_sub*2] aggregates of groups of 32 tiles
     uint32_t* tile_start;              // [P+1] compact prefix of non-empty tiles per subdomain
-    uint32_t* tile_excl;               // [P*tiles_per_sub*32] exclusive per-code prefix of each tile
-    uint32_t* tile_cnt;                // [P*tiles_per_sub*32] per-code count of each tile
+    uint8_t* tile_cnt;                 // [P*tiles_per_sub*32] per-code count of each tile (<= 128 fits a byte)
+    uint32_t* group_excl;              // [P*groups_per_sub*32] exclusive per-code prefix at each group of kGroup tiles
     unsigned int* ticket;              // tile ticket counter
     int* status;                       // sticky error word
     unsigned long long* n_migrated;    // migrants of the last migrate
@@ -70,10 +82,21 @@ __device__ __forceinline__ void st_relaxed_u64(uint64_t* p, uint64_t v)
 }
 
 // streaming (touched once) particle traffic: evict-first so it does not push the fluid bricks out of L2
-__device__ __forceinline__ double2 ld_stream2(const double* p) { return __ldcs(reinterpret_cast<const double2*>(p)); }
-__device__ __forceinline__ longlong2 ld_stream2(const int64_t* p) { return __ldcs(reinterpret_cast<const longlong2*>(p)); }
-__device__ __forceinline__ void st_stream(double* p, double v) { __stcs(p, v); }
-__device__ __forceinline__ void st_stream(int64_t* p, int64_t v) { __stcs(reinterpret_cast<long long*>(p), (long long)v); }
+__device__ __forceinline__ unsigned long long ld_stream(const void* p)
+{
+    return __ldcs(reinterpret_cast<const unsigned long long*>(p));
+}
+__device__ __forceinline__ void st_stream(void* p, unsigned long long v)
+{
+    __stcs(reinterpret_cast<unsigned long long*>(p), v);
+}
+
+__device__ __forceinline__ uint32_t warp_sum(uint32_t v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
 
 // exp(-z), z >= 0: range reduction by ln2 (hi/lo), degree-14 Taylor polynomial in Horner form with
 // explicit fma, scaling by exponent arithmetic.  DESIGN.md R-3.
@@ -104,41 +127,107 @@ __device__ __forceinline__ double exp_neg(double z)
     return p * __longlong_as_double(bits);
 }
 
-struct Axis { int i0, i1; double f; };
-
-__device__ __forceinline__ Axis stencil_axis(double a, double inv_dx, int N)
-{   // cell centre i sits at (i + 1/2) dx; periodic stencil (DESIGN R-9)
-    Axis s;
-    const double ga = fma(a, inv_dx, -0.5);
-    const double fl = floor(ga);
-    int i0 = (int)fl;
-    s.f = ga - fl;
-    i0 = max(-1, min(i0, N - 1));                 // memory safety for corrupt input only
-    s.i0 = (i0 < 0) ? i0 + N : i0;
-    s.i1 = (i0 + 1 >= N) ? i0 + 1 - N : i0 + 1;
-    return s;
-}
-
 __device__ __forceinline__ double lerp(double p, double q, double f) { return fma(f, q - p, p); }
 
-// Fluid is held as one 32-byte record per cell: (u, v, w, 0) -- one L2 sector and one 256-bit load per
-// stencil corner instead of three scattered 8-byte loads.
+// ---------------------------------------------------------------------------------------------
+// a1: gather.  The fluid is held internally as one 32-byte record (u, v, w, 0) per cell with the
+// Z index fastest: record index k + N*(j + N*i).  One L2 sector per stencil corner, and the two
+// corners that differ only in z are adjacent in memory.  The lanes of a pair (2m, 2m+1) share the
+// gather of their two particles: in one load instruction the even lane fetches the z0 corner and
+// the odd lane the z1 corner of the SAME particle, so the pair touches one 128-byte line (three
+// times out of four) instead of two.  Each lane reduces its z-side with the x and y lerps; one
+// exchange of three doubles then feeds the z lerp.  Operation order per particle is exactly
+// lerp x, then y, then z (rule R3).
+// ---------------------------------------------------------------------------------------------
 struct alignas(32) Cell { double u, v, w, pad; };
 
-__device__ __forceinline__ Cell ld_cell(const double* __restrict__ F4, size_t cell)
+__device__ __forceinline__ Cell ld_cell(const double* __restrict__ F4, uint32_t cell)
 {
     Cell r;
     asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
-                 : "=d"(r.u), "=d"(r.v), "=d"(r.w), "=d"(r.pad) : "l"(F4 + 4 * cell));
+                 : "=d"(r.u), "=d"(r.v), "=d"(r.w), "=d"(r.pad) : "l"(F4 + 4 * (size_t)cell));
     return r;
 }
 
+__device__ __forceinline__ void axis_stencil(double a, double inv_dx, int N, int& i0, int& i1, double& f)
+{   // cell centre i sits at (i + 1/2) dx; periodic stencil (DESIGN R-9)
+    const double ga = fma(a, inv_dx, -0.5);
+    int i = __double2int_rd(ga);                  // floor, then integer (rule R5); exact for |ga| < 2^31
+    f = ga - (double)i;
+    i = max(-1, min(i, N - 1));                   // memory safety for corrupt input only
+    i0 = (i < 0) ? i + N : i;
+    i1 = (i + 1 >= N) ? i + 1 - N : i + 1;
+}
+
+struct Vec3 { double x, y, z; };
+
+__device__ __forceinline__ Vec3 shfl_xor1(const Vec3& v)
+{
+    Vec3 r;
+    r.x = __shfl_xor_sync(0xffffffffu, v.x, 1);
+    r.y = __shfl_xor_sync(0xffffffffu, v.y, 1);
+    r.z = __shfl_xor_sync(0xffffffffu, v.z, 1);
+    return r;
+}
+
+// x and y lerps of one z-side: corners (i0,j0) (i1,j0) (i0,j1) (i1,j1)
+__device__ __forceinline__ Vec3 side_partial(const double* __restrict__ F4, const uint32_t idx[4], double fx, double fy)
+{
+    const Cell a = ld_cell(F4, idx[0]), b = ld_cell(F4, idx[1]), c = ld_cell(F4, idx[2]), d = ld_cell(F4, idx[3]);
+    Vec3 r;
+    r.x = lerp(lerp(a.u, b.u, fx), lerp(c.u, d.u, fx), fy);
+    r.y = lerp(lerp(a.v, b.v, fx), lerp(c.v, d.v, fx), fy);
+    r.z = lerp(lerp(a.w, b.w, fx), lerp(c.w, d.w, fx), fy);
+    return r;
+}
+
+// Fluid velocity at (x,y,z) of THIS lane's particle; must be called by all 32 lanes (converged).
+__device__ __forceinline__ Vec3 gather_pair(const double* __restrict__ F4, int N, double inv_dx, double x, double y,
+                                            double z, bool odd)
+{
+    int i0, i1, j0, j1, k0, k1;
+    double fx, fy, fz;
+    axis_stencil(x, inv_dx, N, i0, i1, fx);
+    axis_stencil(y, inv_dx, N, j0, j1, fy);
+    axis_stencil(z, inv_dx, N, k0, k1, fz);
+    const uint32_t Nu = (uint32_t)N;
+    const uint32_t row[4] = {Nu * ((uint32_t)j0 + Nu * (uint32_t)i0), Nu * ((uint32_t)j0 + Nu * (uint32_t)i1),
+                             Nu * ((uint32_t)j1 + Nu * (uint32_t)i0), Nu * ((uint32_t)j1 + Nu * (uint32_t)i1)};
+    // this lane always fetches z-side `odd` (0: k0, 1: k1) -- of its own particle and of its partner's
+    const uint32_t k_mine = odd ? (uint32_t)k1 : (uint32_t)k0;
+    const uint32_t k_other = odd ? (uint32_t)k0 : (uint32_t)k1;       // the side my partner fetches for me
+    uint32_t mine[4], theirs[4];
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        mine[m] = row[m] + k_mine;
+        theirs[m] = __shfl_xor_sync(0xffffffffu, row[m] + k_other, 1);
+    }
+    const double pfx = __shfl_xor_sync(0xffffffffu, fx, 1), pfy = __shfl_xor_sync(0xffffffffu, fy, 1);
+    // load set A = the even lane's particle, set B = the odd lane's particle
+    uint32_t ia[4], ib[4];
+#pragma unroll
+    for (int m = 0; m < 4; ++m) { ia[m] = odd ? theirs[m] : mine[m]; ib[m] = odd ? mine[m] : theirs[m]; }
+    const Vec3 pa = side_partial(F4, ia, odd ? pfx : fx, odd ? pfy : fy);
+    const Vec3 pb = side_partial(F4, ib, odd ? fx : pfx, odd ? fy : pfy);
+    // even lane needs A's z1 side (odd's pa); odd lane needs B's z0 side (even's pb)
+    Vec3 give;
+    give.x = odd ? pa.x : pb.x; give.y = odd ? pa.y : pb.y; give.z = odd ? pa.z : pb.z;
+    const Vec3 got = shfl_xor1(give);
+    Vec3 U;
+    U.x = lerp(odd ? got.x : pa.x, odd ? pb.x : got.x, fz);
+    U.y = lerp(odd ? got.y : pa.y, odd ? pb.y : got.y, fz);
+    U.z = lerp(odd ? got.z : pa.z, odd ? pb.z : got.z, fz);
+    return U;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2 / a3: advance, wrap, classify
+// ---------------------------------------------------------------------------------------------
 struct Particle { double x, y, z, vx, vy, vz, d; };
 
-// Per-block subdomain bounds in unwrapped cell index space.
-struct SubBox { int lox, hix, loy, hiy, loz, hiz; };
+struct SubBox { int lox, hix, loy, hiy, loz, hiz; };   // subdomain bounds in unwrapped cell index space
 
-// One axis of a2/a3: advance, wrap, classify.  Returns d in {-1,0,+1}; sets jump on violation.
+// One axis: returns d in {-1,0,+1}; sets jump on violation.
 __device__ __forceinline__ int advance_axis(double& a, double& v, double U, double g, double tau, double alpha,
                                             double b, double dt, const Geom& G, int lo, int hi, int n_a, bool& jump)
 {
@@ -152,7 +241,7 @@ __device__ __forceinline__ int advance_axis(double& a, double& v, double U, doub
     else if (xu >= G.L) { xu = xu - G.L; wrap = 1; }
     a = xu;
     if (!(xu >= 0.0 && xu < G.L)) { jump = true; return 0; }
-    int ic = (int)floor(xu * G.inv_dx);
+    int ic = __double2int_rd(xu * G.inv_dx);
     ic = max(0, min(ic, G.N - 1));
     const int icu = ic + wrap * G.N;              // unwrapped cell index (DESIGN R-14)
     const int dd = (icu >= hi) - (icu < lo);
@@ -160,37 +249,18 @@ __device__ __forceinline__ int advance_axis(double& a, double& v, double U, doub
     return dd;
 }
 
-// a1-a3 for one particle.  Returns the destination code.
+// a1-a3 for this lane's particle (all 32 lanes must call).  Returns the destination code.
 __device__ __forceinline__ int push_particle(Particle& p, const double* __restrict__ F4, const Geom& G,
-                                             const SubBox& B, double dt, bool& jump)
+                                             const SubBox& B, double dt, bool odd, bool& jump)
 {
-    const Axis sx = stencil_axis(p.x, G.inv_dx, G.N);
-    const Axis sy = stencil_axis(p.y, G.inv_dx, G.N);
-    const Axis sz = stencil_axis(p.z, G.inv_dx, G.N);
-    const size_t Ns = (size_t)G.N;
-    const size_t r00 = Ns * (sy.i0 + Ns * sz.i0), r10 = Ns * (sy.i1 + Ns * sz.i0);
-    const size_t r01 = Ns * (sy.i0 + Ns * sz.i1), r11 = Ns * (sy.i1 + Ns * sz.i1);
-    double Ux, Uy, Uz;
-    {
-        const Cell a0 = ld_cell(F4, r00 + sx.i0), a1 = ld_cell(F4, r00 + sx.i1);
-        const Cell b0 = ld_cell(F4, r10 + sx.i0), b1 = ld_cell(F4, r10 + sx.i1);
-        const Cell c0 = ld_cell(F4, r01 + sx.i0), c1 = ld_cell(F4, r01 + sx.i1);
-        const Cell d0 = ld_cell(F4, r11 + sx.i0), d1 = ld_cell(F4, r11 + sx.i1);
-        // same lerp order as the definition: x, then y, then z
-        Ux = lerp(lerp(lerp(a0.u, a1.u, sx.f), lerp(b0.u, b1.u, sx.f), sy.f),
-                  lerp(lerp(c0.u, c1.u, sx.f), lerp(d0.u, d1.u, sx.f), sy.f), sz.f);
-        Uy = lerp(lerp(lerp(a0.v, a1.v, sx.f), lerp(b0.v, b1.v, sx.f), sy.f),
-                  lerp(lerp(c0.v, c1.v, sx.f), lerp(d0.v, d1.v, sx.f), sy.f), sz.f);
-        Uz = lerp(lerp(lerp(a0.w, a1.w, sx.f), lerp(b0.w, b1.w, sx.f), sy.f),
-                  lerp(lerp(c0.w, c1.w, sx.f), lerp(d0.w, d1.w, sx.f), sy.f), sz.f);
-    }
+    const Vec3 U = gather_pair(F4, G.N, G.inv_dx, p.x, p.y, p.z, odd);
     const double tau = (G.K_tau * p.d) * p.d;     // tau_p = (rho_p/rho) d^2 / (18 nu)
     const double zz = dt / tau;
     const double alpha = exp_neg(zz);
     const double b = tau * (1.0 - alpha);
-    const int dx = advance_axis(p.x, p.vx, Ux, G.gx, tau, alpha, b, dt, G, B.lox, B.hix, G.nx, jump);
-    const int dy = advance_axis(p.y, p.vy, Uy, G.gy, tau, alpha, b, dt, G, B.loy, B.hiy, G.ny, jump);
-    const int dz = advance_axis(p.z, p.vz, Uz, G.gz, tau, alpha, b, dt, G, B.loz, B.hiz, G.nz, jump);
+    const int dx = advance_axis(p.x, p.vx, U.x, G.gx, tau, alpha, b, dt, G, B.lox, B.hix, G.nx, jump);
+    const int dy = advance_axis(p.y, p.vy, U.y, G.gy, tau, alpha, b, dt, G, B.loy, B.hiy, G.ny, jump);
+    const int dz = advance_axis(p.z, p.vz, U.z, G.gz, tau, alpha, b, dt, G, B.loz, B.hiz, G.nz, jump);
     return (dx + 1) + 3 * (dy + 1) + 9 * (dz + 1);
 }
 
@@ -213,327 +283,313 @@ __device__ __forceinline__ int receiver_of(const Geom& G, int s, int c)
 }
 
 // ---------------------------------------------------------------------------------------------
-// warp-level classification bookkeeping: six ballots per item row (x-,x+,y-,y+,z-,z+) + validity
+// Stable per-code ranks of one row of 32 particles.  `cnt_c` (lane c owns code c) is the number of
+// code-c particles in the earlier rows of the tile; on return it includes this row.  Returns this
+// lane's rank among the tile's particles with the same code.  One warp-uniform iteration per
+// distinct code present in the row (almost always 1 to 3).
 // ---------------------------------------------------------------------------------------------
-struct RowBallots { unsigned xm, xp, ym, yp, zm, zp, val; };
-
-__device__ __forceinline__ RowBallots row_ballots(bool valid, int code)
+__device__ __forceinline__ uint32_t row_rank(int code, bool valid, int lane, uint32_t& cnt_c)
 {
-    const int dx = code % 3, dy = (code / 3) % 3, dz = code / 9;   // 0,1,2 <-> -1,0,+1
-    RowBallots r;
-    r.val = __ballot_sync(0xffffffffu, valid);
-    r.xm = __ballot_sync(0xffffffffu, valid && dx == 0);
-    r.xp = __ballot_sync(0xffffffffu, valid && dx == 2);
-    r.ym = __ballot_sync(0xffffffffu, valid && dy == 0);
-    r.yp = __ballot_sync(0xffffffffu, valid && dy == 2);
-    r.zm = __ballot_sync(0xffffffffu, valid && dz == 0);
-    r.zp = __ballot_sync(0xffffffffu, valid && dz == 2);
-    return r;
-}
-
-// lanes of the row whose particle has destination code c
-__device__ __forceinline__ unsigned code_mask(const RowBallots& r, int c)
-{
-    const int dx = c % 3, dy = (c / 3) % 3, dz = c / 9;
-    const unsigned mx = dx == 0 ? r.xm : (dx == 2 ? r.xp : r.val & ~(r.xm | r.xp));
-    const unsigned my = dy == 0 ? r.ym : (dy == 2 ? r.yp : r.val & ~(r.ym | r.yp));
-    const unsigned mz = dz == 0 ? r.zm : (dz == 2 ? r.zp : r.val & ~(r.zm | r.zp));
-    return mx & my & mz;
+    unsigned todo = __ballot_sync(0xffffffffu, valid);
+    const unsigned lt = (1u << lane) - 1u;
+    uint32_t rank = 0;
+    while (todo) {
+        const int leader = __ffs(todo) - 1;
+        const int c = __shfl_sync(0xffffffffu, code, leader);
+        const unsigned m = __ballot_sync(0xffffffffu, code == c);
+        const uint32_t base = __shfl_sync(0xffffffffu, cnt_c, c);
+        if (code == c) rank = base + __popc(m & lt);
+        if (lane == c) cnt_c += __popc(m);
+        todo &= ~m;
+    }
+    return rank;
 }
 
 // ---------------------------------------------------------------------------------------------
-// K0: lcs_set_fluid -- repack the three x-fastest arrays into one (u,v,w,0) record per cell
+// K0: lcs_set_fluid -- repack the three x-fastest arrays u,v,w[i + N*(j + N*k)] into one
+// (u,v,w,0) record per cell with z fastest: F4[k + N*(j + N*i)].  32x32 (i,k) tiles through
+// shared memory so that both the reads (along i) and the writes (along k) are coalesced.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_repack_fluid(size_t ncell, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
+k_repack_fluid(int N, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
                double* __restrict__ F4)
 {
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncell; i += (size_t)gridDim.x * blockDim.x) {
-        const double4 r = make_double4(__ldcs(u + i), __ldcs(v + i), __ldcs(w + i), 0.0);
-        *reinterpret_cast<double4*>(F4 + 4 * i) = r;
+    __shared__ double t[3][32][33];
+    const int j = blockIdx.y;
+    const int tiles = (N + 31) / 32;
+    const int ti = blockIdx.x % tiles, tk = blockIdx.x / tiles;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;      // 32 x 8
+    const size_t Ns = (size_t)N;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int k = tk * 32 + ty + 8 * r, i = ti * 32 + tx;
+        if (k < N && i < N) {
+            const size_t src = i + Ns * (j + Ns * k);
+            t[0][ty + 8 * r][tx] = __ldcs(u + src);
+            t[1][ty + 8 * r][tx] = __ldcs(v + src);
+            t[2][ty + 8 * r][tx] = __ldcs(w + src);
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int i = ti * 32 + ty + 8 * r, k = tk * 32 + tx;
+        if (k < N && i < N) {
+            const size_t dst = k + Ns * (j + Ns * i);
+            const double4 rec = make_double4(t[0][tx][ty + 8 * r], t[1][tx][ty + 8 * r], t[2][tx][ty + 8 * r], 0.0);
+            *reinterpret_cast<double4*>(F4 + 4 * dst) = rec;
+        }
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// K1: unfused push (a1-a4).  One CTA per (subdomain, tile); in place; codes + count table.
+// K1: unfused push (a1-a4), lcs_particle_step.  One warp per tile; in place; codes + count table.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kBlock)
 k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
 {
     const int s = blockIdx.y;
-    const int t = blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int t = blockIdx.x * kWarps + warp;
     const uint32_t cnt_s = T.count[s];
     const int64_t first = (int64_t)t * kTile;
     if (first >= (int64_t)cnt_s) return;
-    __shared__ uint32_t s_cnt[kNC];
-    if (threadIdx.x < kNC) s_cnt[threadIdx.x] = 0;
-    __syncthreads();
     const SubBox B = sub_box(G, s);
-    const int64_t slot0 = first + 2 * (int64_t)threadIdx.x;      // even: 16-byte aligned
-    const size_t base = (size_t)s * (size_t)G.cap + (size_t)slot0;
-    const bool v0 = slot0 < (int64_t)cnt_s, v1 = slot0 + 1 < (int64_t)cnt_s;
-    int c0 = kStay, c1 = kStay;
+    const bool odd = lane & 1;
+    uint32_t cnt_c = 0;
     bool jump = false;
-    if (v0) {
-        double2 q[7];
-#pragma unroll
-        for (int a = 0; a < 7; ++a) q[a] = ld_stream2(S.f[a] + base);
-        Particle p0{q[0].x, q[1].x, q[2].x, q[3].x, q[4].x, q[5].x, q[6].x};
-        Particle p1{q[0].y, q[1].y, q[2].y, q[3].y, q[4].y, q[5].y, q[6].y};
-        c0 = push_particle(p0, F4, G, B, dt, jump);
-        if (v1) c1 = push_particle(p1, F4, G, B, dt, jump);
-        double2 o;
-        o = make_double2(p0.x, p1.x);   __stcs(reinterpret_cast<double2*>(S.f[0] + base), o);
-        o = make_double2(p0.y, p1.y);   __stcs(reinterpret_cast<double2*>(S.f[1] + base), o);
-        o = make_double2(p0.z, p1.z);   __stcs(reinterpret_cast<double2*>(S.f[2] + base), o);
-        o = make_double2(p0.vx, p1.vx); __stcs(reinterpret_cast<double2*>(S.f[3] + base), o);
-        o = make_double2(p0.vy, p1.vy); __stcs(reinterpret_cast<double2*>(S.f[4] + base), o);
-        o = make_double2(p0.vz, p1.vz); __stcs(reinterpret_cast<double2*>(S.f[5] + base), o);
-        const uchar2 cc = make_uchar2((unsigned char)c0, (unsigned char)c1);
-        *reinterpret_cast<uchar2*>(S.code + base) = cc;
+#pragma unroll 1
+    for (int r = 0; r < kRows; ++r) {
+        const int64_t slot = first + 32 * r + lane;
+        if (first + 32 * r >= (int64_t)cnt_s) break;
+        const bool valid = slot < (int64_t)cnt_s;
+        const size_t at = (size_t)s * (size_t)G.cap + (size_t)slot;
+        Particle p{0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0};
+        if (valid) {
+            p.x = __longlong_as_double(ld_stream(S.f[0] + at)); p.y = __longlong_as_double(ld_stream(S.f[1] + at));
+            p.z = __longlong_as_double(ld_stream(S.f[2] + at)); p.vx = __longlong_as_double(ld_stream(S.f[3] + at));
+            p.vy = __longlong_as_double(ld_stream(S.f[4] + at)); p.vz = __longlong_as_double(ld_stream(S.f[5] + at));
+            p.d = __longlong_as_double(ld_stream(S.f[6] + at));
+        }
+        bool jmp = false;
+        int code = push_particle(p, F4, G, B, dt, odd, jmp);
+        if (valid) {
+            jump |= jmp;
+            st_stream(S.f[0] + at, __double_as_longlong(p.x)); st_stream(S.f[1] + at, __double_as_longlong(p.y));
+            st_stream(S.f[2] + at, __double_as_longlong(p.z)); st_stream(S.f[3] + at, __double_as_longlong(p.vx));
+            st_stream(S.f[4] + at, __double_as_longlong(p.vy)); st_stream(S.f[5] + at, __double_as_longlong(p.vz));
+            S.code[at] = (uint8_t)code;
+        } else code = kInvalid;
+        (void)row_rank(code, valid, lane, cnt_c);
     }
     if (jump) raise(T.status, -5);
-    // a4: warp ballots -> per-code popc (lane c owns code c) -> shared -> one atomic per (tile, code)
-    const RowBallots r0 = row_ballots(v0, c0), r1 = row_ballots(v1, c1);
-    const int lane = threadIdx.x & 31;
-    if (lane < kNC) {
-        const uint32_t n = __popc(code_mask(r0, lane)) + __popc(code_mask(r1, lane));
-        if (n) atomicAdd(&s_cnt[lane], n);
-    }
-    __syncthreads();
-    if (threadIdx.x < kNC && s_cnt[threadIdx.x]) atomicAdd(&T.cnt[s * 32 + threadIdx.x], s_cnt[threadIdx.x]);
+    if (lane < kNC && cnt_c) atomicAdd(&T.cnt[s * 32 + lane], cnt_c);      // a4
 }
 
 // ---------------------------------------------------------------------------------------------
 // K2: tile pass of the migration (a5-a7), optionally with the push fused in front (a1-a4).
-//   Persistent CTAs; each takes tiles from an atomic ticket (so every predecessor of a tile is
-//   resident or finished) and maps the ticket to (subdomain, tile) through the compact prefix
-//   tile_start[] (empty tiles never get a ticket).  Per tile:
-//   - in-tile per-code stable ranks from warp ballots (lane c owns code c);
-//   - single-pass decoupled look-back over the tiles of the SAME subdomain with a 32-wide window
-//     (lane L inspects predecessor t-1-L), carrying two running sums: stayers and migrants;
-//   - stayers written in place at their compacted slot; migrants written to the subdomain's send
-//     region at (migrant prefix) + (offset of their code's run in the tile chunk) + (in-tile rank).
-//   The per-code cross-tile prefix needed by the unpack is produced afterwards by k_code_scan
-//   from tile_cnt[] (it is not on the critical path of the look-back).
-// `dep_zero` is always 0; it ties the id/field loads into the published aggregate so that a
-// tile publishes only after its loads have completed (in-place compaction safety).
+//   Persistent grid; every WARP takes tiles from an atomic ticket (so every predecessor of a tile
+//   belongs to a resident warp) and maps the ticket to (subdomain, tile) through the compact prefix
+//   tile_start[] (empty tiles never get a ticket).  The next ticket is prefetched while the current
+//   tile is processed.  Per tile:
+//   - rows of 32 particles: load (64-bit, coalesced), push (fused), stable per-code rank
+//     (row_rank), stage into the warp's private shared-memory area: stayers from the front in
+//     output order, migrants from the back in arrival order with (code, rank-in-code) beside them;
+//   - publish the tile aggregate (stayers, migrants) and the per-code byte counts;
+//   - single-pass look-back over the tiles of the SAME subdomain: two levels of aggregates (tiles of
+//     the own group of 32, then whole groups), two running sums, one lane per predecessor;
+//   - stayers written in place at their compacted slot (coalesced), migrants to the subdomain's
+//     send region at (migrant prefix) + (start of their code's run in the tile chunk) + (rank).
+//   A tile publishes only after every one of its loads has completed (the staging stores consume
+//   the loaded registers and precede the publish in program order), which makes the in-place left
+//   compaction safe: a tile writes only slots below its own end, all of which belong to tiles
+//   that have published.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t warp_sum(uint32_t v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// one window step of the look-back for one of the two running sums; returns true when a PREFIX was found
-__device__ __forceinline__ bool window_step(uint64_t w, bool beyond_start, int lane, uint32_t& excl)
-{
-    const bool is_prefix = beyond_start || ((uint32_t)(w >> 32) & 3u) == kStPrefix;
-    const unsigned pm = __ballot_sync(0xffffffffu, is_prefix);
-    const int first = pm ? (__ffs(pm) - 1) : 32;               // nearest predecessor holding a prefix
-    const uint32_t v = (lane <= first && !beyond_start) ? (uint32_t)w : 0u;
-    excl += warp_sum(v);
-    return pm != 0u;
-}
-
-// A pushed tile staged in shared memory in OUTPUT order: stayers first (stable), then the migrants
-// grouped by destination code (stable inside each code).
-struct TileBuf {
-    double f[7][kTile];
-    long long id[kTile];
+struct WarpStage {
+    unsigned long long f[8][kTile];     // x y z vx vy vz d id as raw 64-bit words, staged order
+    unsigned short meta[kTile];         // migrant a (arrival order): code | rank-in-code << 5
 };
-
-struct TileCtl {
-    uint32_t wtot[kWarps][32];      // per-warp per-code counts of the tile being pushed
-    uint32_t stay_excl;             // look-back result of the tile being resolved
-    long long sendbase;             // first send slot of its chunk, -1 = send region overflow
-    unsigned int next_ticket;
-};
-
-// Per-tile facts carried from its push to its resolve one iteration later (all CTA-uniform).
-struct TileInfo { int s, t; uint32_t n_stay, n_mig, cnt_s; bool valid; };
 
 template <bool kFused>
 __global__ void __launch_bounds__(kBlock, kMinBlocks)
-k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch,
-            unsigned long long dep_zero)
+k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
-    TileBuf* buf = reinterpret_cast<TileBuf*>(s_raw);                                   // [2]
-    uint32_t* s_tile_start = reinterpret_cast<uint32_t*>(s_raw + 2 * sizeof(TileBuf));  // [P+1]
-    __shared__ TileCtl sm;
-
-    for (int i = threadIdx.x; i <= G.P; i += kBlock) s_tile_start[i] = T.tile_start[i];
-    if (threadIdx.x == 0) sm.next_ticket = atomicAdd(T.ticket, 1u);
-    __syncthreads();
-    const unsigned int n_active = s_tile_start[G.P];
+    WarpStage* stage_all = reinterpret_cast<WarpStage*>(s_raw);
+    uint32_t* s_tile_start = reinterpret_cast<uint32_t*>(s_raw + kWarps * sizeof(WarpStage));   // [P+1] if it fits
+    const bool ts_smem = G.P <= kTileStartSmemMax;
+    if (ts_smem) {
+        for (int i = threadIdx.x; i <= G.P; i += kBlock) s_tile_start[i] = T.tile_start[i];
+        __syncthreads();                                   // the only block barrier of the kernel
+    }
+    const uint32_t* __restrict__ tstart = ts_smem ? s_tile_start : T.tile_start;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool odd = lane & 1;
+    const unsigned lt = (1u << lane) - 1u;
+    WarpStage& W = stage_all[warp];
+    const unsigned int n_active = tstart[G.P];
     const uint64_t tag = (uint64_t)(epoch << 2) << 32;
 
-    TileInfo prev; prev.valid = false; prev.s = prev.t = 0; prev.n_stay = prev.n_mig = prev.cnt_s = 0;
-    for (int it = 0;; ++it) {
-        const int b = it & 1;
-        const unsigned int g = sm.next_ticket;
-        TileInfo cur; cur.valid = g < n_active; cur.s = cur.t = 0; cur.n_stay = cur.n_mig = cur.cnt_s = 0;
-        if (!cur.valid && !prev.valid) break;
+    unsigned int g = 0;
+    if (lane == 0) g = atomicAdd(T.ticket, 1u);
+    g = __shfl_sync(0xffffffffu, g, 0);
+    while (g < n_active) {
+        int lo = 0, hi = G.P;                                       // largest s with tile_start[s] <= g
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (tstart[mid] <= g) lo = mid; else hi = mid; }
+        const int s = lo;
+        const int t = (int)(g - tstart[lo]);
+        const uint32_t cnt_s = __ldg(T.count + s);
+        const int64_t first = (int64_t)t * kTile;
+        const size_t slab0 = (size_t)s * (size_t)G.cap;
+        SubBox B;
+        if (kFused) B = sub_box(G, s);
 
-        // ============ push phase of tile g: load, (push,) rank, stage into buf[b], publish aggregate ============
-        if (cur.valid) {
-            int lo = 0, hi = G.P;                                       // largest s with tile_start[s] <= g
-            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (s_tile_start[mid] <= g) lo = mid; else hi = mid; }
-            cur.s = lo;
-            cur.t = (int)(g - s_tile_start[lo]);
-            cur.cnt_s = T.count[lo];
-            const int64_t first = (int64_t)cur.t * kTile;
-            const int64_t slot0 = first + 2 * (int64_t)threadIdx.x;
-            const size_t base = (size_t)cur.s * (size_t)G.cap + (size_t)slot0;
-            const bool v0 = slot0 < (int64_t)cur.cnt_s, v1 = slot0 + 1 < (int64_t)cur.cnt_s;
-
-            Particle p0, p1;
-            int64_t id0 = 0, id1 = 0;
-            int c0 = kStay, c1 = kStay;
-            bool jump = false;
-            unsigned long long dep = 0;
-            if (v0) {
-                double2 q[7];
-#pragma unroll
-                for (int a = 0; a < 7; ++a) q[a] = ld_stream2(S.f[a] + base);
-                const longlong2 qi = ld_stream2(S.id + base);
-                p0 = Particle{q[0].x, q[1].x, q[2].x, q[3].x, q[4].x, q[5].x, q[6].x};
-                p1 = Particle{q[0].y, q[1].y, q[2].y, q[3].y, q[4].y, q[5].y, q[6].y};
-                id0 = qi.x; id1 = qi.y;
-                if (kFused) {
-                    const SubBox B = sub_box(G, cur.s);
-                    c0 = push_particle(p0, F4, G, B, dt, jump);
-                    if (v1) c1 = push_particle(p1, F4, G, B, dt, jump);
-                } else {
-                    const uchar2 cc = *reinterpret_cast<const uchar2*>(S.code + base);
-                    c0 = min((int)cc.x, 26);
-                    c1 = v1 ? min((int)cc.y, 26) : kStay;
+        // ---------------- rows: load, (push,) rank, stage ----------------
+        uint32_t cnt_c = 0;            // lane c: particles of the tile so far with code c
+        uint32_t n_mig = 0;            // migrants of the tile so far (warp-uniform)
+        bool jump = false;
+#pragma unroll 1
+        for (int r = 0; r < kRows; ++r) {
+            if (first + 32 * r >= (int64_t)cnt_s) break;
+            const int64_t slot = first + 32 * r + lane;
+            const bool valid = slot < (int64_t)cnt_s;
+            const size_t at = slab0 + (size_t)slot;
+            Particle p{0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0};
+            unsigned long long id = 0;
+            int code = kStay;
+            if (valid) {
+                p.x = __longlong_as_double(ld_stream(S.f[0] + at)); p.y = __longlong_as_double(ld_stream(S.f[1] + at));
+                p.z = __longlong_as_double(ld_stream(S.f[2] + at)); p.vx = __longlong_as_double(ld_stream(S.f[3] + at));
+                p.vy = __longlong_as_double(ld_stream(S.f[4] + at)); p.vz = __longlong_as_double(ld_stream(S.f[5] + at));
+                p.d = __longlong_as_double(ld_stream(S.f[6] + at));
+                id = ld_stream(S.id + at);
+                if (!kFused) code = min((int)S.code[at], 26);
+            }
+            if (kFused) {
+                bool jmp = false;
+                code = push_particle(p, F4, G, B, dt, odd, jmp);
+                jump |= jmp && valid;
+            }
+            if (!valid) code = kInvalid;
+            const uint32_t rank = row_rank(code, valid, lane, cnt_c);
+            const unsigned mig_m = __ballot_sync(0xffffffffu, valid && code != kStay);
+            if (valid) {
+                uint32_t pos = rank;                                    // stayer: output order from the front
+                if (code != kStay) {
+                    const uint32_t a = n_mig + __popc(mig_m & lt);      // migrant: arrival order from the back
+                    pos = kTile - 1 - a;
+                    W.meta[a] = (unsigned short)(code | (rank << 5));
                 }
+                W.f[0][pos] = __double_as_longlong(p.x); W.f[1][pos] = __double_as_longlong(p.y);
+                W.f[2][pos] = __double_as_longlong(p.z); W.f[3][pos] = __double_as_longlong(p.vx);
+                W.f[4][pos] = __double_as_longlong(p.vy); W.f[5][pos] = __double_as_longlong(p.vz);
+                W.f[6][pos] = __double_as_longlong(p.d); W.f[7][pos] = id;
             }
-            if (jump) raise(T.status, -5);
+            n_mig += __popc(mig_m);
+        }
+        if (jump) raise(T.status, -5);
+        __syncwarp();
 
-            // in-warp ranks and per-warp totals
-            const RowBallots r0 = row_ballots(v0, c0), r1 = row_ballots(v1, c1);
-            const unsigned lt = (1u << lane) - 1u;
-            const uint32_t rank0 = __popc(code_mask(r0, c0) & lt) + __popc(code_mask(r1, c0) & lt);
-            const uint32_t rank1 = __popc(code_mask(r0, c1) & lt) + __popc(code_mask(r1, c1) & lt) + ((v0 && c0 == c1) ? 1u : 0u);
-            sm.wtot[warp][lane] = (lane < kNC) ? (uint32_t)(__popc(code_mask(r0, lane)) + __popc(code_mask(r1, lane))) : 0u;
-            __syncthreads();                                                                             // B1
-            // every warp: lane c sums code c over the warps -> its own exclusive prefix and the tile total
-            uint32_t wexcl = 0, agg = 0;
+        // ---------------- tile totals, publish ----------------
+        const uint32_t n_stay = __shfl_sync(0xffffffffu, cnt_c, kStay);
+        const uint32_t magg = (lane < kNC && lane != kStay) ? cnt_c : 0u;
+        uint32_t inc = magg;
 #pragma unroll
-            for (int w = 0; w < kWarps; ++w) { const uint32_t v = sm.wtot[w][lane]; if (w < warp) wexcl += v; agg += v; }
-            const uint32_t magg = (lane < kNC && lane != kStay) ? agg : 0u;
-            uint32_t inc = magg;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += nb;
-            }
-            cur.n_mig = __shfl_sync(0xffffffffu, inc, 31);
-            cur.n_stay = __shfl_sync(0xffffffffu, agg, kStay);
-            // position of code c's run in the staged tile: stayers at 0, migrants after them in code order
-            const uint32_t run_start = (lane == kStay) ? 0u : cur.n_stay + (inc - magg);
-            const uint32_t my_base = run_start + wexcl;            // lane c: first staged slot of this warp's code-c particles
-            TileBuf& B = buf[b];
-            if (v0) {
-                const uint32_t pos = __shfl_sync(0xffffffffu, my_base, c0) + rank0;
-                B.f[0][pos] = p0.x; B.f[1][pos] = p0.y; B.f[2][pos] = p0.z; B.f[3][pos] = p0.vx;
-                B.f[4][pos] = p0.vy; B.f[5][pos] = p0.vz; B.f[6][pos] = p0.d; B.id[pos] = id0;
-            } else (void)__shfl_sync(0xffffffffu, my_base, 0);
-            if (v1) {
-                const uint32_t pos = __shfl_sync(0xffffffffu, my_base, c1) + rank1;
-                B.f[0][pos] = p1.x; B.f[1][pos] = p1.y; B.f[2][pos] = p1.z; B.f[3][pos] = p1.vx;
-                B.f[4][pos] = p1.vy; B.f[5][pos] = p1.vz; B.f[6][pos] = p1.d; B.id[pos] = id1;
-            } else (void)__shfl_sync(0xffffffffu, my_base, 0);
-            if (warp == 0) {
-                // The staged copies above are this warp's own; the other warps' loads are ordered before the
-                // publish by barrier B1 (their ballots consumed the loaded values) -- see DESIGN.md 6.3.
-                const size_t tile_row = (size_t)cur.s * G.tiles_per_sub + cur.t;
-                T.tile_cnt[tile_row * 32 + lane] = agg;
-                if (lane < 2) {
-                    const uint32_t mine = lane == 0 ? cur.n_stay : cur.n_mig;
-                    const uint32_t st = cur.t == 0 ? kStPrefix : kStAgg;
-                    st_relaxed_u64(T.desc + tile_row * 2 + lane, tag | ((uint64_t)st << 32) | mine);
-                }
-            }
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += nb;
+        }
+        const uint32_t run_start = inc - magg;          // lane c: start of code c's run inside the tile's send chunk
+        const size_t tile_row = (size_t)s * G.tiles_per_sub + t;
+        T.tile_cnt[tile_row * 32 + lane] = (uint8_t)cnt_c;
+        if (lane < 2) {
+            const uint32_t mine = lane == 0 ? n_stay : n_mig;
+            st_relaxed_u64(T.desc + tile_row * 2 + lane, tag | (1ull << 32) | mine);
         }
 
-        // ============ resolve phase of the previous tile: windowed look-back (warp 0) ============
-        if (prev.valid && warp == 0) {
-            uint32_t excl_stay = 0, excl_mig = 0;
-            if (prev.t > 0) {
-                bool done_s = false, done_m = false;
-                for (int nearest = prev.t - 1; !(done_s && done_m); nearest -= 32) {
-                    const int j = nearest - lane;
-                    const bool beyond = j < 0;                       // before the subdomain's first tile: prefix 0
-                    uint64_t wa = 0, wb = 0;
-                    if (!beyond) {
-                        const uint64_t* pd = T.desc + ((size_t)prev.s * G.tiles_per_sub + j) * 2;
+        // ---------------- two-level aggregate look-back (no prefix chain) ----------------
+        // exclusive prefix of tile t = (aggregates of the earlier tiles of its group of 32) + (aggregates of
+        // the earlier groups).  The last tile of a group publishes the group aggregate.  Every word a tile
+        // waits for is published by a tile with a smaller ticket right after that tile's push, so the wait
+        // is a couple of L2 round trips and never a chain through other tiles' look-backs.
+        uint32_t excl_stay = 0, excl_mig = 0;
+        {
+            const int r = t & 31, grp = t >> 5;
+            if (r > 0) {
+                const bool need = lane < r;
+                const uint64_t* pd = T.desc + (tile_row - r + (need ? lane : 0)) * 2;
+                uint64_t wa = 0, wb = 0;
+                for (;;) {
+                    bool ready = true;
+                    if (need) {
                         wa = ld_relaxed_u64(pd);
                         wb = ld_relaxed_u64(pd + 1);
-                        while ((uint32_t)(wa >> 34) != epoch || ((uint32_t)(wa >> 32) & 3u) == 0u ||
-                               (uint32_t)(wb >> 34) != epoch || ((uint32_t)(wb >> 32) & 3u) == 0u) {
-                            __nanosleep(20);
-                            wa = ld_relaxed_u64(pd);
-                            wb = ld_relaxed_u64(pd + 1);
-                        }
+                        ready = (uint32_t)(wa >> 34) == epoch && (uint32_t)(wb >> 34) == epoch;
                     }
-                    if (!done_s) done_s = window_step(wa, beyond, lane, excl_stay);
-                    if (!done_m) done_m = window_step(wb, beyond, lane, excl_mig);
+                    if (__all_sync(0xffffffffu, ready)) break;
+                    __nanosleep(64);
                 }
-                if (lane < 2) {
-                    const uint32_t incl = lane == 0 ? excl_stay + prev.n_stay : excl_mig + prev.n_mig;
-                    st_relaxed_u64(T.desc + ((size_t)prev.s * G.tiles_per_sub + prev.t) * 2 + lane,
-                                   tag | ((uint64_t)kStPrefix << 32) | (uint64_t)incl);
+                excl_stay = warp_sum(need ? (uint32_t)wa : 0u);
+                excl_mig = warp_sum(need ? (uint32_t)wb : 0u);
+            }
+            if (r == 31 && lane < 2) {
+                const uint32_t tot = lane == 0 ? excl_stay + n_stay : excl_mig + n_mig;
+                st_relaxed_u64(T.gdesc + ((size_t)s * G.lbgroups_per_sub + grp) * 2 + lane, tag | (1ull << 32) | tot);
+            }
+            for (int g0 = 0; g0 < grp; g0 += 32) {
+                const bool need = g0 + lane < grp;
+                const uint64_t* pd = T.gdesc + ((size_t)s * G.lbgroups_per_sub + g0 + (need ? lane : 0)) * 2;
+                uint64_t wa = 0, wb = 0;
+                for (;;) {
+                    bool ready = true;
+                    if (need) {
+                        wa = ld_relaxed_u64(pd);
+                        wb = ld_relaxed_u64(pd + 1);
+                        ready = (uint32_t)(wa >> 34) == epoch && (uint32_t)(wb >> 34) == epoch;
+                    }
+                    if (__all_sync(0xffffffffu, ready)) break;
+                    __nanosleep(64);
                 }
+                excl_stay += warp_sum(need ? (uint32_t)wa : 0u);
+                excl_mig += warp_sum(need ? (uint32_t)wb : 0u);
             }
-            if (lane == 0) {
-                sm.stay_excl = excl_stay;
-                long long sb = (long long)prev.s * G.send_cap + (long long)excl_mig;
-                if ((long long)excl_mig + (long long)prev.n_mig > G.send_cap) { raise(T.status, -4); sb = -1; }
-                sm.sendbase = sb;
-                // next ticket: taken only after this look-back has finished, so a CTA never holds an
-                // unpublished ticket while it waits on predecessors
-                sm.next_ticket = atomicAdd(T.ticket, 1u);
-            }
-        } else if (!prev.valid && threadIdx.x == 0) {
-            sm.next_ticket = atomicAdd(T.ticket, 1u);
         }
-        __syncthreads();                                                                                 // B2
+        long long sendbase = (long long)s * G.send_cap + (long long)excl_mig;
+        if ((long long)excl_mig + (long long)n_mig > G.send_cap) { if (lane == 0) raise(T.status, -4); sendbase = -1; }
 
-        // ============ copy-out of the previous tile: staged order == output order, coalesced ============
-        if (prev.valid) {
-            const TileBuf& B = buf[b ^ 1];
-            const size_t stay_base = (size_t)prev.s * (size_t)G.cap + (size_t)sm.stay_excl;
-            const long long sendbase = sm.sendbase;
-            for (uint32_t j = threadIdx.x; j < prev.n_stay; j += kBlock) {
+        // ---------------- copy-out: stayers in place (compacted), migrants to the send region ----------------
+        {
+            const size_t stay_base = slab0 + (size_t)excl_stay;
+            for (uint32_t j = lane; j < n_stay; j += 32) {
                 const size_t dst = stay_base + j;
 #pragma unroll
-                for (int a = 0; a < 7; ++a) st_stream(S.f[a] + dst, B.f[a][j]);
-                st_stream(S.id + dst, (int64_t)B.id[j]);
+                for (int a = 0; a < 7; ++a) st_stream(S.f[a] + dst, W.f[a][j]);
+                st_stream(S.id + dst, W.f[7][j]);
             }
-            if (sendbase >= 0) {
-                for (uint32_t j = threadIdx.x; j < prev.n_mig; j += kBlock) {
-                    const size_t dst = (size_t)sendbase + j;
-                    const uint32_t src = prev.n_stay + j;
+            for (uint32_t a0 = 0; a0 < n_mig; a0 += 32) {
+                const uint32_t a = a0 + lane;
+                const bool ok = a < n_mig;
+                const uint32_t mt = ok ? W.meta[a] : 0u;
+                const uint32_t off = __shfl_sync(0xffffffffu, run_start, mt & 31u) + (mt >> 5);
+                if (ok && sendbase >= 0) {
+                    const size_t dst = (size_t)sendbase + off;
+                    const uint32_t src = kTile - 1 - a;
 #pragma unroll
-                    for (int a = 0; a < 7; ++a) st_stream(Snd.f[a] + dst, B.f[a][src]);
-                    st_stream(Snd.id + dst, (int64_t)B.id[src]);
+                    for (int q = 0; q < 7; ++q) st_stream(Snd.f[q] + dst, W.f[q][src]);
+                    st_stream(Snd.id + dst, W.f[7][src]);
                 }
             }
         }
-        __syncthreads();                                                                                 // B3
-        prev = cur;
+        __syncwarp();                                   // the staging area is reused by the next tile
+        if (lane == 0) g = atomicAdd(T.ticket, 1u);
+        g = __shfl_sync(0xffffffffu, g, 0);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2b: per-(subdomain, code) exclusive scan of tile_cnt over the tiles of the subdomain ->
-// tile_excl (used by the unpack) and the count table totals cnt[s][c] (a4/a5).  One CTA per s.
+// K2b: per-(subdomain, code) exclusive scan of tile_cnt over the tiles of the subdomain, kept at
+// group granularity (kGroup tiles) for the unpack, and the count table totals cnt[s][c] (a4/a5).
+// One CTA per subdomain, lane c owns code c.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_code_scan(Geom G, Tables T)
@@ -543,8 +599,10 @@ k_code_scan(Geom G, Tables T)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t cnt_s = T.count[s];
     const int nt = (int)((cnt_s + kTile - 1) / kTile);
-    const int chunk = (nt + 7) / 8;
-    const int t0 = min(nt, warp * chunk), t1 = min(nt, t0 + chunk);
+    const int ng = (nt + kGroup - 1) / kGroup;
+    const int gchunk = (ng + 7) / 8;
+    const int g0 = min(ng, warp * gchunk), g1 = min(ng, g0 + gchunk);
+    const int t0 = g0 * kGroup, t1 = min(nt, g1 * kGroup);
     const size_t row0 = (size_t)s * G.tiles_per_sub;
     uint32_t sum = 0;
     for (int t = t0; t < t1; ++t) sum += T.tile_cnt[(row0 + t) * 32 + lane];
@@ -552,10 +610,10 @@ k_code_scan(Geom G, Tables T)
     __syncthreads();
     uint32_t run = 0, total = 0;
     for (int w = 0; w < 8; ++w) { const uint32_t v = s_part[w][lane]; if (w < warp) run += v; total += v; }
-    for (int t = t0; t < t1; ++t) {
-        const uint32_t v = T.tile_cnt[(row0 + t) * 32 + lane];
-        T.tile_excl[(row0 + t) * 32 + lane] = run;
-        run += v;
+    for (int g = g0; g < g1; ++g) {
+        T.group_excl[((size_t)s * G.groups_per_sub + g) * 32 + lane] = run;
+        const int te = min(nt, (g + 1) * kGroup);
+        for (int t = g * kGroup; t < te; ++t) run += T.tile_cnt[(row0 + t) * 32 + lane];
     }
     if (warp == 0) T.cnt[s * 32 + lane] = total;
 }
@@ -644,62 +702,59 @@ k_table(Geom G, Tables T)
 }
 
 // ---------------------------------------------------------------------------------------------
-// K4: unpack / append (a8).  One CTA per tile chunk of the send pool; copies each code's run to
-// slab[receiver(s,c)] + recv_off[s][c] + (exclusive per-code prefix of the tile).
+// K4: unpack / append (a8).  One warp per group of kGroup tiles of one subdomain's send region;
+// lane c owns code c: it carries the exclusive prefix of its code and copies its run of every
+// tile chunk to slab[receiver(s,c)] + recv_off[s][c] + prefix.
 // ---------------------------------------------------------------------------------------------
-constexpr int kUnpackBlock = 64;
+constexpr int kUnpackWarps = 4;
 
-__global__ void __launch_bounds__(kUnpackBlock)
+__global__ void __launch_bounds__(32 * kUnpackWarps)
 k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
 {
-    const int s = blockIdx.y, t = blockIdx.x;
+    const int s = blockIdx.y;
+    const int lane = threadIdx.x & 31;
+    const int grp = blockIdx.x * kUnpackWarps + (threadIdx.x >> 5);
     const uint32_t cnt_s = T.count[s];
-    if ((int64_t)t * kTile >= (int64_t)cnt_s) return;
+    const int nt = (int)((cnt_s + kTile - 1) / kTile);
+    const int t0 = grp * kGroup;
+    if (t0 >= nt) return;
     if (*T.status != 0) return;                                 // contents unspecified after an error
-    __shared__ uint32_t s_off[32];       // start of code c inside the chunk
-    __shared__ uint32_t s_len[32];       // length of code c's run
-    __shared__ int64_t s_dst[32];        // destination slot of the first element of code c's run
-    __shared__ uint32_t s_n;
-    __shared__ int64_t s_src;
-    const int lane = threadIdx.x;
-    if (lane < 32) {
-        const size_t trow = ((size_t)s * G.tiles_per_sub + t) * 32 + lane;
-        const bool mig = lane < kNC && lane != kStay;
-        const uint32_t agg = mig ? T.tile_cnt[trow] : 0u;
-        const uint32_t exc = mig ? T.tile_excl[trow] : 0u;
-        uint32_t inc = agg, tot_excl = exc;
+    const int t1 = min(nt, t0 + kGroup);
+    const bool mig = lane < kNC && lane != kStay;
+    const size_t row0 = (size_t)s * G.tiles_per_sub;
+    uint32_t n[kGroup];
+#pragma unroll
+    for (int q = 0; q < kGroup; ++q) n[q] = (mig && t0 + q < t1) ? T.tile_cnt[(row0 + t0 + q) * 32 + lane] : 0u;
+    uint32_t pre = mig ? T.group_excl[((size_t)s * G.groups_per_sub + grp) * 32 + lane] : 0u;
+    const uint32_t roff = mig ? T.recv_off[s * 32 + lane] : 0u;
+    const size_t recv0 = mig ? (size_t)receiver_of(G, s, lane) * (size_t)G.cap + roff : 0;
+    size_t send_pos = (size_t)s * (size_t)G.send_cap + warp_sum(pre);
+#pragma unroll
+    for (int q = 0; q < kGroup; ++q) {
+        if (t0 + q >= t1) break;
+        uint32_t inc = n[q];
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
             if (lane >= o) inc += nb;
-            tot_excl += __shfl_xor_sync(0xffffffffu, tot_excl, o);
         }
-        s_off[lane] = inc - agg;
-        s_len[lane] = agg;
-        int64_t d = -1;
-        if (mig) {
-            const int r = receiver_of(G, s, lane);
-            d = (int64_t)r * G.cap + (int64_t)T.recv_off[s * 32 + lane] + (int64_t)exc;
-            // memory safety if counts were clamped after an overflow
-            if ((int64_t)T.recv_off[s * 32 + lane] + (int64_t)exc + (int64_t)agg > G.cap) d = -1;
-        }
-        s_dst[lane] = d;
-        if (lane == 31) s_n = inc;
-        if (lane == 0) s_src = (int64_t)s * G.send_cap + (int64_t)tot_excl;
-    }
-    __syncthreads();
-    const uint32_t n = s_n;
-    const int64_t src0 = s_src;
-    for (uint32_t i = threadIdx.x; i < n; i += kUnpackBlock) {
-        int c = 0;
-#pragma unroll 1
-        for (int k = 1; k < kNC; ++k) c = (s_len[k] != 0u && s_off[k] <= i) ? k : c;   // last non-empty run starting at or before i
-        if (s_dst[c] < 0) continue;
-        const size_t dst = (size_t)(s_dst[c] + (int64_t)(i - s_off[c]));
-        const size_t src = (size_t)(src0 + (int64_t)i);
+        const uint32_t ntile = __shfl_sync(0xffffffffu, inc, 31);
+        // memory safety if counts were clamped after an overflow
+        if ((uint64_t)roff + pre + n[q] <= (uint64_t)G.cap) {
+            const size_t src = send_pos + (inc - n[q]);
+            const size_t dst = recv0 + pre;
+            for (uint32_t k = 0; k < n[q]; ++k) {
+                unsigned long long v[8];
 #pragma unroll
-        for (int a = 0; a < 7; ++a) S.f[a][dst] = __ldcs(Snd.f[a] + src);
-        S.id[dst] = __ldcs(reinterpret_cast<const long long*>(Snd.id) + src);
+                for (int a = 0; a < 7; ++a) v[a] = ld_stream(Snd.f[a] + src + k);
+                v[7] = ld_stream(Snd.id + src + k);
+#pragma unroll
+                for (int a = 0; a < 7; ++a) S.f[a][dst + k] = __longlong_as_double(v[a]);
+                S.id[dst + k] = (int64_t)v[7];
+            }
+        }
+        pre += n[q];
+        send_pos += ntile;
     }
 }
 
@@ -737,17 +792,18 @@ __global__ void k_counts_out(Geom G, Tables T, int64_t* out, int64_t* prefix)
 }
 
 struct OutPtrs { double* f[7]; int64_t* id; uint8_t* code; };
+constexpr int kCopyTile = 1024;
 
-__global__ void __launch_bounds__(kBlock)
+__global__ void __launch_bounds__(256)
 k_copy_out(Geom G, Slabs S, Tables T, const int64_t* __restrict__ prefix, OutPtrs O, int codes_valid)
 {
     const int s = blockIdx.y, t = blockIdx.x;
     const int64_t cnt_s = (int64_t)T.count[s];
-    const int64_t first = (int64_t)t * kTile;
+    const int64_t first = (int64_t)t * kCopyTile;
     if (first >= cnt_s) return;
     const int64_t obase = prefix[s];
     const size_t slab0 = (size_t)s * (size_t)G.cap;
-    for (int64_t i = first + threadIdx.x; i < min(first + kTile, cnt_s); i += kBlock) {
+    for (int64_t i = first + threadIdx.x; i < min(first + kCopyTile, cnt_s); i += 256) {
 #pragma unroll
         for (int a = 0; a < 7; ++a) if (O.f[a]) O.f[a][obase + i] = S.f[a][slab0 + i];
         if (O.id) O.id[obase + i] = S.id[slab0 + i];
