@@ -31,6 +31,7 @@ struct lcs_handle {
     std::vector<cudaEvent_t>* prof;   // 4 events per recorded step, or null
     int prof_steps, prof_max;
     int grid_fused, grid_pack;         // persistent grid sizes of the tile pass
+    size_t gacc_bytes;
 };
 
 namespace {
@@ -41,7 +42,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
     size_t slab_f[7], slab_id, slab_code;
     size_t pool, pool_bytes, fluid4;
-    size_t count, cnt, recv_off, new_count, desc, gdesc, tile_start, tile_cnt, group_excl, misc, prefix;
+    size_t count, cnt, recv_off, new_count, desc, gacc, gacc_bytes, tile_start, tile_cnt, group_excl, misc, prefix;
     size_t total;
     int tiles_per_sub, groups_per_sub, lbgroups_per_sub;
     int64_t send_cap;
@@ -88,7 +89,7 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     L.recv_off = off;  off = align_up(off + P * 32 * 4);
     L.new_count = off; off = align_up(off + P * 4);
     L.desc = off;      off = align_up(off + ntiles * 2 * 8);
-    L.gdesc = off;     off = align_up(off + P * (size_t)L.lbgroups_per_sub * 2 * 8);
+    L.gacc = off;      L.gacc_bytes = P * (size_t)L.lbgroups_per_sub * 8; off = align_up(off + L.gacc_bytes);
     L.tile_start = off; off = align_up(off + (P + 1) * 4);
     L.tile_cnt = off;  off = align_up(off + ntiles * 32);
     L.group_excl = off; off = align_up(off + P * (size_t)L.groups_per_sub * 32 * 4);
@@ -100,7 +101,7 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
 
 inline size_t tile_pass_smem(int P)
 {
-    return kWarps * sizeof(WarpStage) + (P <= kTileStartSmemMax ? (size_t)(P + 1) * sizeof(uint32_t) : 0);
+    return 2 * kWarps * sizeof(WarpStage) + (P <= kTileStartSmemMax ? (size_t)(P + 1) * sizeof(uint32_t) : 0);
 }
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -120,6 +121,7 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
     cudaEvent_t* ev = rec ? h->prof->data() + 4 * h->prof_steps : nullptr;
     if (rec) cudaEventRecord(ev[0], h->stream);
     const size_t smem = tile_pass_smem(G.P);
+    cudaMemsetAsync(h->T.gacc, 0, h->gacc_bytes, h->stream);
     if (fused)
         k_tile_pass<true><<<h->grid_fused, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch);
     else
@@ -188,7 +190,8 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     h->T.recv_off = reinterpret_cast<uint32_t*>(w + L.recv_off);
     h->T.new_count = reinterpret_cast<uint32_t*>(w + L.new_count);
     h->T.desc = reinterpret_cast<uint64_t*>(w + L.desc);
-    h->T.gdesc = reinterpret_cast<uint64_t*>(w + L.gdesc);
+    h->T.gacc = reinterpret_cast<unsigned long long*>(w + L.gacc);
+    h->gacc_bytes = L.gacc_bytes;
     h->T.tile_start = reinterpret_cast<uint32_t*>(w + L.tile_start);
     h->T.tile_cnt = reinterpret_cast<uint8_t*>(w + L.tile_cnt);
     h->T.group_excl = reinterpret_cast<uint32_t*>(w + L.group_excl);

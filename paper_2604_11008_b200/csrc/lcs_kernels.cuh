@@ -24,7 +24,10 @@ namespace lcs {
 constexpr int kBlock = LCS_BLOCK;            // threads per CTA of the tile pass
 constexpr int kMinBlocks = LCS_MIN_BLOCKS;   // CTAs per SM the tile pass is compiled for
 constexpr int kWarps = kBlock / 32;
-constexpr int kRows = 4;                     // rows (particles per lane) of a warp tile
+#ifndef LCS_ROWS
+#define LCS_ROWS 2
+#endif
+constexpr int kRows = LCS_ROWS;              // rows (particles per lane) of a warp tile
 constexpr int kTile = 32 * kRows;            // particles per tile
 constexpr int kStay = 13;
 constexpr int kNC = 27;                      // destination codes
@@ -55,7 +58,7 @@ struct Tables {
     uint32_t* recv_off;                // [P*32] slot in the receiver slab where segment (s,c) starts
     uint32_t* new_count;               // [P]
     uint64_t* desc;                    // [P*tiles_per_sub*2] tile aggregates: (stay, migrant) words
-    uint64_t* gdesc;                   // [P*lbgroups_per_sub*2] aggregates of groups of 32 tiles
+    unsigned long long* gacc;          // [P*lbgroups_per_sub] accumulators of groups of 32 tiles (zeroed per launch)
     uint32_t* tile_start;              // [P+1] compact prefix of non-empty tiles per subdomain
     uint8_t* tile_cnt;                 // [P*tiles_per_sub*32] per-code count of each tile (<= 128 fits a byte)
     uint32_t* group_excl;              // [P*groups_per_sub*32] exclusive per-code prefix at each group of kGroup tiles
@@ -70,7 +73,7 @@ struct Tables {
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void raise(int* status, int code) { atomicCAS(status, 0, code); }
 
-__device__ __forceinline__ uint64_t ld_relaxed_u64(const uint64_t* p)
+__device__ __forceinline__ uint64_t ld_relaxed_u64(const void* p)
 {
     uint64_t v;
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
@@ -410,13 +413,48 @@ struct WarpStage {
     unsigned short meta[kTile];         // migrant a (arrival order): code | rank-in-code << 5
 };
 
+// What a pushed tile carries from its push to its resolve one iteration later.
+struct TileInfo {
+    int s, t;
+    uint32_t n_stay, n_mig;
+    uint32_t run_start;                 // lane c: start of code c's run inside the tile's send chunk
+};
+
+__device__ __forceinline__ ulonglong2 ld_relaxed_desc(const uint64_t* p)
+{   // both words (stay, migrant) of a descriptor in one 128-bit load
+    ulonglong2 v;
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0,%1}, [%2];" : "=l"(v.x), "=l"(v.y) : "l"(p) : "memory");
+    return v;
+}
+
+// Sum of the (stay, migrant) aggregates desc[first .. first+n), n <= 32, one lane per descriptor; spins until
+// all of them carry this launch's epoch.
+__device__ __forceinline__ void sum_descs(const uint64_t* base, int n, int lane, uint32_t epoch, uint32_t& stay,
+                                          uint32_t& mig)
+{
+    const bool need = lane < n;
+    const uint64_t* pd = base + 2 * (need ? lane : 0);
+    ulonglong2 w = make_ulonglong2(0ull, 0ull);
+    for (;;) {
+        bool ready = true;
+        if (need) {
+            w = ld_relaxed_desc(pd);
+            ready = (uint32_t)(w.x >> 34) == epoch && (uint32_t)(w.y >> 34) == epoch;
+        }
+        if (__all_sync(0xffffffffu, ready)) break;
+        __nanosleep(200);
+    }
+    stay += warp_sum(need ? (uint32_t)w.x : 0u);
+    mig += warp_sum(need ? (uint32_t)w.y : 0u);
+}
+
 template <bool kFused>
 __global__ void __launch_bounds__(kBlock, kMinBlocks)
 k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
-    WarpStage* stage_all = reinterpret_cast<WarpStage*>(s_raw);
-    uint32_t* s_tile_start = reinterpret_cast<uint32_t*>(s_raw + kWarps * sizeof(WarpStage));   // [P+1] if it fits
+    WarpStage* stage_all = reinterpret_cast<WarpStage*>(s_raw);                                     // [kWarps][2]
+    uint32_t* s_tile_start = reinterpret_cast<uint32_t*>(s_raw + 2 * kWarps * sizeof(WarpStage));   // [P+1] if it fits
     const bool ts_smem = G.P <= kTileStartSmemMax;
     if (ts_smem) {
         for (int i = threadIdx.x; i <= G.P; i += kBlock) s_tile_start[i] = T.tile_start[i];
@@ -426,151 +464,139 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool odd = lane & 1;
     const unsigned lt = (1u << lane) - 1u;
-    WarpStage& W = stage_all[warp];
     const unsigned int n_active = tstart[G.P];
-    const uint64_t tag = (uint64_t)(epoch << 2) << 32;
+    const uint64_t tag = ((uint64_t)(epoch << 2) << 32) | (1ull << 32);
 
     unsigned int g = 0;
     if (lane == 0) g = atomicAdd(T.ticket, 1u);
     g = __shfl_sync(0xffffffffu, g, 0);
-    while (g < n_active) {
-        int lo = 0, hi = G.P;                                       // largest s with tile_start[s] <= g
-        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (tstart[mid] <= g) lo = mid; else hi = mid; }
-        const int s = lo;
-        const int t = (int)(g - tstart[lo]);
-        const uint32_t cnt_s = __ldg(T.count + s);
-        const int64_t first = (int64_t)t * kTile;
-        const size_t slab0 = (size_t)s * (size_t)G.cap;
-        SubBox B;
-        if (kFused) B = sub_box(G, s);
+    TileInfo pend;
+    pend.s = pend.t = 0; pend.n_stay = pend.n_mig = pend.run_start = 0;
+    bool have_pend = false;
+    int buf = 0;
+    for (;;) {
+        const bool have = g < n_active;
+        if (!have && !have_pend) break;
+        TileInfo cur = pend;
 
-        // ---------------- rows: load, (push,) rank, stage ----------------
-        uint32_t cnt_c = 0;            // lane c: particles of the tile so far with code c
-        uint32_t n_mig = 0;            // migrants of the tile so far (warp-uniform)
-        bool jump = false;
+        // ================= push of tile g: load, (push,) rank, stage, publish the aggregate =================
+        if (have) {
+            WarpStage& W = stage_all[2 * warp + buf];
+            int lo = 0, hi = G.P;                                       // largest s with tile_start[s] <= g
+            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (tstart[mid] <= g) lo = mid; else hi = mid; }
+            const int s = lo;
+            const int t = (int)(g - tstart[lo]);
+            const uint32_t cnt_s = __ldg(T.count + s);
+            const int64_t first = (int64_t)t * kTile;
+            const size_t slab0 = (size_t)s * (size_t)G.cap;
+            SubBox B;
+            if (kFused) B = sub_box(G, s);
+            uint32_t cnt_c = 0;            // lane c: particles of the tile so far with code c
+            uint32_t n_mig = 0;            // migrants of the tile so far (warp-uniform)
+            bool jump = false;
 #pragma unroll 1
-        for (int r = 0; r < kRows; ++r) {
-            if (first + 32 * r >= (int64_t)cnt_s) break;
-            const int64_t slot = first + 32 * r + lane;
-            const bool valid = slot < (int64_t)cnt_s;
-            const size_t at = slab0 + (size_t)slot;
-            Particle p{0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0};
-            unsigned long long id = 0;
-            int code = kStay;
-            if (valid) {
-                p.x = __longlong_as_double(ld_stream(S.f[0] + at)); p.y = __longlong_as_double(ld_stream(S.f[1] + at));
-                p.z = __longlong_as_double(ld_stream(S.f[2] + at)); p.vx = __longlong_as_double(ld_stream(S.f[3] + at));
-                p.vy = __longlong_as_double(ld_stream(S.f[4] + at)); p.vz = __longlong_as_double(ld_stream(S.f[5] + at));
-                p.d = __longlong_as_double(ld_stream(S.f[6] + at));
-                id = ld_stream(S.id + at);
-                if (!kFused) code = min((int)S.code[at], 26);
-            }
-            if (kFused) {
-                bool jmp = false;
-                code = push_particle(p, F4, G, B, dt, odd, jmp);
-                jump |= jmp && valid;
-            }
-            if (!valid) code = kInvalid;
-            const uint32_t rank = row_rank(code, valid, lane, cnt_c);
-            const unsigned mig_m = __ballot_sync(0xffffffffu, valid && code != kStay);
-            if (valid) {
-                uint32_t pos = rank;                                    // stayer: output order from the front
-                if (code != kStay) {
-                    const uint32_t a = n_mig + __popc(mig_m & lt);      // migrant: arrival order from the back
-                    pos = kTile - 1 - a;
-                    W.meta[a] = (unsigned short)(code | (rank << 5));
+            for (int r = 0; r < kRows; ++r) {
+                if (first + 32 * r >= (int64_t)cnt_s) break;
+                const int64_t slot = first + 32 * r + lane;
+                const bool valid = slot < (int64_t)cnt_s;
+                const size_t at = slab0 + (size_t)slot;
+                Particle p{0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0};
+                unsigned long long id = 0;
+                int code = kStay;
+                if (valid) {
+                    p.x = __longlong_as_double(ld_stream(S.f[0] + at)); p.y = __longlong_as_double(ld_stream(S.f[1] + at));
+                    p.z = __longlong_as_double(ld_stream(S.f[2] + at)); p.vx = __longlong_as_double(ld_stream(S.f[3] + at));
+                    p.vy = __longlong_as_double(ld_stream(S.f[4] + at)); p.vz = __longlong_as_double(ld_stream(S.f[5] + at));
+                    p.d = __longlong_as_double(ld_stream(S.f[6] + at));
+                    id = ld_stream(S.id + at);
+                    if (!kFused) code = min((int)S.code[at], 26);
                 }
-                W.f[0][pos] = __double_as_longlong(p.x); W.f[1][pos] = __double_as_longlong(p.y);
-                W.f[2][pos] = __double_as_longlong(p.z); W.f[3][pos] = __double_as_longlong(p.vx);
-                W.f[4][pos] = __double_as_longlong(p.vy); W.f[5][pos] = __double_as_longlong(p.vz);
-                W.f[6][pos] = __double_as_longlong(p.d); W.f[7][pos] = id;
-            }
-            n_mig += __popc(mig_m);
-        }
-        if (jump) raise(T.status, -5);
-        __syncwarp();
-
-        // ---------------- tile totals, publish ----------------
-        const uint32_t n_stay = __shfl_sync(0xffffffffu, cnt_c, kStay);
-        const uint32_t magg = (lane < kNC && lane != kStay) ? cnt_c : 0u;
-        uint32_t inc = magg;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += nb;
-        }
-        const uint32_t run_start = inc - magg;          // lane c: start of code c's run inside the tile's send chunk
-        const size_t tile_row = (size_t)s * G.tiles_per_sub + t;
-        T.tile_cnt[tile_row * 32 + lane] = (uint8_t)cnt_c;
-        if (lane < 2) {
-            const uint32_t mine = lane == 0 ? n_stay : n_mig;
-            st_relaxed_u64(T.desc + tile_row * 2 + lane, tag | (1ull << 32) | mine);
-        }
-
-        // ---------------- two-level aggregate look-back (no prefix chain) ----------------
-        // exclusive prefix of tile t = (aggregates of the earlier tiles of its group of 32) + (aggregates of
-        // the earlier groups).  The last tile of a group publishes the group aggregate.  Every word a tile
-        // waits for is published by a tile with a smaller ticket right after that tile's push, so the wait
-        // is a couple of L2 round trips and never a chain through other tiles' look-backs.
-        uint32_t excl_stay = 0, excl_mig = 0;
-        {
-            const int r = t & 31, grp = t >> 5;
-            if (r > 0) {
-                const bool need = lane < r;
-                const uint64_t* pd = T.desc + (tile_row - r + (need ? lane : 0)) * 2;
-                uint64_t wa = 0, wb = 0;
-                for (;;) {
-                    bool ready = true;
-                    if (need) {
-                        wa = ld_relaxed_u64(pd);
-                        wb = ld_relaxed_u64(pd + 1);
-                        ready = (uint32_t)(wa >> 34) == epoch && (uint32_t)(wb >> 34) == epoch;
+                if (kFused) {
+                    bool jmp = false;
+                    code = push_particle(p, F4, G, B, dt, odd, jmp);
+                    jump |= jmp && valid;
+                }
+                if (!valid) code = kInvalid;
+                const uint32_t rank = row_rank(code, valid, lane, cnt_c);
+                const unsigned mig_m = __ballot_sync(0xffffffffu, valid && code != kStay);
+                if (valid) {
+                    uint32_t pos = rank;                                    // stayer: output order from the front
+                    if (code != kStay) {
+                        const uint32_t a = n_mig + __popc(mig_m & lt);      // migrant: arrival order from the back
+                        pos = kTile - 1 - a;
+                        W.meta[a] = (unsigned short)(code | (rank << 5));
                     }
-                    if (__all_sync(0xffffffffu, ready)) break;
-                    __nanosleep(64);
+                    W.f[0][pos] = __double_as_longlong(p.x); W.f[1][pos] = __double_as_longlong(p.y);
+                    W.f[2][pos] = __double_as_longlong(p.z); W.f[3][pos] = __double_as_longlong(p.vx);
+                    W.f[4][pos] = __double_as_longlong(p.vy); W.f[5][pos] = __double_as_longlong(p.vz);
+                    W.f[6][pos] = __double_as_longlong(p.d); W.f[7][pos] = id;
                 }
-                excl_stay = warp_sum(need ? (uint32_t)wa : 0u);
-                excl_mig = warp_sum(need ? (uint32_t)wb : 0u);
+                n_mig += __popc(mig_m);
             }
-            if (r == 31 && lane < 2) {
-                const uint32_t tot = lane == 0 ? excl_stay + n_stay : excl_mig + n_mig;
-                st_relaxed_u64(T.gdesc + ((size_t)s * G.lbgroups_per_sub + grp) * 2 + lane, tag | (1ull << 32) | tot);
+            if (jump) raise(T.status, -5);
+            __syncwarp();
+            // tile totals; publish the aggregate and the per-code byte counts
+            const uint32_t n_stay = __shfl_sync(0xffffffffu, cnt_c, kStay);
+            const uint32_t magg = (lane < kNC && lane != kStay) ? cnt_c : 0u;
+            uint32_t inc = magg;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += nb;
             }
+            const size_t tile_row = (size_t)s * G.tiles_per_sub + t;
+            T.tile_cnt[tile_row * 32 + lane] = (uint8_t)cnt_c;
+            if (lane < 2) st_relaxed_u64(T.desc + tile_row * 2 + lane, tag | (lane == 0 ? n_stay : n_mig));
+            if (lane == 2)      // group accumulator [tiles done : 24 | migrants : 20 | stayers : 20], zeroed before the launch
+                atomicAdd(T.gacc + (size_t)s * G.lbgroups_per_sub + (t >> 5),
+                          (1ull << 40) | ((unsigned long long)n_mig << 20) | (unsigned long long)n_stay);
+            cur.s = s; cur.t = t; cur.n_stay = n_stay; cur.n_mig = n_mig; cur.run_start = inc - magg;
+        }
+
+        // ================= resolve of the previous tile: look-back, then copy-out =================
+        // Two-level aggregate look-back (no prefix chain): exclusive prefix of tile t = aggregates of the
+        // earlier tiles of its group of 32 + accumulators of the earlier groups (every tile adds its
+        // aggregate to its group's accumulator with one 64-bit atomic right after its push).  Every word
+        // waited for is produced by the PUSH of a tile with a smaller ticket -- never by another tile's
+        // resolve -- and this warp has pushed a whole tile in between.
+        unsigned int g_next = 0xffffffffu;
+        if (have_pend) {
+            const WarpStage& W = stage_all[2 * warp + (buf ^ 1)];
+            const int s = pend.s, t = pend.t;
+            const size_t tile_row = (size_t)s * G.tiles_per_sub + t;
+            const int r = t & 31, grp = t >> 5;
+            uint32_t excl_stay = 0, excl_mig = 0;
+            if (r > 0) sum_descs(T.desc + (tile_row - r) * 2, r, lane, epoch, excl_stay, excl_mig);
+            const unsigned long long* ga = T.gacc + (size_t)s * G.lbgroups_per_sub;
             for (int g0 = 0; g0 < grp; g0 += 32) {
                 const bool need = g0 + lane < grp;
-                const uint64_t* pd = T.gdesc + ((size_t)s * G.lbgroups_per_sub + g0 + (need ? lane : 0)) * 2;
-                uint64_t wa = 0, wb = 0;
+                unsigned long long w = 0;
                 for (;;) {
                     bool ready = true;
-                    if (need) {
-                        wa = ld_relaxed_u64(pd);
-                        wb = ld_relaxed_u64(pd + 1);
-                        ready = (uint32_t)(wa >> 34) == epoch && (uint32_t)(wb >> 34) == epoch;
-                    }
+                    if (need) { w = ld_relaxed_u64(ga + g0 + lane); ready = (w >> 40) == 32ull; }
                     if (__all_sync(0xffffffffu, ready)) break;
-                    __nanosleep(64);
+                    __nanosleep(200);
                 }
-                excl_stay += warp_sum(need ? (uint32_t)wa : 0u);
-                excl_mig += warp_sum(need ? (uint32_t)wb : 0u);
+                excl_stay += warp_sum(need ? (uint32_t)(w & 0xfffffull) : 0u);
+                excl_mig += warp_sum(need ? (uint32_t)((w >> 20) & 0xfffffull) : 0u);
             }
-        }
-        long long sendbase = (long long)s * G.send_cap + (long long)excl_mig;
-        if ((long long)excl_mig + (long long)n_mig > G.send_cap) { if (lane == 0) raise(T.status, -4); sendbase = -1; }
-
-        // ---------------- copy-out: stayers in place (compacted), migrants to the send region ----------------
-        {
-            const size_t stay_base = slab0 + (size_t)excl_stay;
-            for (uint32_t j = lane; j < n_stay; j += 32) {
+            // next ticket: requested only now, so that no ticket is held unpublished through a look-back wait
+            if (have && lane == 0) g_next = atomicAdd(T.ticket, 1u);
+            long long sendbase = (long long)s * G.send_cap + (long long)excl_mig;
+            if ((long long)excl_mig + (long long)pend.n_mig > G.send_cap) { if (lane == 0) raise(T.status, -4); sendbase = -1; }
+            // copy-out: stayers in place (compacted, coalesced), migrants to the send region
+            const size_t stay_base = (size_t)s * (size_t)G.cap + (size_t)excl_stay;
+            for (uint32_t j = lane; j < pend.n_stay; j += 32) {
                 const size_t dst = stay_base + j;
 #pragma unroll
                 for (int a = 0; a < 7; ++a) st_stream(S.f[a] + dst, W.f[a][j]);
                 st_stream(S.id + dst, W.f[7][j]);
             }
-            for (uint32_t a0 = 0; a0 < n_mig; a0 += 32) {
+            for (uint32_t a0 = 0; a0 < pend.n_mig; a0 += 32) {
                 const uint32_t a = a0 + lane;
-                const bool ok = a < n_mig;
+                const bool ok = a < pend.n_mig;
                 const uint32_t mt = ok ? W.meta[a] : 0u;
-                const uint32_t off = __shfl_sync(0xffffffffu, run_start, mt & 31u) + (mt >> 5);
+                const uint32_t off = __shfl_sync(0xffffffffu, pend.run_start, mt & 31u) + (mt >> 5);
                 if (ok && sendbase >= 0) {
                     const size_t dst = (size_t)sendbase + off;
                     const uint32_t src = kTile - 1 - a;
@@ -579,10 +605,14 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     st_stream(Snd.id + dst, W.f[7][src]);
                 }
             }
+        } else if (have && lane == 0) {
+            g_next = atomicAdd(T.ticket, 1u);
         }
-        __syncwarp();                                   // the staging area is reused by the next tile
-        if (lane == 0) g = atomicAdd(T.ticket, 1u);
-        g = __shfl_sync(0xffffffffu, g, 0);
+        __syncwarp();                                   // the staging area just copied out is reused next
+        g = __shfl_sync(0xffffffffu, g_next, 0);        // 0xffffffff once the tickets have run out
+        pend = cur;
+        have_pend = have;
+        buf ^= 1;
     }
 }
 
