@@ -19,13 +19,13 @@ namespace lcs {
 #define LCS_BLOCK 256
 #endif
 #ifndef LCS_MIN_BLOCKS
-#define LCS_MIN_BLOCKS 3
+#define LCS_MIN_BLOCKS 2
 #endif
 constexpr int kBlock = LCS_BLOCK;            // threads per CTA of the tile pass
 constexpr int kMinBlocks = LCS_MIN_BLOCKS;   // CTAs per SM the tile pass is compiled for
 constexpr int kWarps = kBlock / 32;
 #ifndef LCS_ROWS
-#define LCS_ROWS 2
+#define LCS_ROWS 3
 #endif
 constexpr int kRows = LCS_ROWS;              // rows (particles per lane) of a warp tile
 constexpr int kTile = 32 * kRows;            // particles per tile
@@ -256,7 +256,11 @@ __device__ __forceinline__ int advance_axis(double& a, double& v, double U, doub
 __device__ __forceinline__ int push_particle(Particle& p, const double* __restrict__ F4, const Geom& G,
                                              const SubBox& B, double dt, bool odd, bool& jump)
 {
+#ifdef LCS_X_NOGATHER
+    Vec3 U; U.x = U.y = U.z = 0.0;
+#else
     const Vec3 U = gather_pair(F4, G.N, G.inv_dx, p.x, p.y, p.z, odd);
+#endif
     const double tau = (G.K_tau * p.d) * p.d;     // tau_p = (rho_p/rho) d^2 / (18 nu)
     const double zz = dt / tau;
     const double alpha = exp_neg(zz);
@@ -408,6 +412,34 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
 //   compaction safe: a tile writes only slots below its own end, all of which belong to tiles
 //   that have published.
 // ---------------------------------------------------------------------------------------------
+// ---------------------------------------------------------------------------------------------
+// Fluid brick prefetch.  The tiles of subdomain s are processed in ticket order, so the 8.8 MB brick
+// of fluid records that subdomain s+1 will gather from can be pulled into L2 ahead of time with
+// full-line prefetches, one share per tile of s, instead of being demand-missed one 32-byte sector
+// at a time by the first particle that touches each cell.  Runs along z are contiguous in the
+// internal layout; the two seam planes in z are left to demand misses.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void prefetch_brick_share(const double* __restrict__ F4, const Geom& G, int q, uint32_t share,
+                                                     uint32_t nshares, int lane)
+{
+    const int qx = q % G.Px, qy = (q / G.Px) % G.Py, qz = q / (G.Px * G.Py);
+    const int ka = max(0, qz * G.nz - 1), kb = min(G.N - 1, qz * G.nz + G.nz);        // inclusive
+    const uint32_t nrun = (uint32_t)(G.nx + 2) * (uint32_t)(G.ny + 2);                 // (i,j) columns of the brick
+    const uint32_t per = (nrun + nshares - 1) / nshares;                               // columns per share
+    const uint32_t r0 = share * per, r1 = min(nrun, r0 + min(per, 8u));                // at most 8 columns per tile
+    for (uint32_t rj = r0; rj < r1; ++rj) {                                            // warp-uniform
+        const int ii = (int)(rj / (uint32_t)(G.ny + 2)), jj = (int)(rj % (uint32_t)(G.ny + 2));
+        int i = qx * G.nx - 1 + ii, j = qy * G.ny - 1 + jj;
+        i = i < 0 ? i + G.N : (i >= G.N ? i - G.N : i);
+        j = j < 0 ? j + G.N : (j >= G.N ? j - G.N : j);
+        const size_t col = ((size_t)i * G.N + j) * G.N;
+        const uintptr_t a0 = reinterpret_cast<uintptr_t>(F4 + 4 * (col + ka)) & ~(uintptr_t)127;
+        const uintptr_t a1 = reinterpret_cast<uintptr_t>(F4 + 4 * (col + kb + 1));
+        for (uintptr_t a = a0 + (uintptr_t)lane * 128; a < a1; a += 32 * 128)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+    }
+}
+
 struct WarpStage {
     unsigned long long f[8][kTile];     // x y z vx vy vz d id as raw 64-bit words, staged order
     unsigned short meta[kTile];         // migrant a (arrival order): code | rank-in-code << 5
@@ -490,7 +522,10 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             const int64_t first = (int64_t)t * kTile;
             const size_t slab0 = (size_t)s * (size_t)G.cap;
             SubBox B;
-            if (kFused) B = sub_box(G, s);
+            if (kFused) {
+                B = sub_box(G, s);
+                if (s + 1 < G.P) prefetch_brick_share(F4, G, s + 1, (uint32_t)t, (cnt_s + kTile - 1) / kTile, lane);
+            }
             uint32_t cnt_c = 0;            // lane c: particles of the tile so far with code c
             uint32_t n_mig = 0;            // migrants of the tile so far (warp-uniform)
             bool jump = false;
@@ -559,7 +594,25 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
         // aggregate to its group's accumulator with one 64-bit atomic right after its push).  Every word
         // waited for is produced by the PUSH of a tile with a smaller ticket -- never by another tile's
         // resolve -- and this warp has pushed a whole tile in between.
+        // Next ticket: taken right after this tile's aggregate is out; its tile's particle lines are
+        // prefetched into L2 while the previous tile is resolved.
         unsigned int g_next = 0xffffffffu;
+        if (have) {
+            if (lane == 0) g_next = atomicAdd(T.ticket, 1u);
+            g_next = __shfl_sync(0xffffffffu, g_next, 0);
+            if (g_next < n_active) {
+                int plo = cur.s, phi = G.P;
+                while (phi - plo > 1) { const int mid = (plo + phi) >> 1; if (tstart[mid] <= g_next) plo = mid; else phi = mid; }
+                const size_t pat = (size_t)plo * (size_t)G.cap + (size_t)(g_next - tstart[plo]) * kTile;
+                const char* base[8] = {reinterpret_cast<const char*>(S.f[0]), reinterpret_cast<const char*>(S.f[1]),
+                                       reinterpret_cast<const char*>(S.f[2]), reinterpret_cast<const char*>(S.f[3]),
+                                       reinterpret_cast<const char*>(S.f[4]), reinterpret_cast<const char*>(S.f[5]),
+                                       reinterpret_cast<const char*>(S.f[6]), reinterpret_cast<const char*>(S.id)};
+#pragma unroll
+                for (int fld = 0; fld < 8; ++fld)
+                    if (lane < 2 * kRows) asm volatile("prefetch.global.L2 [%0];" ::"l"(base[fld] + pat * 8 + (size_t)lane * 128));
+            }
+        }
         if (have_pend) {
             const WarpStage& W = stage_all[2 * warp + (buf ^ 1)];
             const int s = pend.s, t = pend.t;
@@ -580,12 +633,13 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 excl_stay += warp_sum(need ? (uint32_t)(w & 0xfffffull) : 0u);
                 excl_mig += warp_sum(need ? (uint32_t)((w >> 20) & 0xfffffull) : 0u);
             }
-            // next ticket: requested only now, so that no ticket is held unpublished through a look-back wait
-            if (have && lane == 0) g_next = atomicAdd(T.ticket, 1u);
             long long sendbase = (long long)s * G.send_cap + (long long)excl_mig;
             if ((long long)excl_mig + (long long)pend.n_mig > G.send_cap) { if (lane == 0) raise(T.status, -4); sendbase = -1; }
             // copy-out: stayers in place (compacted, coalesced), migrants to the send region
             const size_t stay_base = (size_t)s * (size_t)G.cap + (size_t)excl_stay;
+#ifdef LCS_X_NOSTORE
+            if (excl_stay == 0xffffffffu)
+#endif
             for (uint32_t j = lane; j < pend.n_stay; j += 32) {
                 const size_t dst = stay_base + j;
 #pragma unroll
@@ -605,11 +659,9 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     st_stream(Snd.id + dst, W.f[7][src]);
                 }
             }
-        } else if (have && lane == 0) {
-            g_next = atomicAdd(T.ticket, 1u);
         }
         __syncwarp();                                   // the staging area just copied out is reused next
-        g = __shfl_sync(0xffffffffu, g_next, 0);        // 0xffffffff once the tickets have run out
+        g = g_next;                                     // 0xffffffff once the tickets have run out
         pend = cur;
         have_pend = have;
         buf ^= 1;
