@@ -32,7 +32,7 @@ constexpr int kTile = 32 * kRows;            // particles per tile
 constexpr int kStay = 13;
 constexpr int kNC = 27;                      // destination codes
 constexpr int kInvalid = 31;                 // code of a lane beyond the slab's count
-constexpr int kGroup = 16;                   // tiles per unpack warp
+constexpr int kGroup = 8;                    // tiles per unpack warp
 constexpr int kTileStartSmemMax = 2048;      // tile_start[] is mirrored in shared memory up to this P
 
 // Look-back descriptor word: [ epoch:30 | valid:2 | value:32 ]
@@ -788,7 +788,7 @@ k_table(Geom G, Tables T)
 // lane c owns code c: it carries the exclusive prefix of its code and copies its run of every
 // tile chunk to slab[receiver(s,c)] + recv_off[s][c] + prefix.
 // ---------------------------------------------------------------------------------------------
-constexpr int kUnpackWarps = 4;
+constexpr int kUnpackWarps = 2;
 
 __global__ void __launch_bounds__(32 * kUnpackWarps)
 k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
@@ -810,7 +810,11 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
     uint32_t pre = mig ? T.group_excl[((size_t)s * G.groups_per_sub + grp) * 32 + lane] : 0u;
     const uint32_t roff = mig ? T.recv_off[s * 32 + lane] : 0u;
     const size_t recv0 = mig ? (size_t)receiver_of(G, s, lane) * (size_t)G.cap + roff : 0;
-    size_t send_pos = (size_t)s * (size_t)G.send_cap + warp_sum(pre);
+    // phase 1: destination slot of every migrant of the group, in send-region order (shared memory list)
+    __shared__ unsigned long long s_dst[kUnpackWarps][kGroup * kTile];
+    unsigned long long* dstl = s_dst[threadIdx.x >> 5];
+    const size_t send0 = (size_t)s * (size_t)G.send_cap + warp_sum(pre);
+    uint32_t nlist = 0;
 #pragma unroll
     for (int q = 0; q < kGroup; ++q) {
         if (t0 + q >= t1) break;
@@ -821,22 +825,26 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
             if (lane >= o) inc += nb;
         }
         const uint32_t ntile = __shfl_sync(0xffffffffu, inc, 31);
-        // memory safety if counts were clamped after an overflow
-        if ((uint64_t)roff + pre + n[q] <= (uint64_t)G.cap) {
-            const size_t src = send_pos + (inc - n[q]);
-            const size_t dst = recv0 + pre;
-            for (uint32_t k = 0; k < n[q]; ++k) {
-                unsigned long long v[8];
-#pragma unroll
-                for (int a = 0; a < 7; ++a) v[a] = ld_stream(Snd.f[a] + src + k);
-                v[7] = ld_stream(Snd.id + src + k);
-#pragma unroll
-                for (int a = 0; a < 7; ++a) S.f[a][dst + k] = __longlong_as_double(v[a]);
-                S.id[dst + k] = (int64_t)v[7];
-            }
-        }
+        // memory safety if counts were clamped after an overflow: such migrants are dropped
+        const bool fits = (uint64_t)roff + pre + n[q] <= (uint64_t)G.cap;
+        const uint32_t at = nlist + (inc - n[q]);
+        for (uint32_t k = 0; k < n[q]; ++k) dstl[at + k] = fits ? (unsigned long long)(recv0 + pre + k) : ~0ull;
         pre += n[q];
-        send_pos += ntile;
+        nlist += ntile;
+    }
+    __syncwarp();
+    // phase 2: one lane per migrant; the reads from the send region are contiguous across lanes
+    for (uint32_t i = lane; i < nlist; i += 32) {
+        const unsigned long long dst = dstl[i];
+        if (dst == ~0ull) continue;
+        const size_t src = send0 + i;
+        unsigned long long v[8];
+#pragma unroll
+        for (int a = 0; a < 7; ++a) v[a] = ld_stream(Snd.f[a] + src);
+        v[7] = ld_stream(Snd.id + src);
+#pragma unroll
+        for (int a = 0; a < 7; ++a) S.f[a][dst] = __longlong_as_double(v[a]);
+        S.id[dst] = (int64_t)v[7];
     }
 }
 
