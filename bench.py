@@ -87,6 +87,16 @@ class ClockSampler:
         return out
 
 
+def max_over_ranks(value, dist, device):
+    """MAX of a python float over the ranks of the default process group (identity when dist is None)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def pick_device():
     import torch
     rank = int(os.environ.get("RANK", "0"))
@@ -203,10 +213,7 @@ def run_cuda(args):
     if err or n_tot != n:
         print(f"bench.py: step failed: sticky status {err}, total {n_tot}", file=sys.stderr)
         return 3
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist, dev)
     ms_step = ms_total / args.steps
     value = world * n * args.steps / (ms_total * 1e-3)
     m = n_mig / n
@@ -233,10 +240,7 @@ def run_cuda(args):
         t1.record()
         barrier()
         ms_e2e = t0.elapsed_time(t1)
-        if dist is not None:
-            t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e2e = float(t.item())
+        ms_e2e = max_over_ranks(ms_e2e, dist, dev)
         assert int(h_counts.sum()) == n
         e2e = {"value": world * n * args.e2e_steps / (ms_e2e * 1e-3), "unit": "particles/s",
                "h2d_bytes_per_step": 64 * n, "d2h_bytes_per_step": 64 * n + 8 * P,

@@ -280,3 +280,115 @@ def test_medium_shape_sample(torch_cuda, oracle_lib):
     frac = o.n_migrated_last / cfg["n"]
     assert 0.02 < frac < 0.09
     dev.close()
+
+
+def _recipe_pair(torch, oracle_lib, name, n, N, **override):
+    """A BASELINE.json recipe at a size the oracle finishes in seconds; capacity from the actual occupancy."""
+    from workloads import gen
+    cfg = gen.scaled_config(gen.get_config(name), n=n, N=N)
+    cfg.update(override)
+    wl = gen.make_workload(cfg, device="cuda")
+    fluid = [wl[k].cpu().numpy() for k in "uvw"]
+    parts = {k: v.cpu().numpy() for k, v in wl["particles"].items()}
+    o0 = oracle_lib.Oracle(cfg["N"], *cfg["P"], 2)
+    own = np.array([o0.owner(*xyz) for xyz in zip(parts["x"][::37], parts["y"][::37], parts["z"][::37])])
+    o0.close()
+    nP = cfg["P"][0] * cfg["P"][1] * cfg["P"][2]
+    cap = int(2 * (np.bincount(own, minlength=nP).max() * 37 * 1.6 // 2) + 512)
+    o, dev, rc = make_pair(torch, oracle_lib, cfg["N"], cfg["P"], cap, fluid, parts, g=cfg["g"])
+    assert rc == 0
+    return cfg, o, dev
+
+
+def test_clustered_shape_sample(torch_cuda, oracle_lib):
+    """Clustered's recipe (Gaussian clumps, sigma = 2 cells, wide radius distribution): strongly non-uniform
+    slab and migrant counts, ragged tiles everywhere."""
+    cfg, o, dev = _recipe_pair(torch_cuda, oracle_lib, "Clustered", n=393216 + 77, N=64, clumps=48)
+    counts0 = o.counts()
+    assert counts0.max() > 3 * max(1, np.median(counts0))          # the recipe really is non-uniform
+    for step in range(4):
+        dev.step_fused(cfg["dt"])
+        assert o.step(cfg["dt"]) == 0
+        assert dev.get_status() == (0, cfg["n"], o.n_migrated_last)
+    compare_packed(dev, o, "clustered sample")
+    dev.close()
+
+
+def test_stress_shape_sample(torch_cuda, oracle_lib):
+    """Stress's recipe (8x8x8, ~30 % migrants per step, >= 10 % of them to edge/corner neighbours)."""
+    cfg, o, dev = _recipe_pair(torch_cuda, oracle_lib, "Stress", n=786432 + 5, N=64)
+    for step in range(3):
+        dev.particle_step(cfg["dt"])
+        assert o.push(cfg["dt"]) == 0
+        tab = dev.get_count_table().cpu().numpy()
+        assert np.array_equal(tab, o.cnt_table())
+        dev.migrate()
+        assert o.migrate() == 0
+        assert dev.get_status() == (0, cfg["n"], o.n_migrated_last)
+    mig = tab.sum(axis=0)
+    mig[13] = 0
+    faces = mig[[4, 10, 12, 14, 16, 22]].sum()
+    assert 0.2 < mig.sum() / cfg["n"] < 0.4
+    assert (mig.sum() - faces) / mig.sum() >= 0.10
+    compare_packed(dev, o, "stress sample")
+    dev.close()
+
+
+@pytest.mark.slow
+def test_large_full_size_properties(torch_cuda, oracle_lib):
+    """BASELINE.json's Large at full size (2^26 particles, 512^3, 8x8x8, capacity 1.25x) in the launch
+    configuration bench.py times.  Properties that hold at any size + a sample recomputed by the oracle."""
+    torch = torch_cuda
+    from workloads import gen
+    from paper_2604_11008_b200 import LCS
+    cfg = gen.get_config("Large")
+    n, N, P = cfg["n"], cfg["N"], cfg["P"]
+    nP = P[0] * P[1] * P[2]
+    wl = gen.make_workload(cfg, device="cuda")
+    dev = LCS(N, *P, cfg["capacity"], g=cfg["g"])
+    dev.set_fluid(wl["u"], wl["v"], wl["w"])
+    parts = wl["particles"]
+    dev.set_particles(*(parts[k] for k in F8))
+    assert dev.get_status()[:2] == (0, n)
+    before = dev.get_particles(n)
+    slab_of = lambda c: torch.repeat_interleave(torch.arange(nP, device="cuda"), c)
+    prev_slab = torch.empty(n, dtype=torch.int64, device="cuda")
+    prev_pos = torch.empty(n, dtype=torch.int64, device="cuda")
+    prev_slab[before["id"]] = slab_of(before["counts"])
+    prev_pos[before["id"]] = torch.arange(n, device="cuda")
+    dev.step_fused(cfg["dt"])
+    e, n_tot, n_mig = dev.get_status()
+    assert e == 0 and n_tot == n and 0.03 * n < n_mig < 0.07 * n
+    after = dev.get_particles(n)
+    # conservation of count and of the id multiset
+    assert int(after["counts"].sum()) == n
+    assert torch.equal(torch.sort(after["id"]).values, torch.arange(n, device="cuda"))
+    # containment: every particle sits in the slab of the subdomain that contains its position
+    inv_dx = N / L
+    cell = lambda a: torch.clamp(torch.floor(a * inv_dx).to(torch.int64), 0, N - 1)
+    owner = (cell(after["x"]) // (N // P[0]) + P[0] * (cell(after["y"]) // (N // P[1])
+             + P[1] * (cell(after["z"]) // (N // P[2]))))
+    cur_slab = slab_of(after["counts"])
+    assert torch.equal(owner, cur_slab)
+    # order: stayers first in original order, then incoming by (source slab, source slot)
+    ps, pp = prev_slab[after["id"]], prev_pos[after["id"]]
+    stay = ps == cur_slab
+    assert int(stay.sum()) == n - n_mig
+    key = torch.where(stay, torch.full_like(ps, -1), ps) * (2 * n) + pp      # (is_migrant, source, source slot)
+    same = cur_slab[1:] == cur_slab[:-1]
+    assert bool(torch.all(key[1:][same] > key[:-1][same]))
+    # a sample recomputed one by one by the oracle (push only: positions, velocities)
+    rng = np.random.default_rng(11)
+    pick = torch.from_numpy(np.sort(rng.choice(n, 4096, replace=False))).cuda()
+    sample = {k: parts[k][pick].cpu().numpy() for k in F8}
+    o = oracle_lib.Oracle(N, *P, 4096, g=cfg["g"])
+    o.set_fluid(*(wl[k].cpu().numpy() for k in "uvw"))
+    assert o.set_particles(*(sample[k] for k in F8)) == 0
+    assert o.push(cfg["dt"]) == 0
+    want = o.get_particles()
+    where = torch.empty(n, dtype=torch.int64, device="cuda")
+    where[after["id"]] = torch.arange(n, device="cuda")
+    idx = where[torch.from_numpy(want["id"]).cuda()]
+    got = {k: after[k][idx].cpu().numpy() for k in F7}
+    assert_state_close(got, {k: want[k] for k in F7}, "Large sample")
+    o.close(); dev.close()
