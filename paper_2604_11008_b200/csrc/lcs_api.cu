@@ -52,11 +52,13 @@ bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* pr
 {
     if (!prm) return false;
     if (N < 2 || N > 1625 || Px < 1 || Py < 1 || Pz < 1) return false;
+    if (Px > 1024 || Py > 1024 || Pz > 1024) return false;   // packed subdomain coordinates (10 bits each)
     if (N % Px || N % Py || N % Pz) return false;
     const int64_t P = (int64_t)Px * Py * Pz;
     if (P > 8192) return false;                          // grid.y and shared-histogram limits
     if (cap < 2 || (cap & 1)) return false;               // even: slab bases stay 16-byte aligned
     if (cap > 0x7fffffff) return false;
+    if ((unsigned long long)P * (unsigned long long)cap >= (1ull << 32)) return false;   // 32-bit slot indices
     if (prm->send_capacity < 0 || (prm->send_capacity & 1) || prm->send_capacity > cap) return false;
     if (!(prm->nu > 0.0) || !(prm->rho_ratio > 0.0)) return false;
     if (!std::isfinite(prm->g[0]) || !std::isfinite(prm->g[1]) || !std::isfinite(prm->g[2])) return false;
@@ -101,7 +103,7 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
 
 inline size_t tile_pass_smem(int P)
 {
-    return 2 * kWarps * sizeof(WarpStage) + (P <= kTileStartSmemMax ? (size_t)(P + 1) * sizeof(uint32_t) : 0);
+    return 2 * kWarps * sizeof(WarpStage) + (P <= kTableSmemMax ? (size_t)(2 * P + 1) * sizeof(uint32_t) : 0);
 }
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -174,6 +176,8 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     G.K_tau = prm->rho_ratio / (18.0 * prm->nu);  // tau_p = K_tau * d^2
     G.L_below = std::nextafter(G.L, 0.0);
     G.gx = prm->g[0]; G.gy = prm->g[1]; G.gz = prm->g[2];
+    G.inv_brick_w = 1.0f / (float)(G.ny + 2);
+    G.brick_lines = ((G.nz + 2) * 32 + 96 + 127) / 128;
     char* w = static_cast<char*>(d_workspace);
     const size_t P = (size_t)G.P;
     for (int a = 0; a < 7; ++a) h->S.f[a] = reinterpret_cast<double*>(w + L.slab_f[a]);

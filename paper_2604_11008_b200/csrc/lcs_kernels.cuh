@@ -27,13 +27,15 @@ constexpr int kWarps = kBlock / 32;
 #ifndef LCS_ROWS
 #define LCS_ROWS 3
 #endif
+#ifndef LCS_BRICK_LEAD
+#define LCS_BRICK_LEAD 2
+#endif
 constexpr int kRows = LCS_ROWS;              // rows (particles per lane) of a warp tile
 constexpr int kTile = 32 * kRows;            // particles per tile
 constexpr int kStay = 13;
 constexpr int kNC = 27;                      // destination codes
 constexpr int kInvalid = 31;                 // code of a lane beyond the slab's count
 constexpr int kGroup = 8;                    // tiles per unpack warp
-constexpr int kTileStartSmemMax = 2048;      // tile_start[] is mirrored in shared memory up to this P
 
 // Look-back descriptor word: [ epoch:30 | valid:2 | value:32 ]
 
@@ -44,6 +46,8 @@ struct Geom {
     int lbgroups_per_sub;              // ceil(tiles_per_sub / 32): look-back groups
     int64_t cap, send_cap;
     double inv_dx, K_tau, L, L_below, gx, gy, gz;
+    float inv_brick_w;                 // 1 / (ny + 2), for the brick prefetch shares
+    int brick_lines;                   // 128-byte lines of one z-run of a fluid brick (nz + 2 records)
 };
 
 struct Slabs {                         // SoA particle storage, P*cap slots each
@@ -185,8 +189,11 @@ __device__ __forceinline__ Vec3 side_partial(const double* __restrict__ F4, cons
 }
 
 // Fluid velocity at (x,y,z) of THIS lane's particle; must be called by all 32 lanes (converged).
+// Particle A is the even lane's, particle B the odd lane's.  Both lanes of a pair read A's stencil in
+// the first four loads (even lane: z0 side, odd lane: z1 side) and B's in the next four; the routing
+// is done by the source lane of the index shuffles, so no lane-parity selects are needed.
 __device__ __forceinline__ Vec3 gather_pair(const double* __restrict__ F4, int N, double inv_dx, double x, double y,
-                                            double z, bool odd)
+                                            double z, int lane)
 {
     int i0, i1, j0, j1, k0, k1;
     double fx, fy, fz;
@@ -194,32 +201,34 @@ __device__ __forceinline__ Vec3 gather_pair(const double* __restrict__ F4, int N
     axis_stencil(y, inv_dx, N, j0, j1, fy);
     axis_stencil(z, inv_dx, N, k0, k1, fz);
     const uint32_t Nu = (uint32_t)N;
-    const uint32_t row[4] = {Nu * ((uint32_t)j0 + Nu * (uint32_t)i0), Nu * ((uint32_t)j0 + Nu * (uint32_t)i1),
-                             Nu * ((uint32_t)j1 + Nu * (uint32_t)i0), Nu * ((uint32_t)j1 + Nu * (uint32_t)i1)};
-    // this lane always fetches z-side `odd` (0: k0, 1: k1) -- of its own particle and of its partner's
-    const uint32_t k_mine = odd ? (uint32_t)k1 : (uint32_t)k0;
-    const uint32_t k_other = odd ? (uint32_t)k0 : (uint32_t)k1;       // the side my partner fetches for me
-    uint32_t mine[4], theirs[4];
-#pragma unroll
-    for (int m = 0; m < 4; ++m) {
-        mine[m] = row[m] + k_mine;
-        theirs[m] = __shfl_xor_sync(0xffffffffu, row[m] + k_other, 1);
-    }
-    const double pfx = __shfl_xor_sync(0xffffffffu, fx, 1), pfy = __shfl_xor_sync(0xffffffffu, fy, 1);
-    // load set A = the even lane's particle, set B = the odd lane's particle
+    const uint32_t a0 = Nu * (uint32_t)i0, a1 = Nu * (uint32_t)i1;
+    const uint32_t row[4] = {Nu * (a0 + (uint32_t)j0), Nu * (a1 + (uint32_t)j0), Nu * (a0 + (uint32_t)j1),
+                             Nu * (a1 + (uint32_t)j1)};
+    const uint32_t kk = (uint32_t)k0 | ((uint32_t)k1 << 16);          // N <= 1625 fits 16 bits
+    const int le = lane & ~1, lo = lane | 1;
+    const uint32_t sh = (uint32_t)(lane & 1) << 4;                    // this lane always fetches z-side (lane & 1)
+    const uint32_t kA = (__shfl_sync(0xffffffffu, kk, le) >> sh) & 0xffffu;
+    const uint32_t kB = (__shfl_sync(0xffffffffu, kk, lo) >> sh) & 0xffffu;
     uint32_t ia[4], ib[4];
 #pragma unroll
-    for (int m = 0; m < 4; ++m) { ia[m] = odd ? theirs[m] : mine[m]; ib[m] = odd ? mine[m] : theirs[m]; }
-    const Vec3 pa = side_partial(F4, ia, odd ? pfx : fx, odd ? pfy : fy);
-    const Vec3 pb = side_partial(F4, ib, odd ? fx : pfx, odd ? fy : pfy);
-    // even lane needs A's z1 side (odd's pa); odd lane needs B's z0 side (even's pb)
-    Vec3 give;
+    for (int m = 0; m < 4; ++m) {
+        ia[m] = __shfl_sync(0xffffffffu, row[m], le) + kA;
+        ib[m] = __shfl_sync(0xffffffffu, row[m], lo) + kB;
+    }
+    const double fxA = __shfl_sync(0xffffffffu, fx, le), fyA = __shfl_sync(0xffffffffu, fy, le);
+    const double fxB = __shfl_sync(0xffffffffu, fx, lo), fyB = __shfl_sync(0xffffffffu, fy, lo);
+    const Vec3 pa = side_partial(F4, ia, fxA, fyA);
+    const Vec3 pb = side_partial(F4, ib, fxB, fyB);
+    // the even lane needs A's z1 side (the odd lane's pa); the odd lane needs B's z0 side (the even lane's pb)
+    const bool odd = lane & 1;
+    Vec3 give, keep;
     give.x = odd ? pa.x : pb.x; give.y = odd ? pa.y : pb.y; give.z = odd ? pa.z : pb.z;
+    keep.x = odd ? pb.x : pa.x; keep.y = odd ? pb.y : pa.y; keep.z = odd ? pb.z : pa.z;
     const Vec3 got = shfl_xor1(give);
     Vec3 U;
-    U.x = lerp(odd ? got.x : pa.x, odd ? pb.x : got.x, fz);
-    U.y = lerp(odd ? got.y : pa.y, odd ? pb.y : got.y, fz);
-    U.z = lerp(odd ? got.z : pa.z, odd ? pb.z : got.z, fz);
+    U.x = lerp(odd ? got.x : keep.x, odd ? keep.x : got.x, fz);
+    U.y = lerp(odd ? got.y : keep.y, odd ? keep.y : got.y, fz);
+    U.z = lerp(odd ? got.z : keep.z, odd ? keep.z : got.z, fz);
     return U;
 }
 
@@ -228,56 +237,57 @@ __device__ __forceinline__ Vec3 gather_pair(const double* __restrict__ F4, int N
 // ---------------------------------------------------------------------------------------------
 struct Particle { double x, y, z, vx, vy, vz, d; };
 
-struct SubBox { int lox, hix, loy, hiy, loz, hiz; };   // subdomain bounds in unwrapped cell index space
+struct SubBox { int lox, loy, loz; };   // low corner of the subdomain in cell index space
 
-// One axis: returns d in {-1,0,+1}; sets jump on violation.
-__device__ __forceinline__ int advance_axis(double& a, double& v, double U, double g, double tau, double alpha,
-                                            double b, double dt, const Geom& G, int lo, int hi, int n_a, bool& jump)
+// One axis: advances a and v, adds d*w (d in {-1,0,+1}) to `code`; sets jump on violation.
+__device__ __forceinline__ void advance_axis(double& a, double& v, double U, double g, double tau, double alpha,
+                                             double b, double dt, const Geom& G, int lo, int n_a, int w, int& code,
+                                             bool& jump)
 {
     const double vt = fma(tau, g, U);             // terminal velocity under frozen U
-    const double w = v - vt;
-    v = fma(w, alpha, vt);
-    const double disp = fma(w, b, dt * vt);
+    const double ww = v - vt;
+    v = fma(ww, alpha, vt);
+    const double disp = fma(ww, b, dt * vt);
     double xu = a + disp;
-    int wrap = 0;
-    if (xu < 0.0) { xu = xu + G.L; wrap = -1; if (xu >= G.L) xu = G.L_below; }
-    else if (xu >= G.L) { xu = xu - G.L; wrap = 1; }
+    int wrapN = 0;
+    if (xu < 0.0) { xu = xu + G.L; wrapN = -G.N; if (xu >= G.L) xu = G.L_below; }
+    else if (xu >= G.L) { xu = xu - G.L; wrapN = G.N; }
     a = xu;
-    if (!(xu >= 0.0 && xu < G.L)) { jump = true; return 0; }
+    const bool ok = xu >= 0.0 && xu < G.L;
     int ic = __double2int_rd(xu * G.inv_dx);
     ic = max(0, min(ic, G.N - 1));
-    const int icu = ic + wrap * G.N;              // unwrapped cell index (DESIGN R-14)
-    const int dd = (icu >= hi) - (icu < lo);
-    if (icu >= hi + n_a || icu < lo - n_a) jump = true;
-    return dd;
+    int rel = ic + wrapN - lo;                    // unwrapped cell index relative to the subdomain (DESIGN R-14)
+    rel = ok ? rel : 0;
+    if (rel >= n_a) code += w;
+    if (rel < 0) code -= w;
+    jump |= !ok || (unsigned)(rel + n_a) >= 3u * (unsigned)n_a;
 }
 
 // a1-a3 for this lane's particle (all 32 lanes must call).  Returns the destination code.
 __device__ __forceinline__ int push_particle(Particle& p, const double* __restrict__ F4, const Geom& G,
-                                             const SubBox& B, double dt, bool odd, bool& jump)
+                                             const SubBox& B, double dt, int lane, bool& jump)
 {
 #ifdef LCS_X_NOGATHER
     Vec3 U; U.x = U.y = U.z = 0.0;
 #else
-    const Vec3 U = gather_pair(F4, G.N, G.inv_dx, p.x, p.y, p.z, odd);
+    const Vec3 U = gather_pair(F4, G.N, G.inv_dx, p.x, p.y, p.z, lane);
 #endif
     const double tau = (G.K_tau * p.d) * p.d;     // tau_p = (rho_p/rho) d^2 / (18 nu)
     const double zz = dt / tau;
     const double alpha = exp_neg(zz);
     const double b = tau * (1.0 - alpha);
-    const int dx = advance_axis(p.x, p.vx, U.x, G.gx, tau, alpha, b, dt, G, B.lox, B.hix, G.nx, jump);
-    const int dy = advance_axis(p.y, p.vy, U.y, G.gy, tau, alpha, b, dt, G, B.loy, B.hiy, G.ny, jump);
-    const int dz = advance_axis(p.z, p.vz, U.z, G.gz, tau, alpha, b, dt, G, B.loz, B.hiz, G.nz, jump);
-    return (dx + 1) + 3 * (dy + 1) + 9 * (dz + 1);
+    int code = kStay;
+    advance_axis(p.x, p.vx, U.x, G.gx, tau, alpha, b, dt, G, B.lox, G.nx, 1, code, jump);
+    advance_axis(p.y, p.vy, U.y, G.gy, tau, alpha, b, dt, G, B.loy, G.ny, 3, code, jump);
+    advance_axis(p.z, p.vz, U.z, G.gz, tau, alpha, b, dt, G, B.loz, G.nz, 9, code, jump);
+    return code;
 }
 
 __device__ __forceinline__ SubBox sub_box(const Geom& G, int s)
 {
     const int px = s % G.Px, py = (s / G.Px) % G.Py, pz = s / (G.Px * G.Py);
     SubBox B;
-    B.lox = px * G.nx; B.hix = B.lox + G.nx;
-    B.loy = py * G.ny; B.hiy = B.loy + G.ny;
-    B.loz = pz * G.nz; B.hiz = B.loz + G.nz;
+    B.lox = px * G.nx; B.loy = py * G.ny; B.loz = pz * G.nz;
     return B;
 }
 
@@ -362,7 +372,6 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
     const int64_t first = (int64_t)t * kTile;
     if (first >= (int64_t)cnt_s) return;
     const SubBox B = sub_box(G, s);
-    const bool odd = lane & 1;
     uint32_t cnt_c = 0;
     bool jump = false;
 #pragma unroll 1
@@ -379,7 +388,7 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
             p.d = __longlong_as_double(ld_stream(S.f[6] + at));
         }
         bool jmp = false;
-        int code = push_particle(p, F4, G, B, dt, odd, jmp);
+        int code = push_particle(p, F4, G, B, dt, lane, jmp);
         if (valid) {
             jump |= jmp;
             st_stream(S.f[0] + at, __double_as_longlong(p.x)); st_stream(S.f[1] + at, __double_as_longlong(p.y));
@@ -397,46 +406,64 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
 // K2: tile pass of the migration (a5-a7), optionally with the push fused in front (a1-a4).
 //   Persistent grid; every WARP takes tiles from an atomic ticket (so every predecessor of a tile
 //   belongs to a resident warp) and maps the ticket to (subdomain, tile) through the compact prefix
-//   tile_start[] (empty tiles never get a ticket).  The next ticket is prefetched while the current
-//   tile is processed.  Per tile:
+//   tile_start[] (empty tiles never get a ticket).  Per tile:
 //   - rows of 32 particles: load (64-bit, coalesced), push (fused), stable per-code rank
 //     (row_rank), stage into the warp's private shared-memory area: stayers from the front in
 //     output order, migrants from the back in arrival order with (code, rank-in-code) beside them;
 //   - publish the tile aggregate (stayers, migrants) and the per-code byte counts;
-//   - single-pass look-back over the tiles of the SAME subdomain: two levels of aggregates (tiles of
-//     the own group of 32, then whole groups), two running sums, one lane per predecessor;
+//   - take the next ticket, prefetch its particle lines into L2;
+//   - resolve the PREVIOUS tile (depth-2 pipeline): two levels of aggregates (tiles of the own group
+//     of 32, then whole groups), one lane per predecessor, no prefix chain;
 //   - stayers written in place at their compacted slot (coalesced), migrants to the subdomain's
 //     send region at (migrant prefix) + (start of their code's run in the tile chunk) + (rank).
 //   A tile publishes only after every one of its loads has completed (the staging stores consume
 //   the loaded registers and precede the publish in program order), which makes the in-place left
 //   compaction safe: a tile writes only slots below its own end, all of which belong to tiles
-//   that have published (DESIGN.md 6.3).
+//   that have published (DESIGN.md 6.2).
+//   Instruction diet (the kernel is issue/latency bound, not DRAM bound): all per-tile integer
+//   divisions are replaced by tables built once per CTA in shared memory (subdomain coordinates)
+//   or by float reciprocals (prefetch shares, where an approximate answer is good enough); the
+//   ticket -> (s,t) map is an incremental search from the previous subdomain; particle slots are
+//   32-bit indices (P*cap < 2^32 is checked at lcs_create).
 // ---------------------------------------------------------------------------------------------
+constexpr int kBrickLead = LCS_BRICK_LEAD;   // the tiles of subdomain s prefetch the fluid brick of s + kBrickLead
+
 // ---------------------------------------------------------------------------------------------
-// Fluid brick prefetch.  The tiles of subdomain s are processed in ticket order, so the 8.8 MB brick
-// of fluid records that subdomain s+1 will gather from can be pulled into L2 ahead of time with
-// full-line prefetches, one share per tile of s, instead of being demand-missed one 32-byte sector
-// at a time by the first particle that touches each cell.  Runs along z are contiguous in the
-// internal layout; the two seam planes in z are left to demand misses.
+// Fluid brick prefetch.  Tiles are processed in ticket order, so the fluid records a later subdomain
+// will gather from can be pulled into L2 ahead of time with full-line prefetches, one share per
+// tile, instead of being demand-missed one 32-byte sector at a time by the first particle that
+// touches each cell.  Runs along z are contiguous in the internal layout (lane = 128-byte line of a
+// column); the two seam planes in z are left to demand misses.  Purely a hint: shares are computed
+// with float reciprocals and clamped, coverage may overlap by a column.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void prefetch_brick_share(const double* __restrict__ F4, const Geom& G, int q, uint32_t share,
-                                                     uint32_t nshares, int lane)
+__device__ __forceinline__ void prefetch_brick_share(const double* __restrict__ F4, const Geom& G, uint32_t qxyz,
+                                                     uint32_t share, uint32_t nshares, int lane)
 {
-    const int qx = q % G.Px, qy = (q / G.Px) % G.Py, qz = q / (G.Px * G.Py);
-    const int ka = max(0, qz * G.nz - 1), kb = min(G.N - 1, qz * G.nz + G.nz);        // inclusive
-    const uint32_t nrun = (uint32_t)(G.nx + 2) * (uint32_t)(G.ny + 2);                 // (i,j) columns of the brick
-    const uint32_t per = (nrun + nshares - 1) / nshares;                               // columns per share
-    const uint32_t r0 = share * per, r1 = min(nrun, r0 + min(per, 8u));                // at most 8 columns per tile
-    for (uint32_t rj = r0; rj < r1; ++rj) {                                            // warp-uniform
-        const int ii = (int)(rj / (uint32_t)(G.ny + 2)), jj = (int)(rj % (uint32_t)(G.ny + 2));
-        int i = qx * G.nx - 1 + ii, j = qy * G.ny - 1 + jj;
+    const int qx = (int)(qxyz & 1023u), qy = (int)((qxyz >> 10) & 1023u), qz = (int)(qxyz >> 20);
+    const int ka = max(0, qz * G.nz - 1);
+    const uint32_t w = (uint32_t)(G.ny + 2);
+    const uint32_t nrun = (uint32_t)(G.nx + 2) * w;                                   // (i,j) columns of the brick
+    uint32_t per = (uint32_t)__fdividef((float)(nrun + nshares), (float)nshares);     // ~ceil(nrun / nshares)
+    per = min(per, 8u);
+    const uint32_t r0 = share * per;
+    if (r0 >= nrun) return;
+    const uint32_t r1 = min(nrun, r0 + per);
+    uint32_t ii = (uint32_t)((float)r0 * G.inv_brick_w);
+    ii = min(ii, (uint32_t)(G.nx + 1));
+    if (ii * w > r0) --ii;
+    uint32_t jj = r0 - ii * w;
+    if (jj >= w) { jj -= w; ++ii; }
+    const uint32_t z0 = (uint32_t)ka * 32u & ~127u;                                    // byte offset inside a column
+    const uint32_t zend = min((uint32_t)G.N * 32u, z0 + (uint32_t)G.brick_lines * 128u);
+    for (uint32_t rj = r0; rj < r1; ++rj) {                                            // warp-uniform, <= 8 trips
+        int i = qx * G.nx - 1 + (int)ii, j = qy * G.ny - 1 + (int)jj;
         i = i < 0 ? i + G.N : (i >= G.N ? i - G.N : i);
         j = j < 0 ? j + G.N : (j >= G.N ? j - G.N : j);
-        const size_t col = ((size_t)i * G.N + j) * G.N;
-        const uintptr_t a0 = reinterpret_cast<uintptr_t>(F4 + 4 * (col + ka)) & ~(uintptr_t)127;
-        const uintptr_t a1 = reinterpret_cast<uintptr_t>(F4 + 4 * (col + kb + 1));
-        for (uintptr_t a = a0 + (uintptr_t)lane * 128; a < a1; a += 32 * 128)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+        const uint32_t col = ((uint32_t)i * (uint32_t)G.N + (uint32_t)j) * (uint32_t)G.N;   // record index of (i,j,0)
+        const char* a = reinterpret_cast<const char*>(F4) + (size_t)col * 32u;
+        for (uint32_t zo = z0 + (uint32_t)lane * 128u; zo < zend; zo += 32u * 128u)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a + zo));
+        if (++jj == w) { jj = 0; ++ii; }
     }
 }
 
@@ -476,8 +503,16 @@ __device__ __forceinline__ void sum_descs(const uint64_t* base, int n, int lane,
         if (__all_sync(0xffffffffu, ready)) break;
         __nanosleep(200);
     }
-    stay += warp_sum(need ? (uint32_t)w.x : 0u);
-    mig += warp_sum(need ? (uint32_t)w.y : 0u);
+    stay += __reduce_add_sync(0xffffffffu, need ? (uint32_t)w.x : 0u);
+    mig += __reduce_add_sync(0xffffffffu, need ? (uint32_t)w.y : 0u);
+}
+
+constexpr int kTableSmemMax = 1024;     // tile_start[] and the subdomain coordinates are mirrored in shared memory up to this P
+
+__device__ __forceinline__ uint32_t pack_xyz(const Geom& G, int s)
+{   // px | py << 10 | pz << 20 (each < 1024, checked at lcs_create)
+    const int px = s % G.Px, py = (s / G.Px) % G.Py, pz = s / (G.Px * G.Py);
+    return (uint32_t)px | ((uint32_t)py << 10) | ((uint32_t)pz << 20);
 }
 
 template <bool kFused>
@@ -485,23 +520,48 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks)
 k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
-    WarpStage* stage_all = reinterpret_cast<WarpStage*>(s_raw);                                     // [kWarps][2]
-    uint32_t* s_tile_start = reinterpret_cast<uint32_t*>(s_raw + 2 * kWarps * sizeof(WarpStage));   // [P+1] if it fits
-    const bool ts_smem = G.P <= kTileStartSmemMax;
-    if (ts_smem) {
-        for (int i = threadIdx.x; i <= G.P; i += kBlock) s_tile_start[i] = T.tile_start[i];
+    WarpStage* stage_all = reinterpret_cast<WarpStage*>(s_raw);                            // [kWarps][2]
+    uint32_t* s_ts = reinterpret_cast<uint32_t*>(s_raw + 2 * kWarps * sizeof(WarpStage));  // [P+1] if it fits
+    uint32_t* s_xyz = s_ts + (G.P + 1);                                                    // [P]   if it fits
+    const bool big = G.P > kTableSmemMax;
+    if (!big) {
+        for (int i = threadIdx.x; i <= G.P; i += kBlock) {
+            s_ts[i] = T.tile_start[i];
+            if (i < G.P) s_xyz[i] = pack_xyz(G, i);
+        }
         __syncthreads();                                   // the only block barrier of the kernel
     }
-    const uint32_t* __restrict__ tstart = ts_smem ? s_tile_start : T.tile_start;
+    auto ts = [&](int i) -> uint32_t { return big ? __ldg(T.tile_start + i) : s_ts[i]; };
+    auto xyz = [&](int s) -> uint32_t { return big ? pack_xyz(G, s) : s_xyz[s]; };
+    // ticket -> subdomain: the tickets of a warp increase, so search forward from its previous subdomain
+    auto locate = [&](unsigned int g, int s_from) -> int {
+        int s = s_from;
+#pragma unroll 1
+        for (int k = 0; k < 4; ++k) {
+            if (g < ts(s + 1)) return s;
+            ++s;
+        }
+        int lo = s, hi = G.P;                                 // largest s with tile_start[s] <= g
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (ts(mid) <= g) lo = mid; else hi = mid; }
+        return lo;
+    };
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const bool odd = lane & 1;
     const unsigned lt = (1u << lane) - 1u;
-    const unsigned int n_active = tstart[G.P];
+    const unsigned int n_active = ts(G.P);
     const uint64_t tag = ((uint64_t)(epoch << 2) << 32) | (1ull << 32);
+    const uint32_t cap32 = (uint32_t)G.cap;
+    const unsigned long long* const fS[8] = {
+        reinterpret_cast<const unsigned long long*>(S.f[0]), reinterpret_cast<const unsigned long long*>(S.f[1]),
+        reinterpret_cast<const unsigned long long*>(S.f[2]), reinterpret_cast<const unsigned long long*>(S.f[3]),
+        reinterpret_cast<const unsigned long long*>(S.f[4]), reinterpret_cast<const unsigned long long*>(S.f[5]),
+        reinterpret_cast<const unsigned long long*>(S.f[6]), reinterpret_cast<const unsigned long long*>(S.id)};
 
     unsigned int g = 0;
     if (lane == 0) g = atomicAdd(T.ticket, 1u);
     g = __shfl_sync(0xffffffffu, g, 0);
+    int s_cur = 0;
+    uint32_t cnt_cur = 0;
+    if (g < n_active) { s_cur = locate(g, 0); cnt_cur = __ldg(T.count + s_cur); }
     TileInfo pend;
     pend.s = pend.t = 0; pend.n_stay = pend.n_mig = pend.run_start = 0;
     bool have_pend = false;
@@ -514,42 +574,43 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
         // ================= push of tile g: load, (push,) rank, stage, publish the aggregate =================
         if (have) {
             WarpStage& W = stage_all[2 * warp + buf];
-            int lo = 0, hi = G.P;                                       // largest s with tile_start[s] <= g
-            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (tstart[mid] <= g) lo = mid; else hi = mid; }
-            const int s = lo;
-            const int t = (int)(g - tstart[lo]);
-            const uint32_t cnt_s = __ldg(T.count + s);
-            const int64_t first = (int64_t)t * kTile;
-            const size_t slab0 = (size_t)s * (size_t)G.cap;
+            const int s = s_cur;
+            const uint32_t ts_s = ts(s);
+            const int t = (int)(g - ts_s);
+            const uint32_t cnt_s = cnt_cur;
+            const uint32_t first = (uint32_t)t * kTile;
+            const uint32_t slab0 = (uint32_t)s * cap32;
             SubBox B;
+            B.lox = B.loy = B.loz = 0;
             if (kFused) {
-                B = sub_box(G, s);
-                if (s + 1 < G.P) prefetch_brick_share(F4, G, s + 1, (uint32_t)t, (cnt_s + kTile - 1) / kTile, lane);
+                const uint32_t c3 = xyz(s);
+                B.lox = (int)(c3 & 1023u) * G.nx; B.loy = (int)((c3 >> 10) & 1023u) * G.ny; B.loz = (int)(c3 >> 20) * G.nz;
+                if (s + kBrickLead < G.P)
+                    prefetch_brick_share(F4, G, xyz(s + kBrickLead), (uint32_t)t, ts(s + 1) - ts_s, lane);
             }
             uint32_t cnt_c = 0;            // lane c: particles of the tile so far with code c
             uint32_t n_mig = 0;            // migrants of the tile so far (warp-uniform)
             bool jump = false;
 #pragma unroll 1
             for (int r = 0; r < kRows; ++r) {
-                if (first + 32 * r >= (int64_t)cnt_s) break;
-                const int64_t slot = first + 32 * r + lane;
-                const bool valid = slot < (int64_t)cnt_s;
-                const size_t at = slab0 + (size_t)slot;
-                Particle p{0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0};
-                unsigned long long id = 0;
-                int code = kStay;
-                if (valid) {
-                    p.x = __longlong_as_double(ld_stream(S.f[0] + at)); p.y = __longlong_as_double(ld_stream(S.f[1] + at));
-                    p.z = __longlong_as_double(ld_stream(S.f[2] + at)); p.vx = __longlong_as_double(ld_stream(S.f[3] + at));
-                    p.vy = __longlong_as_double(ld_stream(S.f[4] + at)); p.vz = __longlong_as_double(ld_stream(S.f[5] + at));
-                    p.d = __longlong_as_double(ld_stream(S.f[6] + at));
-                    id = ld_stream(S.id + at);
-                    if (!kFused) code = min((int)S.code[at], 26);
-                }
+                const uint32_t row0 = first + 32u * (uint32_t)r;
+                if (row0 >= cnt_s) break;
+                const uint32_t slot = row0 + (uint32_t)lane;
+                const bool valid = slot < cnt_s;
+                const uint32_t at = slab0 + min(slot, cnt_s - 1u);     // lanes past the end re-read the last particle
+                Particle p;
+                p.x = __longlong_as_double(ld_stream(fS[0] + at)); p.y = __longlong_as_double(ld_stream(fS[1] + at));
+                p.z = __longlong_as_double(ld_stream(fS[2] + at)); p.vx = __longlong_as_double(ld_stream(fS[3] + at));
+                p.vy = __longlong_as_double(ld_stream(fS[4] + at)); p.vz = __longlong_as_double(ld_stream(fS[5] + at));
+                p.d = __longlong_as_double(ld_stream(fS[6] + at));
+                const unsigned long long id = ld_stream(fS[7] + at);
+                int code;
                 if (kFused) {
                     bool jmp = false;
-                    code = push_particle(p, F4, G, B, dt, odd, jmp);
+                    code = push_particle(p, F4, G, B, dt, lane, jmp);
                     jump |= jmp && valid;
+                } else {
+                    code = min((int)S.code[at], 26);
                 }
                 if (!valid) code = kInvalid;
                 const uint32_t rank = row_rank(code, valid, lane, cnt_c);
@@ -588,31 +649,32 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             cur.s = s; cur.t = t; cur.n_stay = n_stay; cur.n_mig = n_mig; cur.run_start = inc - magg;
         }
 
+        // ================= next ticket =================
+        // Taken right after this tile's aggregate is out (a ticket held across a wait is a convoy);
+        // its subdomain's count and its particle lines (8 fields x 8 lines, two prefetches per lane) are requested now
+        // and consumed one iteration later.
+        unsigned int g_next = 0xffffffffu;
+        if (have) {
+            if (lane == 0) g_next = atomicAdd(T.ticket, 1u);
+            g_next = __shfl_sync(0xffffffffu, g_next, 0);
+            if (g_next < n_active) {
+                s_cur = locate(g_next, s_cur);
+                cnt_cur = __ldg(T.count + s_cur);
+                const uint32_t pat = (uint32_t)s_cur * cap32 + (g_next - ts(s_cur)) * kTile;
+                const size_t fstride = reinterpret_cast<const char*>(fS[1]) - reinterpret_cast<const char*>(fS[0]);
+                const char* pf = reinterpret_cast<const char*>(fS[0]) + (size_t)pat * 8u + (size_t)(lane & 7) * 128u
+                                 + (size_t)(lane >> 3) * fstride;
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(pf));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(pf + 4 * fstride));
+            }
+        }
+
         // ================= resolve of the previous tile: look-back, then copy-out =================
         // Two-level aggregate look-back (no prefix chain): exclusive prefix of tile t = aggregates of the
         // earlier tiles of its group of 32 + accumulators of the earlier groups (every tile adds its
         // aggregate to its group's accumulator with one 64-bit atomic right after its push).  Every word
         // waited for is produced by the PUSH of a tile with a smaller ticket -- never by another tile's
         // resolve -- and this warp has pushed a whole tile in between.
-        // Next ticket: taken right after this tile's aggregate is out; its tile's particle lines are
-        // prefetched into L2 while the previous tile is resolved.
-        unsigned int g_next = 0xffffffffu;
-        if (have) {
-            if (lane == 0) g_next = atomicAdd(T.ticket, 1u);
-            g_next = __shfl_sync(0xffffffffu, g_next, 0);
-            if (g_next < n_active) {
-                int plo = cur.s, phi = G.P;
-                while (phi - plo > 1) { const int mid = (plo + phi) >> 1; if (tstart[mid] <= g_next) plo = mid; else phi = mid; }
-                const size_t pat = (size_t)plo * (size_t)G.cap + (size_t)(g_next - tstart[plo]) * kTile;
-                const char* base[8] = {reinterpret_cast<const char*>(S.f[0]), reinterpret_cast<const char*>(S.f[1]),
-                                       reinterpret_cast<const char*>(S.f[2]), reinterpret_cast<const char*>(S.f[3]),
-                                       reinterpret_cast<const char*>(S.f[4]), reinterpret_cast<const char*>(S.f[5]),
-                                       reinterpret_cast<const char*>(S.f[6]), reinterpret_cast<const char*>(S.id)};
-#pragma unroll
-                for (int fld = 0; fld < 8; ++fld)
-                    if (lane < 2 * kRows) asm volatile("prefetch.global.L2 [%0];" ::"l"(base[fld] + pat * 8 + (size_t)lane * 128));
-            }
-        }
         if (have_pend) {
             const WarpStage& W = stage_all[2 * warp + (buf ^ 1)];
             const int s = pend.s, t = pend.t;
@@ -630,33 +692,36 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     if (__all_sync(0xffffffffu, ready)) break;
                     __nanosleep(200);
                 }
-                excl_stay += warp_sum(need ? (uint32_t)(w & 0xfffffull) : 0u);
-                excl_mig += warp_sum(need ? (uint32_t)((w >> 20) & 0xfffffull) : 0u);
+                excl_stay += __reduce_add_sync(0xffffffffu, need ? (uint32_t)(w & 0xfffffull) : 0u);
+                excl_mig += __reduce_add_sync(0xffffffffu, need ? (uint32_t)((w >> 20) & 0xfffffull) : 0u);
             }
-            long long sendbase = (long long)s * G.send_cap + (long long)excl_mig;
-            if ((long long)excl_mig + (long long)pend.n_mig > G.send_cap) { if (lane == 0) raise(T.status, -4); sendbase = -1; }
             // copy-out: stayers in place (compacted, coalesced), migrants to the send region
-            const size_t stay_base = (size_t)s * (size_t)G.cap + (size_t)excl_stay;
+            const uint32_t stay_base = (uint32_t)s * cap32 + excl_stay;
 #ifdef LCS_X_NOSTORE
             if (excl_stay == 0xffffffffu)
 #endif
             for (uint32_t j = lane; j < pend.n_stay; j += 32) {
-                const size_t dst = stay_base + j;
+                const uint32_t dst = stay_base + j;
 #pragma unroll
                 for (int a = 0; a < 7; ++a) st_stream(S.f[a] + dst, W.f[a][j]);
                 st_stream(S.id + dst, W.f[7][j]);
             }
-            for (uint32_t a0 = 0; a0 < pend.n_mig; a0 += 32) {
-                const uint32_t a = a0 + lane;
-                const bool ok = a < pend.n_mig;
-                const uint32_t mt = ok ? W.meta[a] : 0u;
-                const uint32_t off = __shfl_sync(0xffffffffu, pend.run_start, mt & 31u) + (mt >> 5);
-                if (ok && sendbase >= 0) {
-                    const size_t dst = (size_t)sendbase + off;
-                    const uint32_t src = kTile - 1 - a;
+            if (pend.n_mig) {
+                bool fits = (long long)excl_mig + (long long)pend.n_mig <= G.send_cap;
+                if (!fits && lane == 0) raise(T.status, -4);
+                const size_t sendbase = (size_t)s * (size_t)G.send_cap + excl_mig;
+                for (uint32_t a0 = 0; a0 < pend.n_mig; a0 += 32) {
+                    const uint32_t a = a0 + lane;
+                    const bool ok = a < pend.n_mig;
+                    const uint32_t mt = ok ? W.meta[a] : 0u;
+                    const uint32_t off = __shfl_sync(0xffffffffu, pend.run_start, mt & 31u) + (mt >> 5);
+                    if (ok && fits) {
+                        const size_t dst = sendbase + off;
+                        const uint32_t src = kTile - 1 - a;
 #pragma unroll
-                    for (int q = 0; q < 7; ++q) st_stream(Snd.f[q] + dst, W.f[q][src]);
-                    st_stream(Snd.id + dst, W.f[7][src]);
+                        for (int q = 0; q < 7; ++q) st_stream(Snd.f[q] + dst, W.f[q][src]);
+                        st_stream(Snd.id + dst, W.f[7][src]);
+                    }
                 }
             }
         }
