@@ -182,7 +182,7 @@ def run_cuda(args):
     parts = wl["particles"]
     lcs.set_particles(*(parts[k] for k in F8))
     err, n_tot, _ = lcs.get_status()
-    if err or n_tot != n:
+    if (err or n_tot != n) and not os.environ.get("LCS_BENCH_ABLATION"):   # ablation builds (-DLCS_X_*) compute wrong results on purpose
         print(f"bench.py: set_particles failed: status {err}, total {n_tot}", file=sys.stderr)
         return 3
     dt = cfg["dt"]
@@ -210,7 +210,7 @@ def run_cuda(args):
     launches = lcs.kernel_launches - launches0
     clocks = sampler.stop() if sampler else None
     err, n_tot, n_mig = lcs.get_status()
-    if err or n_tot != n:
+    if (err or n_tot != n) and not os.environ.get("LCS_BENCH_ABLATION"):   # ablation builds (-DLCS_X_*) compute wrong results on purpose
         print(f"bench.py: step failed: sticky status {err}, total {n_tot}", file=sys.stderr)
         return 3
     ms_total = max_over_ranks(ms_total, dist, dev)

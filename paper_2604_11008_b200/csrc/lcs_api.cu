@@ -103,7 +103,7 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
 
 inline size_t tile_pass_smem(int P)
 {
-    return 2 * kWarps * sizeof(WarpStage) + (P <= kTableSmemMax ? (size_t)(2 * P + 1) * sizeof(uint32_t) : 0);
+    return kWarps * kNBuf * (sizeof(TileBuf) + sizeof(uint64_t)) + (P <= kTableSmemMax ? (size_t)(2 * P + 1) * sizeof(uint32_t) : 0);
 }
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }

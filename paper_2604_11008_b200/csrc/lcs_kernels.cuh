@@ -16,16 +16,16 @@
 namespace lcs {
 
 #ifndef LCS_BLOCK
-#define LCS_BLOCK 256
+#define LCS_BLOCK 384
 #endif
 #ifndef LCS_MIN_BLOCKS
-#define LCS_MIN_BLOCKS 2
+#define LCS_MIN_BLOCKS 1
 #endif
 constexpr int kBlock = LCS_BLOCK;            // threads per CTA of the tile pass
 constexpr int kMinBlocks = LCS_MIN_BLOCKS;   // CTAs per SM the tile pass is compiled for
 constexpr int kWarps = kBlock / 32;
 #ifndef LCS_ROWS
-#define LCS_ROWS 3
+#define LCS_ROWS 2
 #endif
 #ifndef LCS_BRICK_LEAD
 #define LCS_BRICK_LEAD 2
@@ -75,7 +75,11 @@ struct Tables {
 // ---------------------------------------------------------------------------------------------
 // small helpers
 // ---------------------------------------------------------------------------------------------
+#ifdef LCS_X_NOSTATUS               // experiment builds only: errors are not recorded
+__device__ __forceinline__ void raise(int*, int) {}
+#else
 __device__ __forceinline__ void raise(int* status, int code) { atomicCAS(status, 0, code); }
+#endif
 
 __device__ __forceinline__ uint64_t ld_relaxed_u64(const void* p)
 {
@@ -151,8 +155,18 @@ struct alignas(32) Cell { double u, v, w, pad; };
 __device__ __forceinline__ Cell ld_cell(const double* __restrict__ F4, uint32_t cell)
 {
     Cell r;
+#ifdef LCS_X_NOGATHER            // experiment: no fluid loads at all
+    r.u = r.v = r.w = r.pad = 0.0;
+    return r;
+#endif
+#ifdef LCS_X_GATHER_SMALL        // experiment: all gathers fall into the first 8 MB of the field
+    cell &= 0x3ffffu;
+#endif
     asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
                  : "=d"(r.u), "=d"(r.v), "=d"(r.w), "=d"(r.pad) : "l"(F4 + 4 * (size_t)cell));
+#ifdef LCS_X_ZEROU                // experiment: loads kept, values zeroed (same dynamics as LCS_X_NOGATHER)
+    r.u *= 0.0; r.v *= 0.0; r.w *= 0.0;
+#endif
     return r;
 }
 
@@ -404,29 +418,76 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
 
 // ---------------------------------------------------------------------------------------------
 // K2: tile pass of the migration (a5-a7), optionally with the push fused in front (a1-a4).
-//   Persistent grid; every WARP takes tiles from an atomic ticket (so every predecessor of a tile
-//   belongs to a resident warp) and maps the ticket to (subdomain, tile) through the compact prefix
-//   tile_start[] (empty tiles never get a ticket).  Per tile:
-//   - rows of 32 particles: load (64-bit, coalesced), push (fused), stable per-code rank
-//     (row_rank), stage into the warp's private shared-memory area: stayers from the front in
-//     output order, migrants from the back in arrival order with (code, rank-in-code) beside them;
-//   - publish the tile aggregate (stayers, migrants) and the per-code byte counts;
-//   - take the next ticket, prefetch its particle lines into L2;
-//   - resolve the PREVIOUS tile (depth-2 pipeline): two levels of aggregates (tiles of the own group
-//     of 32, then whole groups), one lane per predecessor, no prefix chain;
-//   - stayers written in place at their compacted slot (coalesced), migrants to the subdomain's
-//     send region at (migrant prefix) + (start of their code's run in the tile chunk) + (rank).
-//   A tile publishes only after every one of its loads has completed (the staging stores consume
-//   the loaded registers and precede the publish in program order), which makes the in-place left
-//   compaction safe: a tile writes only slots below its own end, all of which belong to tiles
-//   that have published.
-//   Instruction diet (the kernel is issue/latency bound, not DRAM bound): all per-tile integer
-//   divisions are replaced by tables built once per CTA in shared memory (subdomain coordinates)
-//   or by float reciprocals (prefetch shares, where an approximate answer is good enough); the
-//   ticket -> (s,t) map is an incremental search from the previous subdomain; particle slots are
-//   32-bit indices (P*cap < 2^32 is checked at lcs_create).
+//
+//   Persistent grid, one CTA per SM, every WARP autonomous: it takes tiles (kTile consecutive slots
+//   of one slab) from an atomic ticket, so every predecessor of a tile belongs to a resident warp,
+//   and maps the ticket to (subdomain, tile) through the compact prefix tile_start[] (empty tiles
+//   never get a ticket).  The kernel is bound by memory LATENCY (each particle needs a DRAM stream
+//   read, then eight dependent L2 gathers, then ~250 dependent fp64 instructions), not by any
+//   throughput, so everything is arranged to keep one long-latency request per warp in flight at
+//   all times:
+//   - particle data: the 8 field runs of a tile (8 x kTile x 8 B) are brought into one of the warp's
+//     three shared-memory tile buffers by bulk async copies (cp.async.bulk + mbarrier) issued about
+//     one tile ahead; no registers, no L2 prefetch instructions, no exposed DRAM latency;
+//   - gather: software pipeline over ROWS of 32 particles that runs across tile boundaries: the
+//     eight 32-byte corner loads of row r+1 are issued (64 registers in flight) before the
+//     arithmetic of row r (division, exp, advance, classify, rank), and before the publish /
+//     look-back / copy-out at a tile end;
+//   - the push updates x, v in place in the tile buffer; nothing is compacted in shared memory.
+//     Stayers are compacted on the way out (row masks -> consecutive lanes write consecutive slots),
+//     migrants are listed (position, code, rank-in-code) and written to the send region;
+//   - publish the tile aggregate (stayers, migrants) and the per-code byte counts, take the ticket
+//     of the tile after next, then resolve the PREVIOUS tile (depth-2 pipeline): two levels of
+//     aggregates (tiles of the own group of 32, then whole groups), one lane per predecessor, no
+//     prefix chain; the freed buffer receives the bulk copy of the newly ticketed tile.
+//   A tile publishes only after all of its loads have completed (mbarrier wait), which makes the
+//   in-place left compaction safe: a tile writes only slots below its own end, all of which belong
+//   to tiles that have published; and a tile's input range is only ever overwritten by tiles with a
+//   larger ticket, which resolve after it has published -- so loading a tile early is safe too.
+//   All per-tile integer divisions are replaced by tables built once per CTA in shared memory or by
+//   float reciprocals (prefetch shares); the ticket -> (s,t) map is an incremental search from the
+//   previous subdomain; particle slots are 32-bit indices (P*cap < 2^32 is checked at lcs_create).
 // ---------------------------------------------------------------------------------------------
 constexpr int kBrickLead = LCS_BRICK_LEAD;   // the tiles of subdomain s prefetch the fluid brick of s + kBrickLead
+constexpr int kNBuf = 3;                     // tile buffers per warp: loading / being pushed / awaiting resolve
+constexpr int kTableSmemMax = 1024;          // tile_start[] and the subdomain coordinates are mirrored in shared memory up to this P
+
+struct alignas(128) TileBuf {
+    unsigned long long f[8][kTile];     // x y z vx vy vz d id of the tile's slots, raw 64-bit words; x..vz updated in place
+    uint32_t mlist[kTile];              // migrants in arrival order: position | code << 8 | rank-in-code << 16
+    uint32_t stay_m[4];                 // per row: lanes that stay
+};
+
+// ---- mbarrier / bulk-copy primitives (sm_90+; one elected lane issues, all lanes wait) ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile("{\n"
+                 ".reg .pred p;\n"
+                 "LCS_WAIT_%=:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 "@p bra LCS_DONE_%=;\n"
+                 "bra LCS_WAIT_%=;\n"
+                 "LCS_DONE_%=:\n"
+                 "}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async()
+{   // order this thread's generic-proxy shared-memory accesses before later async-proxy (bulk copy) accesses
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
 
 // ---------------------------------------------------------------------------------------------
 // Fluid brick prefetch.  Tiles are processed in ticket order, so the fluid records a later subdomain
@@ -467,10 +528,100 @@ __device__ __forceinline__ void prefetch_brick_share(const double* __restrict__ 
     }
 }
 
-struct WarpStage {
-    unsigned long long f[8][kTile];     // x y z vx vy vz d id as raw 64-bit words, staged order
-    unsigned short meta[kTile];         // migrant a (arrival order): code | rank-in-code << 5
+// ---------------------------------------------------------------------------------------------
+// Split gather: issue (stencil, index exchange, eight loads) and reduce (lerps), so that the loads of
+// the NEXT row are in flight while the current row is advanced.  Same arithmetic, same order as
+// gather_pair (x, then y, then z lerps; rule R3).
+// ---------------------------------------------------------------------------------------------
+struct Gath {
+    Cell a[4], b[4];                    // this lane's z-side of particle A (even lane's) and of particle B (odd lane's)
+    double fxA, fyA, fxB, fyB, fz;      // fractions: A's and B's in x, y; this lane's own in z
 };
+
+__device__ __forceinline__ void gather_issue(Gath& Q, const double* __restrict__ F4, int N, double inv_dx, double x,
+                                             double y, double z, int lane)
+{
+    int i0, i1, j0, j1, k0, k1;
+    double fx, fy;
+    axis_stencil(x, inv_dx, N, i0, i1, fx);
+    axis_stencil(y, inv_dx, N, j0, j1, fy);
+    axis_stencil(z, inv_dx, N, k0, k1, Q.fz);
+    const uint32_t Nu = (uint32_t)N;
+    const uint32_t a0 = Nu * (uint32_t)i0, a1 = Nu * (uint32_t)i1;
+    const uint32_t row[4] = {Nu * (a0 + (uint32_t)j0), Nu * (a1 + (uint32_t)j0), Nu * (a0 + (uint32_t)j1),
+                             Nu * (a1 + (uint32_t)j1)};
+    const uint32_t kk = (uint32_t)k0 | ((uint32_t)k1 << 16);          // N <= 1625 fits 16 bits
+    const int le = lane & ~1, lo = lane | 1;
+    const uint32_t sh = (uint32_t)(lane & 1) << 4;                    // this lane always fetches z-side (lane & 1)
+    const uint32_t kA = (__shfl_sync(0xffffffffu, kk, le) >> sh) & 0xffffu;
+    const uint32_t kB = (__shfl_sync(0xffffffffu, kk, lo) >> sh) & 0xffffu;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) Q.a[m] = ld_cell(F4, __shfl_sync(0xffffffffu, row[m], le) + kA);
+#pragma unroll
+    for (int m = 0; m < 4; ++m) Q.b[m] = ld_cell(F4, __shfl_sync(0xffffffffu, row[m], lo) + kB);
+    Q.fxA = __shfl_sync(0xffffffffu, fx, le); Q.fyA = __shfl_sync(0xffffffffu, fy, le);
+    Q.fxB = __shfl_sync(0xffffffffu, fx, lo); Q.fyB = __shfl_sync(0xffffffffu, fy, lo);
+}
+
+__device__ __forceinline__ Vec3 side_reduce(const Cell c[4], double fx, double fy)
+{   // corners (i0,j0) (i1,j0) (i0,j1) (i1,j1) of one z-side: x lerps, then y
+    Vec3 r;
+    r.x = lerp(lerp(c[0].u, c[1].u, fx), lerp(c[2].u, c[3].u, fx), fy);
+    r.y = lerp(lerp(c[0].v, c[1].v, fx), lerp(c[2].v, c[3].v, fx), fy);
+    r.z = lerp(lerp(c[0].w, c[1].w, fx), lerp(c[2].w, c[3].w, fx), fy);
+    return r;
+}
+
+__device__ __forceinline__ Vec3 gather_reduce(const Gath& Q, int lane)
+{
+    const Vec3 pa = side_reduce(Q.a, Q.fxA, Q.fyA);
+    const Vec3 pb = side_reduce(Q.b, Q.fxB, Q.fyB);
+    // the even lane needs A's z1 side (the odd lane's pa); the odd lane needs B's z0 side (the even lane's pb)
+    const bool odd = lane & 1;
+    Vec3 give, keep;
+    give.x = odd ? pa.x : pb.x; give.y = odd ? pa.y : pb.y; give.z = odd ? pa.z : pb.z;
+    keep.x = odd ? pb.x : pa.x; keep.y = odd ? pb.y : pa.y; keep.z = odd ? pb.z : pa.z;
+    const Vec3 got = shfl_xor1(give);
+    Vec3 U;
+    U.x = lerp(odd ? got.x : keep.x, odd ? keep.x : got.x, Q.fz);
+    U.y = lerp(odd ? got.y : keep.y, odd ? keep.y : got.y, Q.fz);
+    U.z = lerp(odd ? got.z : keep.z, odd ? keep.z : got.z, Q.fz);
+    return U;
+}
+
+// a2-a3 given the gathered fluid velocity U.  Returns the destination code.
+__device__ __forceinline__ int advance_particle(Particle& p, const Vec3& U, const Geom& G, const SubBox& B, double dt,
+                                                bool& jump)
+{
+    const double tau = (G.K_tau * p.d) * p.d;     // tau_p = (rho_p/rho) d^2 / (18 nu)
+    const double zz = dt / tau;
+    const double alpha = exp_neg(zz);
+    const double b = tau * (1.0 - alpha);
+    int code = kStay;
+    advance_axis(p.x, p.vx, U.x, G.gx, tau, alpha, b, dt, G, B.lox, G.nx, 1, code, jump);
+    advance_axis(p.y, p.vy, U.y, G.gy, tau, alpha, b, dt, G, B.loy, G.ny, 3, code, jump);
+    advance_axis(p.z, p.vz, U.z, G.gz, tau, alpha, b, dt, G, B.loz, G.nz, 9, code, jump);
+    return code;
+}
+
+// Stable rank-in-code of the MIGRANTS of one row (code != stay); lane c owns the running count of code c.
+// One warp-uniform iteration per distinct migrant code present in the row (usually 0 to 2).
+__device__ __forceinline__ uint32_t migrant_rank(int code, unsigned mig_m, int lane, uint32_t& cnt_c)
+{
+    const unsigned lt = (1u << lane) - 1u;
+    uint32_t rank = 0;
+    unsigned todo = mig_m;
+    while (todo) {
+        const int leader = __ffs(todo) - 1;
+        const int c = __shfl_sync(0xffffffffu, code, leader);
+        const unsigned m = __ballot_sync(0xffffffffu, code == c) & mig_m;
+        const uint32_t base = __shfl_sync(0xffffffffu, cnt_c, c);
+        if (code == c) rank = base + __popc(m & lt);
+        if (lane == c) cnt_c += __popc(m);
+        todo &= ~m;
+    }
+    return rank;
+}
 
 // What a pushed tile carries from its push to its resolve one iteration later.
 struct TileInfo {
@@ -487,27 +638,25 @@ __device__ __forceinline__ ulonglong2 ld_relaxed_desc(const uint64_t* p)
 }
 
 // Sum of the (stay, migrant) aggregates desc[first .. first+n), n <= 32, one lane per descriptor; spins until
-// all of them carry this launch's epoch.
-__device__ __forceinline__ void sum_descs(const uint64_t* base, int n, int lane, uint32_t epoch, uint32_t& stay,
-                                          uint32_t& mig)
+// all of them carry this launch's epoch.  `w` is the first poll, loaded early by the caller (lanes < n).
+__device__ __forceinline__ void sum_descs(const uint64_t* base, int n, int lane, uint32_t epoch, ulonglong2 w,
+                                          uint32_t& stay, uint32_t& mig)
 {
     const bool need = lane < n;
     const uint64_t* pd = base + 2 * (need ? lane : 0);
-    ulonglong2 w = make_ulonglong2(0ull, 0ull);
     for (;;) {
-        bool ready = true;
-        if (need) {
-            w = ld_relaxed_desc(pd);
-            ready = (uint32_t)(w.x >> 34) == epoch && (uint32_t)(w.y >> 34) == epoch;
-        }
+#ifdef LCS_X_NOWAIT                // experiment: never wait for a predecessor (wrong results)
+        const bool ready = true;
+#else
+        const bool ready = !need || ((uint32_t)(w.x >> 34) == epoch && (uint32_t)(w.y >> 34) == epoch);
+#endif
         if (__all_sync(0xffffffffu, ready)) break;
-        __nanosleep(200);
+        __nanosleep(100);
+        if (need) w = ld_relaxed_desc(pd);
     }
     stay += __reduce_add_sync(0xffffffffu, need ? (uint32_t)w.x : 0u);
     mig += __reduce_add_sync(0xffffffffu, need ? (uint32_t)w.y : 0u);
 }
-
-constexpr int kTableSmemMax = 1024;     // tile_start[] and the subdomain coordinates are mirrored in shared memory up to this P
 
 __device__ __forceinline__ uint32_t pack_xyz(const Geom& G, int s)
 {   // px | py << 10 | pz << 20 (each < 1024, checked at lcs_create)
@@ -515,124 +664,204 @@ __device__ __forceinline__ uint32_t pack_xyz(const Geom& G, int s)
     return (uint32_t)px | ((uint32_t)py << 10) | ((uint32_t)pz << 20);
 }
 
+struct TileRef { int s, t; uint32_t cnt; bool ok; };     // a ticketed tile: subdomain, tile index, count[s]
+
 template <bool kFused>
 __global__ void __launch_bounds__(kBlock, kMinBlocks)
 k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch)
 {
-    extern __shared__ __align__(16) unsigned char s_raw[];
-    WarpStage* stage_all = reinterpret_cast<WarpStage*>(s_raw);                            // [kWarps][2]
-    uint32_t* s_ts = reinterpret_cast<uint32_t*>(s_raw + 2 * kWarps * sizeof(WarpStage));  // [P+1] if it fits
-    uint32_t* s_xyz = s_ts + (G.P + 1);                                                    // [P]   if it fits
+    extern __shared__ __align__(128) unsigned char s_raw[];
+    TileBuf* bufs = reinterpret_cast<TileBuf*>(s_raw);                                      // [kWarps][kNBuf]
+    uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_raw + kWarps * kNBuf * sizeof(TileBuf)); // [kWarps][kNBuf]
+    uint32_t* s_ts = reinterpret_cast<uint32_t*>(s_bar + kWarps * kNBuf);                   // [P+1] if it fits
+    uint32_t* s_xyz = s_ts + (G.P + 1);                                                     // [P]   if it fits
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool big = G.P > kTableSmemMax;
     if (!big) {
         for (int i = threadIdx.x; i <= G.P; i += kBlock) {
             s_ts[i] = T.tile_start[i];
             if (i < G.P) s_xyz[i] = pack_xyz(G, i);
         }
-        __syncthreads();                                   // the only block barrier of the kernel
     }
+    TileBuf* const my = bufs + warp * kNBuf;
+    const uint32_t bar0 = smem_u32(s_bar + warp * kNBuf);
+    if (lane == 0) {
+#pragma unroll
+        for (int b = 0; b < kNBuf; ++b) mbar_init(bar0 + 8u * b, 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();                                       // the only block barrier of the kernel
     auto ts = [&](int i) -> uint32_t { return big ? __ldg(T.tile_start + i) : s_ts[i]; };
     auto xyz = [&](int s) -> uint32_t { return big ? pack_xyz(G, s) : s_xyz[s]; };
-    // ticket -> subdomain: the tickets of a warp increase, so search forward from its previous subdomain
-    auto locate = [&](unsigned int g, int s_from) -> int {
-        int s = s_from;
-#pragma unroll 1
-        for (int k = 0; k < 4; ++k) {
-            if (g < ts(s + 1)) return s;
-            ++s;
-        }
-        int lo = s, hi = G.P;                                 // largest s with tile_start[s] <= g
-        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (ts(mid) <= g) lo = mid; else hi = mid; }
-        return lo;
-    };
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const unsigned lt = (1u << lane) - 1u;
     const unsigned int n_active = ts(G.P);
     const uint64_t tag = ((uint64_t)(epoch << 2) << 32) | (1ull << 32);
     const uint32_t cap32 = (uint32_t)G.cap;
-    const unsigned long long* const fS[8] = {
-        reinterpret_cast<const unsigned long long*>(S.f[0]), reinterpret_cast<const unsigned long long*>(S.f[1]),
-        reinterpret_cast<const unsigned long long*>(S.f[2]), reinterpret_cast<const unsigned long long*>(S.f[3]),
-        reinterpret_cast<const unsigned long long*>(S.f[4]), reinterpret_cast<const unsigned long long*>(S.f[5]),
-        reinterpret_cast<const unsigned long long*>(S.f[6]), reinterpret_cast<const unsigned long long*>(S.id)};
+    const size_t fstride = reinterpret_cast<const char*>(S.f[1]) - reinterpret_cast<const char*>(S.f[0]);   // bytes; id = field 7
+    int s_hint = 0;
+    uint32_t phase = 0;                                    // bit b: parity of the next completion of buffer b's mbarrier
 
-    unsigned int g = 0;
-    if (lane == 0) g = atomicAdd(T.ticket, 1u);
-    g = __shfl_sync(0xffffffffu, g, 0);
-    int s_cur = 0;
-    uint32_t cnt_cur = 0;
-    if (g < n_active) { s_cur = locate(g, 0); cnt_cur = __ldg(T.count + s_cur); }
+    // ticket -> (subdomain, tile): the tickets of a warp increase, so search forward from its previous subdomain
+    auto take_issue = [&]() -> unsigned int {              // lane 0 holds the ticket; the others 0
+        unsigned int g = 0;                                // atom.inc: an atom.add would be warp-aggregated by ptxas, and the
+        if (lane == 0)                                     // broadcast of the aggregated result waits for the atomic right here
+            asm volatile("atom.relaxed.gpu.global.inc.u32 %0, [%1], 0x7fffffff;" : "=r"(g) : "l"(T.ticket) : "memory");
+        return g;
+    };
+    auto take_finish = [&](TileRef& R, unsigned int g) {
+        g = __shfl_sync(0xffffffffu, g, 0);
+        R.ok = g < n_active;
+        R.s = R.t = 0; R.cnt = 0;
+        if (R.ok) {
+            int s = s_hint;
+            bool found = false;
+#pragma unroll 1
+            for (int k = 0; k < 4 && !found; ++k) {
+                if (g < ts(s + 1)) found = true; else ++s;
+            }
+            if (!found) {
+                int lo = s, hi = G.P;                         // largest s with tile_start[s] <= g
+                while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (ts(mid) <= g) lo = mid; else hi = mid; }
+                s = lo;
+            }
+            s_hint = s;
+            R.s = s; R.t = (int)(g - ts(s)); R.cnt = __ldg(T.count + s);
+        }
+    };
+    auto take = [&](TileRef& R) { take_finish(R, take_issue()); };
+    // bulk copy of the 8 field runs of tile R into buffer b (one lane issues; completion on the buffer's mbarrier)
+    auto issue_load = [&](const TileRef& R, int b) {
+        fence_proxy_async();                               // this warp's earlier accesses to the buffer come first
+        __syncwarp();
+        if (lane == 0) {
+            const uint32_t bar = bar0 + 8u * b;
+            mbar_expect_tx(bar, 8u * kTile * 8u);
+            const char* src = reinterpret_cast<const char*>(S.f[0]) + ((size_t)R.s * (size_t)G.cap + (size_t)R.t * kTile) * 8u;
+            const uint32_t dst = smem_u32(&my[b].f[0][0]);
+#pragma unroll
+            for (int a = 0; a < 8; ++a) bulk_g2s(dst + a * (kTile * 8u), src + a * fstride, kTile * 8u, bar);
+        }
+    };
+    auto wait_buf = [&](int b) {
+        mbar_wait(bar0 + 8u * b, (phase >> b) & 1u);
+        phase ^= 1u << b;
+    };
+
+    TileRef cur, nxt, nn;
+    take(cur);
+    if (!cur.ok) return;
+    issue_load(cur, 0);
+    take(nxt);
+    if (nxt.ok) issue_load(nxt, 1);
+    nn.ok = false; nn.s = nn.t = 0; nn.cnt = 0;
+    Gath Q;
+    if (kFused) {
+        wait_buf(0);
+        const unsigned long long* px = &my[0].f[0][0];
+        gather_issue(Q, F4, G.N, G.inv_dx, __longlong_as_double(px[lane]), __longlong_as_double(px[kTile + lane]),
+                     __longlong_as_double(px[2 * kTile + lane]), lane);
+    }
     TileInfo pend;
     pend.s = pend.t = 0; pend.n_stay = pend.n_mig = pend.run_start = 0;
     bool have_pend = false;
-    int buf = 0;
+    int bc = 0, bp = 0;                                    // buffers of the current and of the pending tile
     for (;;) {
-        const bool have = g < n_active;
+        const bool have = cur.ok;
         if (!have && !have_pend) break;
-        TileInfo cur = pend;
+        TileInfo ti = pend;
+        nn.ok = false;
+        unsigned int g_early = 0u;
+        ulonglong2 lb_w = make_ulonglong2(0ull, 0ull);     // first look-back poll of the pending tile (early, see the row loop)
+        unsigned long long lb_g = 0ull;
+        if (!have && have_pend) {                          // drain: no row loop ran, poll now
+            const int pr = pend.t & 31, pgrp = pend.t >> 5;
+            if (lane < pr) lb_w = ld_relaxed_desc(T.desc + ((size_t)pend.s * G.tiles_per_sub + (pend.t - pr) + lane) * 2);
+            if (lane < pgrp) lb_g = ld_relaxed_u64(T.gacc + (size_t)pend.s * G.lbgroups_per_sub + lane);
+        }
 
-        // ================= push of tile g: load, (push,) rank, stage, publish the aggregate =================
+        // ================= push of the current tile: (push,) rank, update in place, publish the aggregate =================
         if (have) {
-            WarpStage& W = stage_all[2 * warp + buf];
-            const int s = s_cur;
-            const uint32_t ts_s = ts(s);
-            const int t = (int)(g - ts_s);
-            const uint32_t cnt_s = cnt_cur;
+            TileBuf& W = my[bc];
+            const int bn = bc + 1 == kNBuf ? 0 : bc + 1;
+            const int s = cur.s, t = cur.t;
             const uint32_t first = (uint32_t)t * kTile;
-            const uint32_t slab0 = (uint32_t)s * cap32;
+            const uint32_t nvalid = min((uint32_t)kTile, cur.cnt - first);
+            const int nrows = (int)((nvalid + 31u) >> 5);
             SubBox B;
             B.lox = B.loy = B.loz = 0;
             if (kFused) {
                 const uint32_t c3 = xyz(s);
                 B.lox = (int)(c3 & 1023u) * G.nx; B.loy = (int)((c3 >> 10) & 1023u) * G.ny; B.loz = (int)(c3 >> 20) * G.nz;
                 if (s + kBrickLead < G.P)
-                    prefetch_brick_share(F4, G, xyz(s + kBrickLead), (uint32_t)t, ts(s + 1) - ts_s, lane);
+                    prefetch_brick_share(F4, G, xyz(s + kBrickLead), (uint32_t)t, ts(s + 1) - ts(s), lane);
+            } else {
+                wait_buf(bc);
             }
-            uint32_t cnt_c = 0;            // lane c: particles of the tile so far with code c
-            uint32_t n_mig = 0;            // migrants of the tile so far (warp-uniform)
+            if (lane < kRows) W.stay_m[lane] = 0u;
+            uint32_t cnt_c = 0;            // lane c: migrants of the tile so far with code c
+            uint32_t n_mig = 0, n_stay = 0;
+            g_early = 0u;
             bool jump = false;
 #pragma unroll 1
-            for (int r = 0; r < kRows; ++r) {
-                const uint32_t row0 = first + 32u * (uint32_t)r;
-                if (row0 >= cnt_s) break;
-                const uint32_t slot = row0 + (uint32_t)lane;
-                const bool valid = slot < cnt_s;
-                const uint32_t at = slab0 + min(slot, cnt_s - 1u);     // lanes past the end re-read the last particle
-                Particle p;
-                p.x = __longlong_as_double(ld_stream(fS[0] + at)); p.y = __longlong_as_double(ld_stream(fS[1] + at));
-                p.z = __longlong_as_double(ld_stream(fS[2] + at)); p.vx = __longlong_as_double(ld_stream(fS[3] + at));
-                p.vy = __longlong_as_double(ld_stream(fS[4] + at)); p.vz = __longlong_as_double(ld_stream(fS[5] + at));
-                p.d = __longlong_as_double(ld_stream(fS[6] + at));
-                const unsigned long long id = ld_stream(fS[7] + at);
+            for (int r = 0; r < nrows; ++r) {
+                Vec3 U;
+                U.x = U.y = U.z = 0.0;
+                if (kFused) U = gather_reduce(Q, lane);
+                if (r + 1 == nrows) {
+                    // long-latency requests of the tile end, issued under the arithmetic of the last row (and BEFORE the
+                    // gather of the next row: ptxas tracks all of them on one scoreboard, so a load issued after the gather
+                    // would first wait for it): the ticket
+                    // of the tile after next, and the first look-back poll of the pending tile
+                    if (nxt.ok) g_early = take_issue();
+                    if (have_pend) {
+                        const int pr = pend.t & 31, pgrp = pend.t >> 5;
+                        if (lane < pr) lb_w = ld_relaxed_desc(T.desc + ((size_t)pend.s * G.tiles_per_sub + (pend.t - pr) + lane) * 2);
+                        if (lane < pgrp) lb_g = ld_relaxed_u64(T.gacc + (size_t)pend.s * G.lbgroups_per_sub + lane);
+                    }
+                }
+                if (kFused) {
+                    // gather of the next row: of this tile, or row 0 of the next tile (whose bulk copy must have landed)
+                    // (after the very last row of this warp's work the current row is gathered again, unused: issuing
+                    // unconditionally keeps the in-flight registers of Q out of any copy)
+                    const unsigned long long* px = &W.f[0][32 * r];
+                    if (r + 1 < nrows) px += 32;
+                    else if (nxt.ok) { wait_buf(bn); px = &my[bn].f[0][0]; }
+                    gather_issue(Q, F4, G.N, G.inv_dx, __longlong_as_double(px[lane]),
+                                 __longlong_as_double(px[kTile + lane]), __longlong_as_double(px[2 * kTile + lane]), lane);
+                }
+                const uint32_t p = 32u * (uint32_t)r + (uint32_t)lane;
+                const bool valid = p < nvalid;
                 int code;
                 if (kFused) {
+                    Particle q;
+                    q.x = __longlong_as_double(W.f[0][p]); q.y = __longlong_as_double(W.f[1][p]);
+                    q.z = __longlong_as_double(W.f[2][p]); q.vx = __longlong_as_double(W.f[3][p]);
+                    q.vy = __longlong_as_double(W.f[4][p]); q.vz = __longlong_as_double(W.f[5][p]);
+                    q.d = __longlong_as_double(W.f[6][p]);
                     bool jmp = false;
-                    code = push_particle(p, F4, G, B, dt, lane, jmp);
+                    code = advance_particle(q, U, G, B, dt, jmp);
                     jump |= jmp && valid;
+                    W.f[0][p] = __double_as_longlong(q.x); W.f[1][p] = __double_as_longlong(q.y);
+                    W.f[2][p] = __double_as_longlong(q.z); W.f[3][p] = __double_as_longlong(q.vx);
+                    W.f[4][p] = __double_as_longlong(q.vy); W.f[5][p] = __double_as_longlong(q.vz);
                 } else {
-                    code = min((int)S.code[at], 26);
+                    code = min((int)S.code[(uint32_t)s * cap32 + first + min(p, nvalid - 1u)], 26);
                 }
-                if (!valid) code = kInvalid;
-                const uint32_t rank = row_rank(code, valid, lane, cnt_c);
+                const unsigned stay_m = __ballot_sync(0xffffffffu, valid && code == kStay);
                 const unsigned mig_m = __ballot_sync(0xffffffffu, valid && code != kStay);
-                if (valid) {
-                    uint32_t pos = rank;                                    // stayer: output order from the front
-                    if (code != kStay) {
-                        const uint32_t a = n_mig + __popc(mig_m & lt);      // migrant: arrival order from the back
-                        pos = kTile - 1 - a;
-                        W.meta[a] = (unsigned short)(code | (rank << 5));
-                    }
-                    W.f[0][pos] = __double_as_longlong(p.x); W.f[1][pos] = __double_as_longlong(p.y);
-                    W.f[2][pos] = __double_as_longlong(p.z); W.f[3][pos] = __double_as_longlong(p.vx);
-                    W.f[4][pos] = __double_as_longlong(p.vy); W.f[5][pos] = __double_as_longlong(p.vz);
-                    W.f[6][pos] = __double_as_longlong(p.d); W.f[7][pos] = id;
+                if (mig_m) {
+                    const uint32_t rank = migrant_rank(code, mig_m, lane, cnt_c);
+                    if ((mig_m >> lane) & 1u)
+                        W.mlist[n_mig + __popc(mig_m & lt)] = p | ((uint32_t)code << 8) | (rank << 16);
+                    n_mig += __popc(mig_m);
                 }
-                n_mig += __popc(mig_m);
+                if (lane == 0) W.stay_m[r] = stay_m;
+                n_stay += __popc(stay_m);
             }
             if (jump) raise(T.status, -5);
             __syncwarp();
             // tile totals; publish the aggregate and the per-code byte counts
-            const uint32_t n_stay = __shfl_sync(0xffffffffu, cnt_c, kStay);
+            if (lane == kStay) cnt_c = n_stay;
             const uint32_t magg = (lane < kNC && lane != kStay) ? cnt_c : 0u;
             uint32_t inc = magg;
 #pragma unroll
@@ -646,27 +875,9 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             if (lane == 2)      // group accumulator [tiles done : 24 | migrants : 20 | stayers : 20], zeroed before the launch
                 atomicAdd(T.gacc + (size_t)s * G.lbgroups_per_sub + (t >> 5),
                           (1ull << 40) | ((unsigned long long)n_mig << 20) | (unsigned long long)n_stay);
-            cur.s = s; cur.t = t; cur.n_stay = n_stay; cur.n_mig = n_mig; cur.run_start = inc - magg;
-        }
-
-        // ================= next ticket =================
-        // Taken right after this tile's aggregate is out (a ticket held across a wait is a convoy);
-        // its subdomain's count and its particle lines (8 fields x 8 lines, two prefetches per lane) are requested now
-        // and consumed one iteration later.
-        unsigned int g_next = 0xffffffffu;
-        if (have) {
-            if (lane == 0) g_next = atomicAdd(T.ticket, 1u);
-            g_next = __shfl_sync(0xffffffffu, g_next, 0);
-            if (g_next < n_active) {
-                s_cur = locate(g_next, s_cur);
-                cnt_cur = __ldg(T.count + s_cur);
-                const uint32_t pat = (uint32_t)s_cur * cap32 + (g_next - ts(s_cur)) * kTile;
-                const size_t fstride = reinterpret_cast<const char*>(fS[1]) - reinterpret_cast<const char*>(fS[0]);
-                const char* pf = reinterpret_cast<const char*>(fS[0]) + (size_t)pat * 8u + (size_t)(lane & 7) * 128u
-                                 + (size_t)(lane >> 3) * fstride;
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(pf));
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(pf + 4 * fstride));
-            }
+            ti.s = s; ti.t = t; ti.n_stay = n_stay; ti.n_mig = n_mig; ti.run_start = inc - magg;
+            // ticket of the tile after next: taken right after this tile's aggregate is out
+            if (nxt.ok) take_finish(nn, g_early);
         }
 
         // ================= resolve of the previous tile: look-back, then copy-out =================
@@ -676,48 +887,61 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
         // waited for is produced by the PUSH of a tile with a smaller ticket -- never by another tile's
         // resolve -- and this warp has pushed a whole tile in between.
         if (have_pend) {
-            const WarpStage& W = stage_all[2 * warp + (buf ^ 1)];
+            const TileBuf& W = my[bp];
             const int s = pend.s, t = pend.t;
             const size_t tile_row = (size_t)s * G.tiles_per_sub + t;
             const int r = t & 31, grp = t >> 5;
             uint32_t excl_stay = 0, excl_mig = 0;
-            if (r > 0) sum_descs(T.desc + (tile_row - r) * 2, r, lane, epoch, excl_stay, excl_mig);
+            if (r > 0) sum_descs(T.desc + (tile_row - r) * 2, r, lane, epoch, lb_w, excl_stay, excl_mig);
             const unsigned long long* ga = T.gacc + (size_t)s * G.lbgroups_per_sub;
             for (int g0 = 0; g0 < grp; g0 += 32) {
                 const bool need = g0 + lane < grp;
-                unsigned long long w = 0;
+                unsigned long long w = lb_g;
+                if (g0 > 0 && need) w = ld_relaxed_u64(ga + g0 + lane);
                 for (;;) {
-                    bool ready = true;
-                    if (need) { w = ld_relaxed_u64(ga + g0 + lane); ready = (w >> 40) == 32ull; }
+#ifdef LCS_X_NOWAIT
+                    const bool ready = true;
+#else
+                    const bool ready = !need || (w >> 40) == 32ull;
+#endif
                     if (__all_sync(0xffffffffu, ready)) break;
-                    __nanosleep(200);
+                    __nanosleep(100);
+                    if (need) w = ld_relaxed_u64(ga + g0 + lane);
                 }
                 excl_stay += __reduce_add_sync(0xffffffffu, need ? (uint32_t)(w & 0xfffffull) : 0u);
                 excl_mig += __reduce_add_sync(0xffffffffu, need ? (uint32_t)((w >> 20) & 0xfffffull) : 0u);
             }
-            // copy-out: stayers in place (compacted, coalesced), migrants to the send region
-            const uint32_t stay_base = (uint32_t)s * cap32 + excl_stay;
-#ifdef LCS_X_NOSTORE
+            // copy-out, stayers: in place, compacted; the stayers of a row are consecutive lanes -> consecutive slots
+            uint32_t base = (uint32_t)s * cap32 + excl_stay;
+#ifdef LCS_X_NOSTORE             // experiment: no stayer stores
             if (excl_stay == 0xffffffffu)
 #endif
-            for (uint32_t j = lane; j < pend.n_stay; j += 32) {
-                const uint32_t dst = stay_base + j;
+#pragma unroll 1
+            for (int rr = 0; rr < kRows; ++rr) {
+                const unsigned m = W.stay_m[rr];
+                if (m == 0u) continue;
+                if ((m >> lane) & 1u) {
+                    const uint32_t dst = base + __popc(m & lt);
+                    const uint32_t src = 32u * (uint32_t)rr + (uint32_t)lane;
 #pragma unroll
-                for (int a = 0; a < 7; ++a) st_stream(S.f[a] + dst, W.f[a][j]);
-                st_stream(S.id + dst, W.f[7][j]);
+                    for (int a = 0; a < 7; ++a) st_stream(S.f[a] + dst, W.f[a][src]);
+                    st_stream(S.id + dst, W.f[7][src]);
+                }
+                base += __popc(m);
             }
+            // copy-out, migrants: to the send region of s, grouped by code inside the tile's chunk
             if (pend.n_mig) {
-                bool fits = (long long)excl_mig + (long long)pend.n_mig <= G.send_cap;
+                const bool fits = (long long)excl_mig + (long long)pend.n_mig <= G.send_cap;
                 if (!fits && lane == 0) raise(T.status, -4);
                 const size_t sendbase = (size_t)s * (size_t)G.send_cap + excl_mig;
                 for (uint32_t a0 = 0; a0 < pend.n_mig; a0 += 32) {
                     const uint32_t a = a0 + lane;
                     const bool ok = a < pend.n_mig;
-                    const uint32_t mt = ok ? W.meta[a] : 0u;
-                    const uint32_t off = __shfl_sync(0xffffffffu, pend.run_start, mt & 31u) + (mt >> 5);
+                    const uint32_t e = ok ? W.mlist[a] : 0u;
+                    const uint32_t off = __shfl_sync(0xffffffffu, pend.run_start, (e >> 8) & 31u) + (e >> 16);
                     if (ok && fits) {
                         const size_t dst = sendbase + off;
-                        const uint32_t src = kTile - 1 - a;
+                        const uint32_t src = e & 0xffu;
 #pragma unroll
                         for (int q = 0; q < 7; ++q) st_stream(Snd.f[q] + dst, W.f[q][src]);
                         st_stream(Snd.id + dst, W.f[7][src]);
@@ -725,11 +949,14 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 }
             }
         }
-        __syncwarp();                                   // the staging area just copied out is reused next
-        g = g_next;                                     // 0xffffffff once the tickets have run out
-        pend = cur;
+        // the buffer just resolved (or, the first time, the unused third one) receives the tile after next
+        if (nn.ok) issue_load(nn, bc + 2 >= kNBuf ? bc + 2 - kNBuf : bc + 2);
+        pend = ti;
         have_pend = have;
-        buf ^= 1;
+        bp = bc;
+        bc = bc + 1 == kNBuf ? 0 : bc + 1;
+        cur = nxt;
+        nxt = nn;
     }
 }
 
