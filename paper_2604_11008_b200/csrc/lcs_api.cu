@@ -176,8 +176,6 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     G.K_tau = prm->rho_ratio / (18.0 * prm->nu);  // tau_p = K_tau * d^2
     G.L_below = std::nextafter(G.L, 0.0);
     G.gx = prm->g[0]; G.gy = prm->g[1]; G.gz = prm->g[2];
-    G.inv_brick_w = 1.0f / (float)(G.ny + 2);
-    G.brick_lines = ((G.nz + 2) * 32 + 96 + 127) / 128;
     char* w = static_cast<char*>(d_workspace);
     const size_t P = (size_t)G.P;
     for (int a = 0; a < 7; ++a) h->S.f[a] = reinterpret_cast<double*>(w + L.slab_f[a]);

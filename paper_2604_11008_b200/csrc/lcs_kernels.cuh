@@ -27,9 +27,6 @@ constexpr int kWarps = kBlock / 32;
 #ifndef LCS_ROWS
 #define LCS_ROWS 2
 #endif
-#ifndef LCS_BRICK_LEAD
-#define LCS_BRICK_LEAD 2
-#endif
 constexpr int kRows = LCS_ROWS;              // rows (particles per lane) of a warp tile
 constexpr int kTile = 32 * kRows;            // particles per tile
 constexpr int kStay = 13;
@@ -46,8 +43,6 @@ struct Geom {
     int lbgroups_per_sub;              // ceil(tiles_per_sub / 32): look-back groups
     int64_t cap, send_cap;
     double inv_dx, K_tau, L, L_below, gx, gy, gz;
-    float inv_brick_w;                 // 1 / (ny + 2), for the brick prefetch shares
-    int brick_lines;                   // 128-byte lines of one z-run of a fluid brick (nz + 2 records)
 };
 
 struct Slabs {                         // SoA particle storage, P*cap slots each
@@ -110,7 +105,15 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v)
 }
 
 // exp(-z), z >= 0: range reduction by ln2 (hi/lo), degree-14 Taylor polynomial in Horner form with
-// explicit fma, scaling by exponent arithmetic.  DESIGN.md R-3.
+// explicit fma, scaling by exponent arithmetic.  DESIGN.md R-3.  The coefficients (correctly rounded
+// 1/j!, j = 14 .. 0) sit in constant memory so that each fma takes its addend straight from the
+// constant bank instead of two moves.
+__constant__ double kExpC[15] = {1.1470745597729725e-11, 1.6059043836821613e-10, 2.08767569878681e-09,
+                                 2.505210838544172e-08,  2.755731922398589e-07,  2.7557319223985893e-06,
+                                 2.48015873015873e-05,   0.0001984126984126984,  0.001388888888888889,
+                                 0.008333333333333333,   0.041666666666666664,   0.16666666666666666,
+                                 0.5,                    1.0,                    1.0};
+
 __device__ __forceinline__ double exp_neg(double z)
 {
     if (!(z <= 708.0)) return (z != z) ? z : 0.0;
@@ -118,21 +121,9 @@ __device__ __forceinline__ double exp_neg(double z)
     const double k = rint(y * 1.4426950408889634);
     double r = fma(-k, 6.93147180369123816490e-01, y);
     r = fma(-k, 1.90821492927058770002e-10, r);
-    double p = 1.1470745597729725e-11;            // 1/14!
-    p = fma(p, r, 1.6059043836821613e-10);        // 1/13!
-    p = fma(p, r, 2.08767569878681e-09);          // 1/12!
-    p = fma(p, r, 2.505210838544172e-08);         // 1/11!
-    p = fma(p, r, 2.755731922398589e-07);         // 1/10!
-    p = fma(p, r, 2.7557319223985893e-06);        // 1/9!
-    p = fma(p, r, 2.48015873015873e-05);          // 1/8!
-    p = fma(p, r, 0.0001984126984126984);         // 1/7!
-    p = fma(p, r, 0.001388888888888889);          // 1/6!
-    p = fma(p, r, 0.008333333333333333);          // 1/5!
-    p = fma(p, r, 0.041666666666666664);          // 1/4!
-    p = fma(p, r, 0.16666666666666666);           // 1/3!
-    p = fma(p, r, 0.5);
-    p = fma(p, r, 1.0);
-    p = fma(p, r, 1.0);
+    double p = kExpC[0];                          // 1/14!
+#pragma unroll
+    for (int j = 1; j < 15; ++j) p = fma(p, r, kExpC[j]);
     // 2^k, k in [-1022, 0]: always a normal number, so the product is exact
     const long long bits = (long long)(1023 + (int)k) << 52;
     return p * __longlong_as_double(bits);
@@ -448,7 +439,6 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
 //   float reciprocals (prefetch shares); the ticket -> (s,t) map is an incremental search from the
 //   previous subdomain; particle slots are 32-bit indices (P*cap < 2^32 is checked at lcs_create).
 // ---------------------------------------------------------------------------------------------
-constexpr int kBrickLead = LCS_BRICK_LEAD;   // the tiles of subdomain s prefetch the fluid brick of s + kBrickLead
 constexpr int kNBuf = 3;                     // tile buffers per warp: loading / being pushed / awaiting resolve
 constexpr int kTableSmemMax = 1024;          // tile_start[] and the subdomain coordinates are mirrored in shared memory up to this P
 
@@ -487,45 +477,6 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 __device__ __forceinline__ void fence_proxy_async()
 {   // order this thread's generic-proxy shared-memory accesses before later async-proxy (bulk copy) accesses
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-}
-
-// ---------------------------------------------------------------------------------------------
-// Fluid brick prefetch.  Tiles are processed in ticket order, so the fluid records a later subdomain
-// will gather from can be pulled into L2 ahead of time with full-line prefetches, one share per
-// tile, instead of being demand-missed one 32-byte sector at a time by the first particle that
-// touches each cell.  Runs along z are contiguous in the internal layout (lane = 128-byte line of a
-// column); the two seam planes in z are left to demand misses.  Purely a hint: shares are computed
-// with float reciprocals and clamped, coverage may overlap by a column.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void prefetch_brick_share(const double* __restrict__ F4, const Geom& G, uint32_t qxyz,
-                                                     uint32_t share, uint32_t nshares, int lane)
-{
-    const int qx = (int)(qxyz & 1023u), qy = (int)((qxyz >> 10) & 1023u), qz = (int)(qxyz >> 20);
-    const int ka = max(0, qz * G.nz - 1);
-    const uint32_t w = (uint32_t)(G.ny + 2);
-    const uint32_t nrun = (uint32_t)(G.nx + 2) * w;                                   // (i,j) columns of the brick
-    uint32_t per = (uint32_t)__fdividef((float)(nrun + nshares), (float)nshares);     // ~ceil(nrun / nshares)
-    per = min(per, 8u);
-    const uint32_t r0 = share * per;
-    if (r0 >= nrun) return;
-    const uint32_t r1 = min(nrun, r0 + per);
-    uint32_t ii = (uint32_t)((float)r0 * G.inv_brick_w);
-    ii = min(ii, (uint32_t)(G.nx + 1));
-    if (ii * w > r0) --ii;
-    uint32_t jj = r0 - ii * w;
-    if (jj >= w) { jj -= w; ++ii; }
-    const uint32_t z0 = (uint32_t)ka * 32u & ~127u;                                    // byte offset inside a column
-    const uint32_t zend = min((uint32_t)G.N * 32u, z0 + (uint32_t)G.brick_lines * 128u);
-    for (uint32_t rj = r0; rj < r1; ++rj) {                                            // warp-uniform, <= 8 trips
-        int i = qx * G.nx - 1 + (int)ii, j = qy * G.ny - 1 + (int)jj;
-        i = i < 0 ? i + G.N : (i >= G.N ? i - G.N : i);
-        j = j < 0 ? j + G.N : (j >= G.N ? j - G.N : j);
-        const uint32_t col = ((uint32_t)i * (uint32_t)G.N + (uint32_t)j) * (uint32_t)G.N;   // record index of (i,j,0)
-        const char* a = reinterpret_cast<const char*>(F4) + (size_t)col * 32u;
-        for (uint32_t zo = z0 + (uint32_t)lane * 128u; zo < zend; zo += 32u * 128u)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(a + zo));
-        if (++jj == w) { jj = 0; ++ii; }
-    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -589,18 +540,28 @@ __device__ __forceinline__ Vec3 gather_reduce(const Gath& Q, int lane)
     return U;
 }
 
-// a2-a3 given the gathered fluid velocity U.  Returns the destination code.
-__device__ __forceinline__ int advance_particle(Particle& p, const Vec3& U, const Geom& G, const SubBox& B, double dt,
-                                                bool& jump)
+// a2, the part that depends on the particle alone: tau_p, alpha = exp(-dt/tau_p), b = tau_p (1 - alpha).  A serial
+// chain of ~35 fp64 operations; kept apart so that it can be issued under the lerps of the gather.
+struct Drag { double tau, alpha, b; };
+
+__device__ __forceinline__ Drag drag_coeffs(double d, double dt, const Geom& G)
 {
-    const double tau = (G.K_tau * p.d) * p.d;     // tau_p = (rho_p/rho) d^2 / (18 nu)
-    const double zz = dt / tau;
-    const double alpha = exp_neg(zz);
-    const double b = tau * (1.0 - alpha);
+    Drag D;
+    D.tau = (G.K_tau * d) * d;                    // tau_p = (rho_p/rho) d^2 / (18 nu)
+    const double zz = dt / D.tau;
+    D.alpha = exp_neg(zz);
+    D.b = D.tau * (1.0 - D.alpha);
+    return D;
+}
+
+// a2-a3 given the gathered fluid velocity U.  Returns the destination code.
+__device__ __forceinline__ int advance_particle(Particle& p, const Vec3& U, const Drag& D, const Geom& G,
+                                                const SubBox& B, double dt, bool& jump)
+{
     int code = kStay;
-    advance_axis(p.x, p.vx, U.x, G.gx, tau, alpha, b, dt, G, B.lox, G.nx, 1, code, jump);
-    advance_axis(p.y, p.vy, U.y, G.gy, tau, alpha, b, dt, G, B.loy, G.ny, 3, code, jump);
-    advance_axis(p.z, p.vz, U.z, G.gz, tau, alpha, b, dt, G, B.loz, G.nz, 9, code, jump);
+    advance_axis(p.x, p.vx, U.x, G.gx, D.tau, D.alpha, D.b, dt, G, B.lox, G.nx, 1, code, jump);
+    advance_axis(p.y, p.vy, U.y, G.gy, D.tau, D.alpha, D.b, dt, G, B.loy, G.ny, 3, code, jump);
+    advance_axis(p.z, p.vz, U.z, G.gz, D.tau, D.alpha, D.b, dt, G, B.loz, G.nz, 9, code, jump);
     return code;
 }
 
@@ -644,14 +605,14 @@ __device__ __forceinline__ void sum_descs(const uint64_t* base, int n, int lane,
 {
     const bool need = lane < n;
     const uint64_t* pd = base + 2 * (need ? lane : 0);
-    for (;;) {
+    for (unsigned ns = 64;; ns = min(ns * 2u, 1024u)) {
 #ifdef LCS_X_NOWAIT                // experiment: never wait for a predecessor (wrong results)
         const bool ready = true;
 #else
         const bool ready = !need || ((uint32_t)(w.x >> 34) == epoch && (uint32_t)(w.y >> 34) == epoch);
 #endif
         if (__all_sync(0xffffffffu, ready)) break;
-        __nanosleep(100);
+        __nanosleep(ns);
         if (need) w = ld_relaxed_desc(pd);
     }
     stay += __reduce_add_sync(0xffffffffu, need ? (uint32_t)w.x : 0u);
@@ -792,8 +753,6 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             if (kFused) {
                 const uint32_t c3 = xyz(s);
                 B.lox = (int)(c3 & 1023u) * G.nx; B.loy = (int)((c3 >> 10) & 1023u) * G.ny; B.loz = (int)(c3 >> 20) * G.nz;
-                if (s + kBrickLead < G.P)
-                    prefetch_brick_share(F4, G, xyz(s + kBrickLead), (uint32_t)t, ts(s + 1) - ts(s), lane);
             } else {
                 wait_buf(bc);
             }
@@ -804,20 +763,26 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             bool jump = false;
 #pragma unroll 1
             for (int r = 0; r < nrows; ++r) {
+                const uint32_t p = 32u * (uint32_t)r + (uint32_t)lane;
                 Vec3 U;
                 U.x = U.y = U.z = 0.0;
-                if (kFused) U = gather_reduce(Q, lane);
+                Drag D;
+                D.tau = D.alpha = D.b = 0.0;
+                if (kFused) {
+                    D = drag_coeffs(__longlong_as_double(W.f[6][p]), dt, G);   // serial chain, issued under the lerps
+                    U = gather_reduce(Q, lane);
+                }
                 if (r + 1 == nrows) {
                     // long-latency requests of the tile end, issued under the arithmetic of the last row (and BEFORE the
                     // gather of the next row: ptxas tracks all of them on one scoreboard, so a load issued after the gather
                     // would first wait for it): the ticket
                     // of the tile after next, and the first look-back poll of the pending tile
-                    if (nxt.ok) g_early = take_issue();
                     if (have_pend) {
                         const int pr = pend.t & 31, pgrp = pend.t >> 5;
                         if (lane < pr) lb_w = ld_relaxed_desc(T.desc + ((size_t)pend.s * G.tiles_per_sub + (pend.t - pr) + lane) * 2);
                         if (lane < pgrp) lb_g = ld_relaxed_u64(T.gacc + (size_t)pend.s * G.lbgroups_per_sub + lane);
                     }
+                    if (nxt.ok) g_early = take_issue();       // after the polls: they would wait on the atomic's scoreboard
                 }
                 if (kFused) {
                     // gather of the next row: of this tile, or row 0 of the next tile (whose bulk copy must have landed)
@@ -829,7 +794,6 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     gather_issue(Q, F4, G.N, G.inv_dx, __longlong_as_double(px[lane]),
                                  __longlong_as_double(px[kTile + lane]), __longlong_as_double(px[2 * kTile + lane]), lane);
                 }
-                const uint32_t p = 32u * (uint32_t)r + (uint32_t)lane;
                 const bool valid = p < nvalid;
                 int code;
                 if (kFused) {
@@ -837,9 +801,9 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     q.x = __longlong_as_double(W.f[0][p]); q.y = __longlong_as_double(W.f[1][p]);
                     q.z = __longlong_as_double(W.f[2][p]); q.vx = __longlong_as_double(W.f[3][p]);
                     q.vy = __longlong_as_double(W.f[4][p]); q.vz = __longlong_as_double(W.f[5][p]);
-                    q.d = __longlong_as_double(W.f[6][p]);
+                    q.d = 0.0;
                     bool jmp = false;
-                    code = advance_particle(q, U, G, B, dt, jmp);
+                    code = advance_particle(q, U, D, G, B, dt, jmp);
                     jump |= jmp && valid;
                     W.f[0][p] = __double_as_longlong(q.x); W.f[1][p] = __double_as_longlong(q.y);
                     W.f[2][p] = __double_as_longlong(q.z); W.f[3][p] = __double_as_longlong(q.vx);
@@ -898,14 +862,14 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 const bool need = g0 + lane < grp;
                 unsigned long long w = lb_g;
                 if (g0 > 0 && need) w = ld_relaxed_u64(ga + g0 + lane);
-                for (;;) {
+                for (unsigned ns = 64;; ns = min(ns * 2u, 1024u)) {
 #ifdef LCS_X_NOWAIT
                     const bool ready = true;
 #else
                     const bool ready = !need || (w >> 40) == 32ull;
 #endif
                     if (__all_sync(0xffffffffu, ready)) break;
-                    __nanosleep(100);
+                    __nanosleep(ns);
                     if (need) w = ld_relaxed_u64(ga + g0 + lane);
                 }
                 excl_stay += __reduce_add_sync(0xffffffffu, need ? (uint32_t)(w & 0xfffffull) : 0u);
