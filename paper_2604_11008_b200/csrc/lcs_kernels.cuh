@@ -761,8 +761,13 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             uint32_t n_mig = 0, n_stay = 0;
             g_early = 0u;
             bool jump = false;
+#ifdef LCS_X_UNROLL_ROWS
+#pragma unroll
+#else
 #pragma unroll 1
-            for (int r = 0; r < nrows; ++r) {
+#endif
+            for (int r = 0; r < kRows; ++r) {
+                if (r >= nrows) break;
                 const uint32_t p = 32u * (uint32_t)r + (uint32_t)lane;
                 Vec3 U;
                 U.x = U.y = U.z = 0.0;
