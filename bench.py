@@ -28,6 +28,9 @@ sys.path.insert(0, ROOT)
 
 METRIC = "particles/s (fused push + prefix-scan migrate step)"
 F8 = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
+# DRAM bytes of one k_tile_pass<fused> launch from the committed ncu --set full capture (profiles/r1c_tile_pass_full.md):
+# 9.080516 GB read + 4.309978 GB written.  --traffic-bytes overrides it after a new capture.
+NCU_TRAFFIC_BYTES = {"Large": 9.080516e9 + 4.309978e9}
 
 
 def measured_peak_hbm():
@@ -295,8 +298,14 @@ def run_cuda(args):
     tile_ms = prof["tile_pass_ms"] / max(prof["steps"], 1)
     achieved = alg_bytes / (tile_ms * 1e-3) / 1e9
     step_bytes = n * (128.0 + 128.0 * m) + 24.0 * N ** 3
+    traffic = args.traffic_bytes
+    if traffic is None and args.workload in NCU_TRAFFIC_BYTES:
+        traffic = NCU_TRAFFIC_BYTES[args.workload]
     roofline = {"bound": "hbm", "kernel": "k_tile_pass<fused>", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": args.traffic_bytes, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic,
+                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch, profiles/r1c_tile_pass_full.md"
+                if traffic is not None else None,
+                "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": tile_ms,
                 "kernel_share_of_step": tile_ms / ms_step,
                 "table_ms": prof["table_ms"] / max(prof["steps"], 1),

@@ -155,6 +155,28 @@ def test_fused_and_unfused_match_oracle_ballistic(torch_cuda, oracle_lib, P, N):
     dev.close(); dev2.close()
 
 
+@pytest.mark.parametrize("P,N,per_sub", [((16, 16, 8), 32, 40),      # P = 2048 > 1024: tables read from global memory
+                                         ((1, 1, 2), 8, 80000),      # > 32 look-back groups of 32 tiles in one slab
+                                         ((32, 1, 1), 32, 700)])
+def test_many_subdomains_and_long_slabs(torch_cuda, oracle_lib, P, N, per_sub):
+    """The two table paths of the tile pass (shared-memory mirror up to P = 1024, global beyond), slabs long enough for
+    a second chunk of group accumulators in the look-back, and the incremental ticket search across many short slabs."""
+    rng = np.random.default_rng(P[0] * 1000 + per_sub)
+    nP = P[0] * P[1] * P[2]
+    n = per_sub * nP + 5
+    Ls = np.array([L / P[0], L / P[1], L / P[2]])
+    parts = random_parts(rng, n, 0.45 * Ls)
+    z = np.zeros(N ** 3)
+    cap = 2 * (int(1.6 * n / nP) // 2 + 100)
+    o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, cap, (z, z, z), parts)
+    for step in range(2):
+        assert o.step(0.6) == 0
+        dev.step_fused(0.6)
+        assert dev.get_status() == (0, n, o.n_migrated_last)
+        compare_packed(dev, o, f"P={P} step {step}")
+    dev.close()
+
+
 def test_all_27_codes_hand_placed(torch_cuda, oracle_lib):
     for P in [(3, 3, 3), (2, 2, 2), (1, 2, 3), (1, 1, 1)]:
         N = 24
