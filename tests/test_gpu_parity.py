@@ -357,52 +357,69 @@ def test_stress_shape_sample(torch_cuda, oracle_lib):
 
 
 @pytest.mark.slow
-def test_large_full_size_properties(torch_cuda, oracle_lib):
-    """BASELINE.json's Large at full size (2^26 particles, 512^3, 8x8x8, capacity 1.25x) in the launch
-    configuration bench.py times.  Properties that hold at any size + a sample recomputed by the oracle."""
+@pytest.mark.parametrize("name", ["Clustered", "Large", "Stress"])
+def test_full_size_properties(torch_cuda, oracle_lib, name):
+    """BASELINE.json's configurations at FULL size (Large: 2^26 particles, 512^3, 8x8x8, capacity 1.25x; Stress: 2^28
+    particles, 1024^3, 30 % migrants; Clustered: 4096 clumps) in the launch configuration bench.py times.  Properties
+    that hold at any size + a sample recomputed one by one by the oracle on the full fluid field."""
     torch = torch_cuda
     from workloads import gen
     from paper_2604_11008_b200 import LCS
-    cfg = gen.get_config("Large")
+    cfg = gen.get_config(name)
     n, N, P = cfg["n"], cfg["N"], cfg["P"]
     nP = P[0] * P[1] * P[2]
     wl = gen.make_workload(cfg, device="cuda")
-    dev = LCS(N, *P, cfg["capacity"], g=cfg["g"])
+    dev = LCS(N, *P, cfg["capacity"], g=cfg["g"], send_capacity=cfg["capacity"] // 2)
     dev.set_fluid(wl["u"], wl["v"], wl["w"])
     parts = wl["particles"]
     dev.set_particles(*(parts[k] for k in F8))
     assert dev.get_status()[:2] == (0, n)
-    before = dev.get_particles(n)
-    slab_of = lambda c: torch.repeat_interleave(torch.arange(nP, device="cuda"), c)
-    prev_slab = torch.empty(n, dtype=torch.int64, device="cuda")
-    prev_pos = torch.empty(n, dtype=torch.int64, device="cuda")
-    prev_slab[before["id"]] = slab_of(before["counts"])
-    prev_pos[before["id"]] = torch.arange(n, device="cuda")
-    dev.step_fused(cfg["dt"])
-    e, n_tot, n_mig = dev.get_status()
-    assert e == 0 and n_tot == n and 0.03 * n < n_mig < 0.07 * n
-    after = dev.get_particles(n)
-    # conservation of count and of the id multiset
-    assert int(after["counts"].sum()) == n
-    assert torch.equal(torch.sort(after["id"]).values, torch.arange(n, device="cuda"))
-    # containment: every particle sits in the slab of the subdomain that contains its position
-    inv_dx = N / L
-    cell = lambda a: torch.clamp(torch.floor(a * inv_dx).to(torch.int64), 0, N - 1)
-    owner = (cell(after["x"]) // (N // P[0]) + P[0] * (cell(after["y"]) // (N // P[1])
-             + P[1] * (cell(after["z"]) // (N // P[2]))))
-    cur_slab = slab_of(after["counts"])
-    assert torch.equal(owner, cur_slab)
-    # order: stayers first in original order, then incoming by (source slab, source slot)
-    ps, pp = prev_slab[after["id"]], prev_pos[after["id"]]
-    stay = ps == cur_slab
-    assert int(stay.sum()) == n - n_mig
-    key = torch.where(stay, torch.full_like(ps, -1), ps) * (2 * n) + pp      # (is_migrant, source, source slot)
-    same = cur_slab[1:] == cur_slab[:-1]
-    assert bool(torch.all(key[1:][same] > key[:-1][same]))
-    # a sample recomputed one by one by the oracle (push only: positions, velocities)
     rng = np.random.default_rng(11)
     pick = torch.from_numpy(np.sort(rng.choice(n, 4096, replace=False))).cuda()
     sample = {k: parts[k][pick].cpu().numpy() for k in F8}
+    del parts
+    wl["particles"] = None
+    torch.cuda.empty_cache()
+    before = dev.get_particles(n)
+    slab_of = lambda c: torch.repeat_interleave(torch.arange(nP, device="cuda"), c)
+    prev_slab = torch.empty(n, dtype=torch.int32, device="cuda")
+    prev_pos = torch.empty(n, dtype=torch.int64, device="cuda")
+    prev_slab[before["id"]] = slab_of(before["counts"]).to(torch.int32)
+    prev_pos[before["id"]] = torch.arange(n, device="cuda")
+    del before
+    torch.cuda.empty_cache()
+    dev.step_fused(cfg["dt"])
+    e, n_tot, n_mig = dev.get_status()
+    m = cfg["target_m"]
+    assert e == 0 and n_tot == n and 0.6 * m * n < n_mig < 1.4 * m * n
+    after = dev.get_particles(n)
+    # conservation of count and of the id multiset
+    assert int(after["counts"].sum()) == n
+    seen = torch.zeros(n, dtype=torch.bool, device="cuda")
+    seen[after["id"]] = True
+    assert bool(seen.all())
+    del seen
+    # containment: every particle sits in the slab of the subdomain that contains its position
+    inv_dx = N / L
+    cell = lambda a: torch.clamp(torch.floor(a * inv_dx).to(torch.int32), 0, N - 1)
+    owner = cell(after["x"]) // (N // P[0])
+    owner += P[0] * (cell(after["y"]) // (N // P[1]))
+    owner += P[0] * P[1] * (cell(after["z"]) // (N // P[2]))
+    cur_slab = slab_of(after["counts"]).to(torch.int32)
+    assert torch.equal(owner, cur_slab)
+    del owner
+    # order: stayers first in original order, then incoming by (source slab, source slot)
+    ps, pp = prev_slab[after["id"]], prev_pos[after["id"]]
+    del prev_slab, prev_pos
+    stay = ps == cur_slab
+    assert int(stay.sum()) == n - n_mig
+    key = torch.where(stay, torch.full_like(pp, -1), ps.to(torch.int64)) * (2 * n) + pp   # (is_migrant, source, source slot)
+    del ps, pp, stay
+    same = cur_slab[1:] == cur_slab[:-1]
+    assert bool(torch.all(key[1:][same] > key[:-1][same]))
+    del key, same, cur_slab
+    torch.cuda.empty_cache()
+    # a sample recomputed one by one by the oracle (push only: positions, velocities)
     o = oracle_lib.Oracle(N, *P, 4096, g=cfg["g"])
     o.set_fluid(*(wl[k].cpu().numpy() for k in "uvw"))
     assert o.set_particles(*(sample[k] for k in F8)) == 0
@@ -412,5 +429,5 @@ def test_large_full_size_properties(torch_cuda, oracle_lib):
     where[after["id"]] = torch.arange(n, device="cuda")
     idx = where[torch.from_numpy(want["id"]).cuda()]
     got = {k: after[k][idx].cpu().numpy() for k in F7}
-    assert_state_close(got, {k: want[k] for k in F7}, "Large sample")
+    assert_state_close(got, {k: want[k] for k in F7}, f"{name} sample")
     o.close(); dev.close()
