@@ -130,7 +130,7 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
         k_tile_pass<false><<<h->grid_pack, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch);
     if (rec) cudaEventRecord(ev[1], h->stream);
     k_code_scan<<<G.P, 256, 0, h->stream>>>(G, h->T);
-    k_table<<<1, 256, 0, h->stream>>>(G, h->T);
+    k_table<<<(G.P + 7) / 8, 256, 0, h->stream>>>(G, h->T);
     if (rec) cudaEventRecord(ev[2], h->stream);
     k_unpack<<<dim3((G.groups_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, h->S, h->Snd, h->T);
     k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, 1);

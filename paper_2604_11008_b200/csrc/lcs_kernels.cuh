@@ -32,7 +32,10 @@ constexpr int kTile = 32 * kRows;            // particles per tile
 constexpr int kStay = 13;
 constexpr int kNC = 27;                      // destination codes
 constexpr int kInvalid = 31;                 // code of a lane beyond the slab's count
-constexpr int kGroup = 8;                    // tiles per unpack warp
+#ifndef LCS_GROUP
+#define LCS_GROUP 8
+#endif
+constexpr int kGroup = LCS_GROUP;            // tiles per unpack warp
 
 // Look-back descriptor word: [ epoch:30 | valid:2 | value:32 ]
 
@@ -959,6 +962,7 @@ k_code_scan(Geom G, Tables T)
         for (int t = g * kGroup; t < te; ++t) run += T.tile_cnt[(row0 + t) * 32 + lane];
     }
     if (warp == 0) T.cnt[s * 32 + lane] = total;
+    if (s == 0 && threadIdx.x == 0) { *T.n_migrated = 0ull; *T.n_total = 0ull; }   // k_table accumulates them
 }
 
 // compact tile prefix: tile_start[s] = sum_{s' < s} ceil(count[s'] / kTile); one CTA
@@ -1000,48 +1004,39 @@ k_tile_index(Geom G, Tables T, int commit)
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_table(Geom G, Tables T)
-{
-    __shared__ unsigned long long s_mig, s_tot;
-    if (threadIdx.x == 0) { s_mig = 0; s_tot = 0; }
-    __syncthreads();
-    unsigned long long my_mig = 0, my_tot = 0;
-    for (int r = threadIdx.x; r < G.P; r += blockDim.x) {
-        // the 26 incoming segments (s_c, c): s_c is the neighbour of r in direction -d(c)
-        int src[kNC];
-        uint32_t len[kNC];
+{   // one WARP per receiver r; lane c owns the incoming segment (s_c, c), s_c = the neighbour of r in direction -d(c)
+    const int lane = threadIdx.x & 31;
+    const int r = blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (r >= G.P) return;
+    const bool seg = lane < kNC && lane != kStay;
+    int src = 0x7fffffff;
+    uint32_t len = 0;
+    if (seg) {
         const int rx = r % G.Px, ry = (r / G.Px) % G.Py, rz = r / (G.Px * G.Py);
-        for (int c = 0; c < kNC; ++c) {
-            const int dx = c % 3 - 1, dy = (c / 3) % 3 - 1, dz = c / 9 - 1;
-            const int sx = (rx - dx + G.Px) % G.Px, sy = (ry - dy + G.Py) % G.Py, sz = (rz - dz + G.Pz) % G.Pz;
-            const int sc = sx + G.Px * (sy + G.Py * sz);
-            src[c] = sc;
-            len[c] = (T.count[sc] == 0) ? 0u : T.cnt[sc * 32 + c];
-        }
-        const uint32_t stay = (T.count[r] == 0) ? 0u : T.cnt[r * 32 + kStay];
-        // fixed order: s ascending, then c ascending (DESIGN R-12).  Rank of (src[c], c) among the 26.
-        unsigned long long fill = stay;
-        uint32_t off[kNC];
-        for (int c = 0; c < kNC; ++c) {
-            if (c == kStay) { off[c] = 0; continue; }
-            unsigned long long before = stay;
-            for (int c2 = 0; c2 < kNC; ++c2) {
-                if (c2 == kStay) continue;
-                if (src[c2] < src[c] || (src[c2] == src[c] && c2 < c)) before += len[c2];
-            }
-            off[c] = (uint32_t)min(before, (unsigned long long)0xffffffffu);
-            fill += len[c];
-            my_mig += len[c];
-        }
-        if (fill > (unsigned long long)G.cap) { raise(T.status, -4); fill = (unsigned long long)G.cap; }
-        for (int c = 0; c < kNC; ++c)
-            if (c != kStay) T.recv_off[src[c] * 32 + c] = off[c];
-        T.new_count[r] = (uint32_t)fill;
-        my_tot += fill;
+        const int dx = lane % 3 - 1, dy = (lane / 3) % 3 - 1, dz = lane / 9 - 1;
+        const int sx = (rx - dx + G.Px) % G.Px, sy = (ry - dy + G.Py) % G.Py, sz = (rz - dz + G.Pz) % G.Pz;
+        src = sx + G.Px * (sy + G.Py * sz);
+        len = (T.count[src] == 0) ? 0u : T.cnt[src * 32 + lane];
     }
-    atomicAdd(&s_mig, my_mig);
-    atomicAdd(&s_tot, my_tot);
-    __syncthreads();
-    if (threadIdx.x == 0) { *T.n_migrated = s_mig; *T.n_total = s_tot; }
+    const uint32_t stay = (T.count[r] == 0) ? 0u : T.cnt[r * 32 + kStay];
+    // fixed order: s ascending, then c ascending (DESIGN R-12): offset of segment c = stay + the segments before it
+    unsigned long long before = stay;
+#pragma unroll
+    for (int c2 = 0; c2 < kNC; ++c2) {
+        if (c2 == kStay) continue;
+        const int s2 = __shfl_sync(0xffffffffu, src, c2);
+        const uint32_t l2 = __shfl_sync(0xffffffffu, len, c2);
+        if (s2 < src || (s2 == src && c2 < lane)) before += l2;
+    }
+    const uint32_t mig = __reduce_add_sync(0xffffffffu, seg ? len : 0u);      // <= 26 * cap < 2^32 (cap < 2^27 is far off)
+    unsigned long long fill = (unsigned long long)stay + mig;
+    if (seg) T.recv_off[src * 32 + lane] = (uint32_t)min(before, (unsigned long long)0xffffffffu);
+    if (lane == 0) {
+        if (fill > (unsigned long long)G.cap) { raise(T.status, -4); fill = (unsigned long long)G.cap; }
+        T.new_count[r] = (uint32_t)fill;
+        atomicAdd(T.n_migrated, (unsigned long long)mig);
+        atomicAdd(T.n_total, fill);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1049,7 +1044,10 @@ k_table(Geom G, Tables T)
 // lane c owns code c: it carries the exclusive prefix of its code and copies its run of every
 // tile chunk to slab[receiver(s,c)] + recv_off[s][c] + prefix.
 // ---------------------------------------------------------------------------------------------
-constexpr int kUnpackWarps = 2;
+#ifndef LCS_UNPACK_WARPS
+#define LCS_UNPACK_WARPS 2
+#endif
+constexpr int kUnpackWarps = LCS_UNPACK_WARPS;
 
 __global__ void __launch_bounds__(32 * kUnpackWarps)
 k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
