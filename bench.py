@@ -257,6 +257,40 @@ def run_cuda(args):
     value = world * n * args.steps / (ms_total * 1e-3)
     m = n_mig / n
 
+    # ---- push and migrate separately (north_star: "for push and migrate separately and together") ---
+    # the unfused pair lcs_particle_step + lcs_migrate gives the same result as lcs_step_fused; timed on rank 0's
+    # stream with CUDA events, continuing from the state the fused steps left
+    phases = None
+    if args.phase_steps > 0:
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.phase_steps)]
+        for k in range(args.phase_steps):
+            ev[k][0].record(); lcs.particle_step(dt)
+            ev[k][1].record(); lcs.migrate()
+            ev[k][2].record()
+        torch.cuda.synchronize()
+        err_u, n_tot_u, n_mig_u = lcs.get_status()
+        if (err_u or n_tot_u != n) and not os.environ.get("LCS_BENCH_ABLATION"):
+            print(f"bench.py: unfused step failed: sticky status {err_u}, total {n_tot_u}", file=sys.stderr)
+            return 3
+        push_ms = float(np.median([e[0].elapsed_time(e[1]) for e in ev]))
+        mig_ms = float(np.median([e[1].elapsed_time(e[2]) for e in ev]))
+        m_u = n_mig_u / n
+        peak_p, _ = measured_peak_hbm()
+        push_bytes = 105.0 * n + 24.0 * N ** 3            # R 56 + W 48 + 1 code byte per particle + the grid once
+        mig_bytes = n * (129.0 + 128.0 * m_u)             # code byte + stayers R/W 64 + migrants' second hop
+        phases = {
+            "steps": args.phase_steps, "timing": "median of per-call CUDA-event times",
+            "push": {"call": "lcs_particle_step", "ms": push_ms, "particles_per_s": n / (push_ms * 1e-3),
+                     "algorithmic_GBps": push_bytes / (push_ms * 1e-3) / 1e9,
+                     "frac_of_measured_peak": push_bytes / (push_ms * 1e-3) / 1e9 / peak_p},
+            "migrate": {"call": "lcs_migrate", "ms": mig_ms, "particles_per_s": n / (mig_ms * 1e-3),
+                        "algorithmic_GBps": mig_bytes / (mig_ms * 1e-3) / 1e9,
+                        "frac_of_measured_peak": mig_bytes / (mig_ms * 1e-3) / 1e9 / peak_p,
+                        "migrant_fraction": m_u},
+            "fused": {"call": "lcs_step_fused", "ms": ms_total / args.steps,
+                      "particles_per_s": n / (ms_total / args.steps * 1e-3)},
+        }
+
     # ---- end to end through the host-buffer entry point (rank-local, then max over ranks) ----------
     e2e = None
     if args.e2e_steps > 0:
@@ -330,7 +364,8 @@ def run_cuda(args):
         "config": {"workload": cfg["name"], "N": N, "P": cfg["P"], "particles_per_gpu": n, "capacity": cfg["capacity"],
                    "dt": dt, "migrant_fraction_last_step": m, "l2": "inputs larger than L2 (no flush)",
                    "parallelism": "independent box per GPU" if world > 1 else "single GPU"},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "phases": phases,
+        "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -346,6 +381,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="Large")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--phase-steps", type=int, default=5, help="unfused steps timed for the push / migrate split (0 = skip)")
     ap.add_argument("--cpu-sample", type=int, default=1 << 22, help="particles in the oracle's timed sample (0 = skip)")
     ap.add_argument("--ref-sample", type=int, default=1 << 21, help="--impl reference: particles per timed step")
     ap.add_argument("--traffic-bytes", type=float, default=None,
