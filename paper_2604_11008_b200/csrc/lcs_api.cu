@@ -31,6 +31,7 @@ struct lcs_handle {
     std::vector<cudaEvent_t>* prof;   // 4 events per recorded step, or null
     int prof_steps, prof_max;
     int grid_fused, grid_pack;         // persistent grid sizes of the tile pass
+    CUtensorMap slab_map;              // 2-D view [8 fields][P*cap slots] of the slabs, box 8 x kTile (bulk tile loads)
     size_t gacc_bytes;
 };
 
@@ -124,10 +125,12 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
     if (rec) cudaEventRecord(ev[0], h->stream);
     const size_t smem = tile_pass_smem(G.P);
     cudaMemsetAsync(h->T.gacc, 0, h->gacc_bytes, h->stream);
-    if (fused)
-        k_tile_pass<true><<<h->grid_fused, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch);
-    else
-        k_tile_pass<false><<<h->grid_pack, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch);
+    const bool big = G.P > kTableSmemMax;
+#define LCS_LAUNCH_TP(F, B, GRID) \
+    k_tile_pass<F, B><<<GRID, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch, h->slab_map)
+    if (fused) { if (big) LCS_LAUNCH_TP(true, true, h->grid_fused); else LCS_LAUNCH_TP(true, false, h->grid_fused); }
+    else       { if (big) LCS_LAUNCH_TP(false, true, h->grid_pack); else LCS_LAUNCH_TP(false, false, h->grid_pack); }
+#undef LCS_LAUNCH_TP
     if (rec) cudaEventRecord(ev[1], h->stream);
     k_code_scan<<<G.P, 256, 0, h->stream>>>(G, h->T);
     k_table<<<(G.P + 7) / 8, 256, 0, h->stream>>>(G, h->T);
@@ -203,15 +206,37 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     h->T.n_total = reinterpret_cast<unsigned long long*>(w + L.misc + 48);
     h->prefix = reinterpret_cast<int64_t*>(w + L.prefix);
     h->stream = static_cast<cudaStream_t>(cuda_stream);
+    {   // tensor map of the slabs for the bulk tile loads: 2-D [8 fields][P*cap slots] of 8-byte words, rows `stride` apart
+        typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                      const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                      CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) { delete h; return LCS_ERR_CUDA; }
+        const cuuint64_t gdim[2] = {(cuuint64_t)P * (cuuint64_t)capacity, 8};
+        const cuuint64_t gstride[1] = {(cuuint64_t)(L.slab_f[1] - L.slab_f[0])};
+        const cuuint32_t box[2] = {(cuuint32_t)kTile, 8};
+        const cuuint32_t estr[2] = {1, 1};
+        if (reinterpret_cast<encode_fn>(fn)(&h->slab_map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, w + L.slab_f[0], gdim, gstride, box, estr,
+                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { delete h; return LCS_ERR_CUDA; }
+    }
     {   // persistent grids: one wave of resident CTAs
         int dev = 0, sms = 0, occ_f = 0, occ_p = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         const size_t smem = tile_pass_smem(G.P);
-        cudaFuncSetAttribute(k_tile_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaFuncSetAttribute(k_tile_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_tile_pass<true>, kBlock, smem);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, k_tile_pass<false>, kBlock, smem);
+        if (G.P > kTableSmemMax) {
+            cudaFuncSetAttribute(k_tile_pass<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaFuncSetAttribute(k_tile_pass<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_tile_pass<true, true>, kBlock, smem);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, k_tile_pass<false, true>, kBlock, smem);
+        } else {
+            cudaFuncSetAttribute(k_tile_pass<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaFuncSetAttribute(k_tile_pass<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_tile_pass<true, false>, kBlock, smem);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, k_tile_pass<false, false>, kBlock, smem);
+        }
         if (sms < 1) sms = 148;
         const long long max_tiles = ((long long)G.P * G.tiles_per_sub + kWarps - 1) / kWarps;
         h->grid_fused = (int)std::min<long long>(max_tiles, (long long)sms * (occ_f > 0 ? occ_f : 1));

@@ -10,6 +10,7 @@
 // barrier): the 24 resident warps of an SM drift apart in phase, so the DRAM stream, the L2
 // gather, the fp64 arithmetic, the look-back and the write-out of different tiles overlap.
 #pragma once
+#include <cuda.h>            // CUtensorMap (the type only; the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -466,6 +467,11 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+__device__ __forceinline__ void bulk_tensor2d_g2s(uint32_t dst, const CUtensorMap* tmap, uint32_t c0, uint32_t c1, uint32_t bar)
+{   // one box of the 2-D tensor (here: 8 field rows x kTile slots) into shared memory
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     asm volatile("{\n"
@@ -630,9 +636,10 @@ __device__ __forceinline__ uint32_t pack_xyz(const Geom& G, int s)
 
 struct TileRef { int s, t; uint32_t cnt; bool ok; };     // a ticketed tile: subdomain, tile index, count[s]
 
-template <bool kFused>
+template <bool kFused, bool kBig>
 __global__ void __launch_bounds__(kBlock, kMinBlocks)
-k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch)
+k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch,
+            const __grid_constant__ CUtensorMap slab_map)
 {
     extern __shared__ __align__(128) unsigned char s_raw[];
     TileBuf* bufs = reinterpret_cast<TileBuf*>(s_raw);                                      // [kWarps][kNBuf]
@@ -640,7 +647,7 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
     uint32_t* s_ts = reinterpret_cast<uint32_t*>(s_bar + kWarps * kNBuf);                   // [P+1] if it fits
     uint32_t* s_xyz = s_ts + (G.P + 1);                                                     // [P]   if it fits
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const bool big = G.P > kTableSmemMax;
+    constexpr bool big = kBig;                             // P > kTableSmemMax: tables stay in global memory
     if (!big) {
         for (int i = threadIdx.x; i <= G.P; i += kBlock) {
             s_ts[i] = T.tile_start[i];
@@ -661,7 +668,6 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
     const unsigned int n_active = ts(G.P);
     const uint64_t tag = ((uint64_t)(epoch << 2) << 32) | (1ull << 32);
     const uint32_t cap32 = (uint32_t)G.cap;
-    const size_t fstride = reinterpret_cast<const char*>(S.f[1]) - reinterpret_cast<const char*>(S.f[0]);   // bytes; id = field 7
     int s_hint = 0;
     uint32_t phase = 0;                                    // bit b: parity of the next completion of buffer b's mbarrier
 
@@ -693,17 +699,16 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
         }
     };
     auto take = [&](TileRef& R) { take_finish(R, take_issue()); };
-    // bulk copy of the 8 field runs of tile R into buffer b (one lane issues; completion on the buffer's mbarrier)
+    // bulk copy of the 8 field runs of tile R into buffer b: ONE tensor copy (box = 8 fields x kTile slots of the 2-D
+    // view [field][slot] of the slabs; slots past the end of the last slab are zero-filled by the copy engine);
+    // one lane issues, completion on the buffer's mbarrier
     auto issue_load = [&](const TileRef& R, int b) {
         fence_proxy_async();                               // this warp's earlier accesses to the buffer come first
         __syncwarp();
         if (lane == 0) {
             const uint32_t bar = bar0 + 8u * b;
             mbar_expect_tx(bar, 8u * kTile * 8u);
-            const char* src = reinterpret_cast<const char*>(S.f[0]) + ((size_t)R.s * (size_t)G.cap + (size_t)R.t * kTile) * 8u;
-            const uint32_t dst = smem_u32(&my[b].f[0][0]);
-#pragma unroll
-            for (int a = 0; a < 8; ++a) bulk_g2s(dst + a * (kTile * 8u), src + a * fstride, kTile * 8u, bar);
+            bulk_tensor2d_g2s(smem_u32(&my[b].f[0][0]), &slab_map, (uint32_t)R.s * cap32 + (uint32_t)R.t * kTile, 0u, bar);
         }
     };
     auto wait_buf = [&](int b) {
