@@ -910,14 +910,14 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             if (pend.n_mig) {
                 const bool fits = (long long)excl_mig + (long long)pend.n_mig <= G.send_cap;
                 if (!fits && lane == 0) raise(T.status, -4);
-                const size_t sendbase = (size_t)s * (size_t)G.send_cap + excl_mig;
+                const uint32_t sendbase = (uint32_t)s * (uint32_t)G.send_cap + excl_mig;      // P*send_cap <= P*cap < 2^32
                 for (uint32_t a0 = 0; a0 < pend.n_mig; a0 += 32) {
                     const uint32_t a = a0 + lane;
                     const bool ok = a < pend.n_mig;
                     const uint32_t e = ok ? W.mlist[a] : 0u;
                     const uint32_t off = __shfl_sync(0xffffffffu, pend.run_start, (e >> 8) & 31u) + (e >> 16);
                     if (ok && fits) {
-                        const size_t dst = sendbase + off;
+                        const uint32_t dst = sendbase + off;
                         const uint32_t src = e & 0xffu;
 #pragma unroll
                         for (int q = 0; q < 7; ++q) st_stream(Snd.f[q] + dst, W.f[q][src]);
