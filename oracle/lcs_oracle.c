@@ -16,6 +16,8 @@
  *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"):
  *   orc_exp_neg            libm exp within 2 ulp; exact at z=0; monotone
+ *   orc_pow_0687           libm pow within 2e-14 relative; exact at R = 0 and R = 1; monotone
+ *   orc_push (drag_model 1) one-step closed form with frozen f; settling speed w f(w) = tau g; Stokes limit
  *   orc_cell / orc_owner   face coordinates and nextafter neighbours; interval brute force
  *   orc_interp             constant / nodal / tri-affine closed forms; O(dx^2) convergence; seam
  *   orc_push (advance)     closed-form drag relaxation V(t), X(t) under constant U and g
@@ -38,6 +40,8 @@ typedef struct orc {
     int N, Px, Py, Pz, P, nx, ny, nz;
     int64_t cap;
     double L, inv_dx, K_tau, L_below, g[3];
+    double inv_nu;                      /* 1 / nu, computed once (rule R6) */
+    int drag_model;                     /* 0 = Stokes (f = 1); 1 = f = 1 + 0.15 Re_p^0.687, R-23 */
     const double *u, *v, *w;            /* borrowed, N^3 each, x fastest */
     double *f[7];                       /* x y z vx vy vz d : P*cap each (SoA) */
     int64_t *id;                        /* P*cap */
@@ -50,21 +54,60 @@ typedef struct orc {
     int64_t n_migrated_last;
 } orc_t;
 
-/* ---- exp(-z), z >= 0.  DESIGN.md R-3 (specified so two independent implementations agree). ---- */
-double orc_exp_neg(double z)
+/* ---- exp(y) for |y| <= 708: the specified evaluation of DESIGN.md R-3 (range reduction by ln2 hi/lo, degree-14
+ * Taylor polynomial in Horner form with fma, exact scaling).  Shared by exp(-z) and by the power of R-23. ---- */
+static double exp_spec(double y)
 {
     static const double inv_fact[15] = {
         1.0, 1.0, 1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0,
         1.0 / 40320.0, 1.0 / 362880.0, 1.0 / 3628800.0, 1.0 / 39916800.0, 1.0 / 479001600.0,
         1.0 / 6227020800.0, 1.0 / 87178291200.0 };
-    if (!(z <= 708.0)) return (z != z) ? z : 0.0;   /* z > 708 -> 0 ; NaN propagates */
-    double y = -z;
     double k = rint(y * 1.4426950408889634);        /* round to nearest even */
     double r = fma(-k, 6.93147180369123816490e-01, y);
     r = fma(-k, 1.90821492927058770002e-10, r);
     double p = inv_fact[14];
     for (int j = 13; j >= 0; --j) p = fma(p, r, inv_fact[j]);
     return ldexp(p, (int)k);
+}
+
+/* ---- exp(-z), z >= 0.  DESIGN.md R-3 (specified so two independent implementations agree). ---- */
+double orc_exp_neg(double z)
+{
+    if (!(z <= 708.0)) return (z != z) ? z : 0.0;   /* z > 708 -> 0 ; NaN propagates */
+    return exp_spec(-z);
+}
+
+/* ---- R^0.687 for the drag factor of PAPER.md:59 (Eq. 7), R-23: exp(0.687 ln R) with the logarithm
+ * specified too.  R below the smallest normal number (in particular R = 0: no slip) gives 0, so f = 1. ---- */
+double orc_pow_0687(double R)
+{
+    static const double inv_odd[11] = {             /* 1/(2k+1), k = 0..10: atanh series of ln m */
+        1.0, 1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0, 1.0 / 15.0, 1.0 / 17.0,
+        1.0 / 19.0, 1.0 / 21.0 };
+    if (!(R >= 2.2250738585072014e-308)) return (R != R) ? R : 0.0;
+    if (R > 1.7976931348623157e308) return R;       /* +inf */
+    int e;
+    double m = 2.0 * frexp(R, &e);                  /* R = m 2^(e-1), m in [1, 2) */
+    e -= 1;
+    if (m > 1.4142135623730951) { m = 0.5 * m; e += 1; }   /* m in (sqrt(1/2), sqrt(2)] */
+    double s = (m - 1.0) / (m + 1.0);
+    double t = s * s;
+    double q = inv_odd[10];
+    for (int k = 9; k >= 0; --k) q = fma(q, t, inv_odd[k]);
+    double lm = (2.0 * s) * q;                      /* ln m = 2 atanh(s) */
+    double ed = (double)e;
+    double lnR = fma(ed, 6.93147180369123816490e-01, fma(ed, 1.90821492927058770002e-10, lm));
+    return exp_spec(0.687 * lnR);
+}
+
+/* drag factor f(Re_p) = 1 + 0.15 Re_p^0.687 (Eq. 7), Re_p = d |V - U| / nu (Eq. 8 with 2r = d) */
+double orc_drag_factor(const orc_t *o, double d, double dvx, double dvy, double dvz)
+{
+    if (o->drag_model == 0) return 1.0;
+    double s2 = fma(dvz, dvz, fma(dvy, dvy, dvx * dvx));
+    double w = sqrt(s2);
+    double Re = (d * w) * o->inv_nu;
+    return fma(0.15, orc_pow_0687(Re), 1.0);
 }
 
 /* ---- geometry ---- */
@@ -158,6 +201,8 @@ orc_t *orc_create(int N, int Px, int Py, int Pz, int64_t cap, double nu, double 
     o->L = 6.283185307179586;                       /* 2*pi*L0, L0 = 1 */
     o->inv_dx = (double)N / o->L;
     o->K_tau = rho_ratio / (18.0 * nu);
+    o->inv_nu = 1.0 / nu;
+    o->drag_model = 0;
     o->L_below = nextafter(o->L, 0.0);
     o->g[0] = g[0]; o->g[1] = g[1]; o->g[2] = g[2];
     size_t slots = (size_t)o->P * (size_t)cap;
@@ -172,6 +217,13 @@ orc_t *orc_create(int N, int Px, int Py, int Pz, int64_t cap, double nu, double 
     if (!ok) { /* leak on this path is acceptable for test infrastructure */ return NULL; }
     memset(o->code, ORC_STAY, slots);
     return o;
+}
+
+int orc_set_drag_model(orc_t *o, int model)
+{
+    if (model != 0 && model != 1) return ORC_ERR_ARG;
+    o->drag_model = model;
+    return ORC_OK;
 }
 
 void orc_destroy(orc_t *o)
@@ -263,6 +315,8 @@ int orc_push(orc_t *o, double dt)
             /* a2 advance: exact solution of dV/dt = -(V-U)/tau + g, dX/dt = V with U frozen */
             double d = o->f[6][slot];
             double tau = (o->K_tau * d) * d;
+            if (o->drag_model == 1)                            /* f frozen at the start of the step, tau_eff = tau_p / f */
+                tau = tau / orc_drag_factor(o, d, o->f[3][slot] - U[0], o->f[4][slot] - U[1], o->f[5][slot] - U[2]);
             double zz = dt / tau;
             double alpha = orc_exp_neg(zz);
             double b = tau * (1.0 - alpha);

@@ -42,6 +42,9 @@ def lib():
         L = C.CDLL(build())
         L.orc_exp_neg.restype = C.c_double
         L.orc_exp_neg.argtypes = [C.c_double]
+        L.orc_pow_0687.restype = C.c_double
+        L.orc_pow_0687.argtypes = [C.c_double]
+        L.orc_set_drag_model.argtypes = [C.c_void_p, C.c_int]
         L.orc_create.restype = C.c_void_p
         L.orc_create.argtypes = [C.c_int] * 4 + [C.c_int64, C.c_double, C.c_double, _dp]
         L.orc_destroy.argtypes = [C.c_void_p]
@@ -93,19 +96,26 @@ def exp_neg(z: float) -> float:
     return lib().orc_exp_neg(float(z))
 
 
+def pow_0687(R: float) -> float:
+    """R^0.687 as specified in DESIGN.md R-23 (the drag factor of PAPER.md:59 is 1 + 0.15 * this)."""
+    return lib().orc_pow_0687(float(R))
+
+
 FIELDS = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
 
 
 class Oracle:
     """One periodic box [0, 2*pi)^3 with an N^3 fluid grid and Px*Py*Pz virtual subdomains."""
 
-    def __init__(self, N, Px, Py, Pz, capacity, nu=1.5e-5, rho_ratio=1000.0, g=(0.0, 0.0, 0.0)):
+    def __init__(self, N, Px, Py, Pz, capacity, nu=1.5e-5, rho_ratio=1000.0, g=(0.0, 0.0, 0.0), drag_model=0):
         self.N, self.Px, self.Py, self.Pz, self.cap = N, Px, Py, Pz, int(capacity)
         self.P = Px * Py * Pz
         gv = (C.c_double * 3)(*g)
         self._h = lib().orc_create(N, Px, Py, Pz, int(capacity), float(nu), float(rho_ratio), gv)
         if not self._h:
             raise ValueError("orc_create: invalid arguments")
+        if lib().orc_set_drag_model(self._h, int(drag_model)):
+            raise ValueError("drag_model must be 0 (Stokes) or 1 (1 + 0.15 Re^0.687)")
         self._fluid = None
 
     def close(self):
