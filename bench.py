@@ -216,7 +216,7 @@ def run_cuda(args):
     cfg, wl = build_workload(args.workload, dev)
     n, N = cfg["n"], cfg["N"]
     P = cfg["P"][0] * cfg["P"][1] * cfg["P"][2]
-    lcs = LCS(N, *cfg["P"], cfg["capacity"], g=cfg["g"], device=dev)
+    lcs = LCS(N, *cfg["P"], cfg["capacity"], g=cfg["g"], drag_model=args.drag_model, device=dev)
     lcs.set_fluid(wl["u"], wl["v"], wl["w"])
     parts = wl["particles"]
     lcs.set_particles(*(parts[k] for k in F8))
@@ -362,7 +362,8 @@ def run_cuda(args):
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg["name"], "N": N, "P": cfg["P"], "particles_per_gpu": n, "capacity": cfg["capacity"],
-                   "dt": dt, "migrant_fraction_last_step": m, "l2": "inputs larger than L2 (no flush)",
+                   "dt": dt, "migrant_fraction_last_step": m, "drag_model": args.drag_model,
+                   "l2": "inputs larger than L2 (no flush)",
                    "parallelism": "independent box per GPU" if world > 1 else "single GPU"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "phases": phases,
         "cpu_baseline": cpu,
@@ -384,6 +385,8 @@ def main():
     ap.add_argument("--phase-steps", type=int, default=5, help="unfused steps timed for the push / migrate split (0 = skip)")
     ap.add_argument("--cpu-sample", type=int, default=1 << 22, help="particles in the oracle's timed sample (0 = skip)")
     ap.add_argument("--ref-sample", type=int, default=1 << 21, help="--impl reference: particles per timed step")
+    ap.add_argument("--drag-model", type=int, default=0, choices=[0, 1],
+                    help="0: Stokes drag (BASELINE.json's configs); 1: f = 1 + 0.15 Re^0.687 (SURVEY 8(f) NEXT #2)")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), reported as roofline.traffic")
     args = ap.parse_args()

@@ -53,6 +53,9 @@ typedef struct {
     double  rho_ratio;      /* rho_p / rho: 843 in PAPER.md:57, 1000 in BASELINE.json's configs     */
     double  g[3];           /* gravity; (0,0,0) reproduces Eq. 6, DESIGN R-4          */
     int64_t send_capacity;  /* migrant slots per subdomain send region; 0 = capacity (never full)  */
+    int32_t drag_model;     /* 0: Stokes drag, f = 1 (the hot path of BASELINE.json's configs);
+                               1: f = 1 + 0.15 Re_p^0.687, Re_p = d|V-U|/nu (Eq. 7-8),
+                                  frozen at the start of the step, tau_eff = tau_p / f (DESIGN R-23)  */
 } lcs_params;
 
 /* Bytes of device workspace lcs_create needs; 0 if the arguments are invalid. */

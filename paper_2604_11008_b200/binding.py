@@ -25,7 +25,7 @@ class LcsError(RuntimeError):
 
 class LcsParams(C.Structure):
     _fields_ = [("nu", C.c_double), ("rho_ratio", C.c_double), ("g", C.c_double * 3),
-                ("send_capacity", C.c_int64)]
+                ("send_capacity", C.c_int64), ("drag_model", C.c_int32)]
 
 
 def lib_path() -> str:
@@ -82,7 +82,7 @@ class LCS:
     Device tensors in, device tensors out; torch allocates, the library computes."""
 
     def __init__(self, N, Px, Py, Pz, capacity, nu=1.5e-5, rho_ratio=1000.0, g=(0.0, 0.0, 0.0),
-                 send_capacity=0, device="cuda:0", stream=None):
+                 send_capacity=0, drag_model=0, device="cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2604_11008_b200 needs a CUDA device (no CPU fallback)")
@@ -91,7 +91,7 @@ class LCS:
         self.device = torch.device(device)
         self.N, self.Px, self.Py, self.Pz, self.capacity = N, Px, Py, Pz, int(capacity)
         self.P = Px * Py * Pz
-        self._prm = LcsParams(nu, rho_ratio, (C.c_double * 3)(*g), int(send_capacity))
+        self._prm = LcsParams(nu, rho_ratio, (C.c_double * 3)(*g), int(send_capacity), int(drag_model))
         nbytes = self._L.lcs_workspace_bytes(N, Px, Py, Pz, int(capacity), C.byref(self._prm))
         if nbytes == 0:
             raise LcsError("lcs_workspace_bytes", LCS_ERR_INVALID_ARG)

@@ -62,6 +62,7 @@ bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* pr
     if ((unsigned long long)P * (unsigned long long)cap >= (1ull << 32)) return false;   // 32-bit slot indices
     if (prm->send_capacity < 0 || (prm->send_capacity & 1) || prm->send_capacity > cap) return false;
     if (!(prm->nu > 0.0) || !(prm->rho_ratio > 0.0)) return false;
+    if (prm->drag_model != 0 && prm->drag_model != 1) return false;
     if (!std::isfinite(prm->g[0]) || !std::isfinite(prm->g[1]) || !std::isfinite(prm->g[2])) return false;
     return true;
 }
@@ -126,10 +127,15 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
     const size_t smem = tile_pass_smem(G.P);
     cudaMemsetAsync(h->T.gacc, 0, h->gacc_bytes, h->stream);
     const bool big = G.P > kTableSmemMax;
-#define LCS_LAUNCH_TP(F, B, GRID) \
-    k_tile_pass<F, B><<<GRID, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch, h->slab_map)
-    if (fused) { if (big) LCS_LAUNCH_TP(true, true, h->grid_fused); else LCS_LAUNCH_TP(true, false, h->grid_fused); }
-    else       { if (big) LCS_LAUNCH_TP(false, true, h->grid_pack); else LCS_LAUNCH_TP(false, false, h->grid_pack); }
+    const bool sn = fused && G.drag_model == 1;            // the unfused pass carries no push: one instantiation
+#define LCS_LAUNCH_TP(F, B, D, GRID) \
+    k_tile_pass<F, B, D><<<GRID, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch, h->slab_map)
+    if (fused) {
+        if (big) { if (sn) LCS_LAUNCH_TP(true, true, 1, h->grid_fused); else LCS_LAUNCH_TP(true, true, 0, h->grid_fused); }
+        else     { if (sn) LCS_LAUNCH_TP(true, false, 1, h->grid_fused); else LCS_LAUNCH_TP(true, false, 0, h->grid_fused); }
+    } else {
+        if (big) LCS_LAUNCH_TP(false, true, 0, h->grid_pack); else LCS_LAUNCH_TP(false, false, 0, h->grid_pack);
+    }
 #undef LCS_LAUNCH_TP
     if (rec) cudaEventRecord(ev[1], h->stream);
     k_code_scan<<<G.P, 256, 0, h->stream>>>(G, h->T);
@@ -179,6 +185,8 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     G.K_tau = prm->rho_ratio / (18.0 * prm->nu);  // tau_p = K_tau * d^2
     G.L_below = std::nextafter(G.L, 0.0);
     G.gx = prm->g[0]; G.gy = prm->g[1]; G.gz = prm->g[2];
+    G.inv_nu = 1.0 / prm->nu;
+    G.drag_model = prm->drag_model;
     char* w = static_cast<char*>(d_workspace);
     const size_t P = (size_t)G.P;
     for (int a = 0; a < 7; ++a) h->S.f[a] = reinterpret_cast<double*>(w + L.slab_f[a]);
@@ -226,16 +234,18 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         const size_t smem = tile_pass_smem(G.P);
+        auto setup = [&](auto kernel, int& occ) {
+            cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            int o = 0;
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kernel, kBlock, smem);
+            occ = occ == 0 ? o : std::min(occ, o);
+        };
         if (G.P > kTableSmemMax) {
-            cudaFuncSetAttribute(k_tile_pass<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            cudaFuncSetAttribute(k_tile_pass<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_tile_pass<true, true>, kBlock, smem);
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, k_tile_pass<false, true>, kBlock, smem);
+            setup(k_tile_pass<true, true, 0>, occ_f); setup(k_tile_pass<true, true, 1>, occ_f);
+            setup(k_tile_pass<false, true, 0>, occ_p);
         } else {
-            cudaFuncSetAttribute(k_tile_pass<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            cudaFuncSetAttribute(k_tile_pass<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_tile_pass<true, false>, kBlock, smem);
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, k_tile_pass<false, false>, kBlock, smem);
+            setup(k_tile_pass<true, false, 0>, occ_f); setup(k_tile_pass<true, false, 1>, occ_f);
+            setup(k_tile_pass<false, false, 0>, occ_p);
         }
         if (sms < 1) sms = 148;
         const long long max_tiles = ((long long)G.P * G.tiles_per_sub + kWarps - 1) / kWarps;

@@ -47,6 +47,8 @@ struct Geom {
     int lbgroups_per_sub;              // ceil(tiles_per_sub / 32): look-back groups
     int64_t cap, send_cap;
     double inv_dx, K_tau, L, L_below, gx, gy, gz;
+    double inv_nu;                     // 1 / nu, for Re_p (drag_model 1)
+    int drag_model;                    // 0 = Stokes, 1 = f = 1 + 0.15 Re_p^0.687 (DESIGN R-23)
 };
 
 struct Slabs {                         // SoA particle storage, P*cap slots each
@@ -118,19 +120,57 @@ __constant__ double kExpC[15] = {1.1470745597729725e-11, 1.6059043836821613e-10,
                                  0.008333333333333333,   0.041666666666666664,   0.16666666666666666,
                                  0.5,                    1.0,                    1.0};
 
-__device__ __forceinline__ double exp_neg(double z)
+__device__ __forceinline__ double exp_core(double y)          // |y| <= 708
 {
-    if (!(z <= 708.0)) return (z != z) ? z : 0.0;
-    const double y = -z;
     const double k = rint(y * 1.4426950408889634);
     double r = fma(-k, 6.93147180369123816490e-01, y);
     r = fma(-k, 1.90821492927058770002e-10, r);
     double p = kExpC[0];                          // 1/14!
 #pragma unroll
     for (int j = 1; j < 15; ++j) p = fma(p, r, kExpC[j]);
-    // 2^k, k in [-1022, 0]: always a normal number, so the product is exact
+    // 2^k, |k| <= 1022: always a normal number, so the product is exact
     const long long bits = (long long)(1023 + (int)k) << 52;
     return p * __longlong_as_double(bits);
+}
+
+__device__ __forceinline__ double exp_neg(double z)
+{
+    if (!(z <= 708.0)) return (z != z) ? z : 0.0;
+    return exp_core(-z);
+}
+
+// R^0.687 of the drag factor f = 1 + 0.15 Re_p^0.687 (Eq. 7), evaluated as DESIGN.md R-23 specifies:
+// R = m 2^e with m in (sqrt(1/2), sqrt(2)], ln m = 2 atanh((m-1)/(m+1)) by an 11-term series in Horner form with fma
+// (coefficients: the correctly rounded 1/(2k+1), k = 10 .. 0), ln R = e ln2 + ln m (hi/lo), then exp_core(0.687 ln R).
+__constant__ double kLnC[11] = {1.0 / 21.0, 1.0 / 19.0, 1.0 / 17.0, 1.0 / 15.0, 1.0 / 13.0, 1.0 / 11.0,
+                                1.0 / 9.0,  1.0 / 7.0,  1.0 / 5.0,  1.0 / 3.0,  1.0};
+
+__device__ __forceinline__ double pow_0687(double R)
+{
+    if (!(R >= 2.2250738585072014e-308)) return (R != R) ? R : 0.0;     // below the smallest normal number: no slip, f = 1
+    if (R > 1.7976931348623157e308) return R;
+    const long long bits = __double_as_longlong(R);
+    int e = (int)(bits >> 52) - 1023;                                     // R = m 2^e, m in [1, 2)
+    double m = __longlong_as_double((bits & 0x000fffffffffffffLL) | 0x3ff0000000000000LL);
+    if (m > 1.4142135623730951) { m = 0.5 * m; e += 1; }
+    const double s = (m - 1.0) / (m + 1.0);
+    const double t = s * s;
+    double q = kLnC[0];
+#pragma unroll
+    for (int j = 1; j < 11; ++j) q = fma(q, t, kLnC[j]);
+    const double lm = (2.0 * s) * q;
+    const double ed = (double)e;
+    const double lnR = fma(ed, 6.93147180369123816490e-01, fma(ed, 1.90821492927058770002e-10, lm));
+    return exp_core(0.687 * lnR);
+}
+
+// f(Re_p), Re_p = d |V - U| / nu (Eq. 7-8 with 2r = d); operation order of DESIGN.md R-23
+__device__ __forceinline__ double drag_factor(double d, double dvx, double dvy, double dvz, double inv_nu)
+{
+    const double s2 = fma(dvz, dvz, fma(dvy, dvy, dvx * dvx));
+    const double w = sqrt(s2);
+    const double Re = (d * w) * inv_nu;
+    return fma(0.15, pow_0687(Re), 1.0);
 }
 
 __device__ __forceinline__ double lerp(double p, double q, double f) { return fma(f, q - p, p); }
@@ -281,7 +321,8 @@ __device__ __forceinline__ int push_particle(Particle& p, const double* __restri
 #else
     const Vec3 U = gather_pair(F4, G.N, G.inv_dx, p.x, p.y, p.z, lane);
 #endif
-    const double tau = (G.K_tau * p.d) * p.d;     // tau_p = (rho_p/rho) d^2 / (18 nu)
+    double tau = (G.K_tau * p.d) * p.d;           // tau_p = (rho_p/rho) d^2 / (18 nu)
+    if (G.drag_model == 1) tau = tau / drag_factor(p.d, p.vx - U.x, p.vy - U.y, p.vz - U.z, G.inv_nu);   // DESIGN R-23
     const double zz = dt / tau;
     const double alpha = exp_neg(zz);
     const double b = tau * (1.0 - alpha);
@@ -553,10 +594,11 @@ __device__ __forceinline__ Vec3 gather_reduce(const Gath& Q, int lane)
 // chain of ~35 fp64 operations; kept apart so that it can be issued under the lerps of the gather.
 struct Drag { double tau, alpha, b; };
 
-__device__ __forceinline__ Drag drag_coeffs(double d, double dt, const Geom& G)
+__device__ __forceinline__ Drag drag_coeffs(double d, double dt, const Geom& G, double f = 1.0, bool nonlinear = false)
 {
     Drag D;
     D.tau = (G.K_tau * d) * d;                    // tau_p = (rho_p/rho) d^2 / (18 nu)
+    if (nonlinear) D.tau = D.tau / f;             // tau_eff = tau_p / f, f frozen at the start of the step (DESIGN R-23)
     const double zz = dt / D.tau;
     D.alpha = exp_neg(zz);
     D.b = D.tau * (1.0 - D.alpha);
@@ -636,7 +678,7 @@ __device__ __forceinline__ uint32_t pack_xyz(const Geom& G, int s)
 
 struct TileRef { int s, t; uint32_t cnt; bool ok; };     // a ticketed tile: subdomain, tile index, count[s]
 
-template <bool kFused, bool kBig>
+template <bool kFused, bool kBig, int kDrag>
 __global__ void __launch_bounds__(kBlock, kMinBlocks)
 k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch,
             const __grid_constant__ CUtensorMap slab_map)
@@ -782,7 +824,7 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 Drag D;
                 D.tau = D.alpha = D.b = 0.0;
                 if (kFused) {
-                    D = drag_coeffs(__longlong_as_double(W.f[6][p]), dt, G);   // serial chain, issued under the lerps
+                    if (kDrag == 0) D = drag_coeffs(__longlong_as_double(W.f[6][p]), dt, G);   // serial chain, issued under the lerps
                     U = gather_reduce(Q, lane);
                 }
                 if (r + 1 == nrows) {
@@ -815,6 +857,10 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     q.z = __longlong_as_double(W.f[2][p]); q.vx = __longlong_as_double(W.f[3][p]);
                     q.vy = __longlong_as_double(W.f[4][p]); q.vz = __longlong_as_double(W.f[5][p]);
                     q.d = 0.0;
+                    if (kDrag == 1) {                                   // f needs the slip V - U(X): after the gather (R-23)
+                        const double dd = __longlong_as_double(W.f[6][p]);
+                        D = drag_coeffs(dd, dt, G, drag_factor(dd, q.vx - U.x, q.vy - U.y, q.vz - U.z, G.inv_nu), true);
+                    }
                     bool jmp = false;
                     code = advance_particle(q, U, D, G, B, dt, jmp);
                     jump |= jmp && valid;

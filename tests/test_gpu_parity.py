@@ -43,12 +43,12 @@ def assert_state_close(got, want, tag=""):
         assert ulps(got[k], want[k]) == 0, (tag, k, "ulp distance", ulps(got[k], want[k]))
 
 
-def make_pair(torch, oracle_lib, N, P, cap, fluid, parts, g=(0.0, 0.0, 0.0), rho=1000.0, send_capacity=0):
+def make_pair(torch, oracle_lib, N, P, cap, fluid, parts, g=(0.0, 0.0, 0.0), rho=1000.0, send_capacity=0, drag_model=0):
     from paper_2604_11008_b200 import LCS
-    o = oracle_lib.Oracle(N, *P, cap, g=g, rho_ratio=rho)
+    o = oracle_lib.Oracle(N, *P, cap, g=g, rho_ratio=rho, drag_model=drag_model)
     o.set_fluid(*fluid)
     rc = o.set_particles(*(parts[k] for k in F8))
-    dev = LCS(N, *P, cap, g=g, rho_ratio=rho, send_capacity=send_capacity)
+    dev = LCS(N, *P, cap, g=g, rho_ratio=rho, send_capacity=send_capacity, drag_model=drag_model)
     df = [torch.from_numpy(np.ascontiguousarray(f, dtype=np.float64)).cuda() for f in fluid]
     dev.set_fluid(*df)
     dp = to_dev(torch, parts)
@@ -175,6 +175,35 @@ def test_many_subdomains_and_long_slabs(torch_cuda, oracle_lib, P, N, per_sub):
         assert dev.get_status() == (0, n, o.n_migrated_last)
         compare_packed(dev, o, f"P={P} step {step}")
     dev.close()
+
+
+@pytest.mark.parametrize("scale_d,P", [(1.0, (2, 2, 2)), (12.0, (2, 2, 2)), (30.0, (1, 2, 3))])
+def test_nonlinear_drag_model_matches_oracle(torch_cuda, oracle_lib, scale_d, P):
+    """drag_model = 1 (f = 1 + 0.15 Re_p^0.687, DESIGN R-23): the Tiny recipe's field with droplets
+    of 10, 120 and 300 um radius (Re_p up to O(10), f up to ~2), gravity on; fused and unfused against the oracle, 0 ulp."""
+    from workloads import gen
+    cfg = gen.scaled_config(gen.get_config("Tiny"), n=20000, N=24)
+    cfg["P"] = list(P)
+    wl = gen.make_workload(cfg)
+    fluid = [wl[k].numpy() for k in "uvw"]
+    parts = {k: v.numpy().copy() for k, v in wl["particles"].items()}
+    parts["d"] = parts["d"] * scale_d
+    g = (0.0, 0.0, -9.81)
+    nP = P[0] * P[1] * P[2]
+    cap = 2 * (int(2.5 * cfg["n"] / nP) // 2)
+    dt = 0.02
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, cfg["N"], P, cap, fluid, parts, g=g, drag_model=1)
+    _, dev2, _ = make_pair(torch_cuda, oracle_lib, cfg["N"], P, cap, fluid, parts, g=g, drag_model=1)
+    assert rc == 0
+    for step in range(4):
+        assert o.step(dt) == 0
+        dev.step_fused(dt)
+        dev2.particle_step(dt)
+        dev2.migrate()
+        assert dev.get_status() == (0, cfg["n"], o.n_migrated_last)
+        compare_packed(dev, o, f"drag fused {step}")
+        compare_packed(dev2, o, f"drag unfused {step}")
+    dev.close(); dev2.close()
 
 
 def test_all_27_codes_hand_placed(torch_cuda, oracle_lib):
