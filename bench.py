@@ -272,6 +272,13 @@ def run_cuda(args):
         if (err_u or n_tot_u != n) and not os.environ.get("LCS_BENCH_ABLATION"):
             print(f"bench.py: unfused step failed: sticky status {err_u}, total {n_tot_u}", file=sys.stderr)
             return 3
+        # per-step fluid refresh (first half): lcs_set_fluid = the repack of the three x-fastest
+        # arrays into the internal (u,v,w,0) z-fastest records, as a coupled solver would call it every step
+        evf = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(3)]
+        for k in range(3):
+            evf[k][0].record(); lcs.set_fluid(wl["u"], wl["v"], wl["w"]); evf[k][1].record()
+        torch.cuda.synchronize()
+        fluid_ms = float(np.median([e[0].elapsed_time(e[1]) for e in evf]))
         push_ms = float(np.median([e[0].elapsed_time(e[1]) for e in ev]))
         mig_ms = float(np.median([e[1].elapsed_time(e[2]) for e in ev]))
         m_u = n_mig_u / n
@@ -287,6 +294,9 @@ def run_cuda(args):
                         "algorithmic_GBps": mig_bytes / (mig_ms * 1e-3) / 1e9,
                         "frac_of_measured_peak": mig_bytes / (mig_ms * 1e-3) / 1e9 / peak_p,
                         "migrant_fraction": m_u},
+            "set_fluid": {"call": "lcs_set_fluid", "ms": fluid_ms,
+                          "GBps": (24.0 + 32.0) * N ** 3 / (fluid_ms * 1e-3) / 1e9,
+                          "note": "reads 24 B and writes 32 B per cell; off the timed step (the fluid is frozen)"},
             "fused": {"call": "lcs_step_fused", "ms": ms_total / args.steps,
                       "particles_per_s": n / (ms_total / args.steps * 1e-3)},
         }
