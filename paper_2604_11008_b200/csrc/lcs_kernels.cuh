@@ -551,6 +551,15 @@ __device__ __forceinline__ void gather_issue(Gath& Q, const double* __restrict__
     const uint32_t a0 = Nu * (uint32_t)i0, a1 = Nu * (uint32_t)i1;
     const uint32_t row[4] = {Nu * (a0 + (uint32_t)j0), Nu * (a1 + (uint32_t)j0), Nu * (a0 + (uint32_t)j1),
                              Nu * (a1 + (uint32_t)j1)};
+#ifdef LCS_X_NOPAIR               // experiment: every lane gathers its own eight corners, no exchange
+    (void)lane;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) Q.a[m] = ld_cell(F4, row[m] + (uint32_t)k0);
+#pragma unroll
+    for (int m = 0; m < 4; ++m) Q.b[m] = ld_cell(F4, row[m] + (uint32_t)k1);
+    Q.fxA = Q.fxB = fx; Q.fyA = Q.fyB = fy;
+    return;
+#endif
     const uint32_t kk = (uint32_t)k0 | ((uint32_t)k1 << 16);          // N <= 1625 fits 16 bits
     const int le = lane & ~1, lo = lane | 1;
     const uint32_t sh = (uint32_t)(lane & 1) << 4;                    // this lane always fetches z-side (lane & 1)
@@ -577,6 +586,13 @@ __device__ __forceinline__ Vec3 gather_reduce(const Gath& Q, int lane)
 {
     const Vec3 pa = side_reduce(Q.a, Q.fxA, Q.fyA);
     const Vec3 pb = side_reduce(Q.b, Q.fxB, Q.fyB);
+#ifdef LCS_X_NOPAIR
+    {
+        Vec3 U0;
+        U0.x = lerp(pa.x, pb.x, Q.fz); U0.y = lerp(pa.y, pb.y, Q.fz); U0.z = lerp(pa.z, pb.z, Q.fz);
+        return U0;
+    }
+#endif
     // the even lane needs A's z1 side (the odd lane's pa); the odd lane needs B's z0 side (the even lane's pb)
     const bool odd = lane & 1;
     Vec3 give, keep;
@@ -811,11 +827,7 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             uint32_t n_mig = 0, n_stay = 0;
             g_early = 0u;
             bool jump = false;
-#ifdef LCS_X_UNROLL_ROWS
-#pragma unroll
-#else
 #pragma unroll 1
-#endif
             for (int r = 0; r < kRows; ++r) {
                 if (r >= nrows) break;
                 const uint32_t p = 32u * (uint32_t)r + (uint32_t)lane;
