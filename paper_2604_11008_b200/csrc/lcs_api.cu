@@ -317,7 +317,7 @@ int lcs_particle_step(lcs_t* h, double dt)
     if (h->sticky) return h->sticky;
     const Geom& G = h->G;
     cudaMemsetAsync(h->T.cnt, 0, (size_t)G.P * 32 * 4, h->stream);
-    k_push<<<dim3((G.tiles_per_sub + kWarps - 1) / kWarps, G.P), kBlock, 0, h->stream>>>(G, h->S, h->T, h->fluid4, dt);
+    k_push<<<dim3((G.tiles_per_sub + kPushWarps - 1) / kPushWarps, G.P), 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->T, h->fluid4, dt);
     h->pushed = true;
     return check_launch(h);
 }

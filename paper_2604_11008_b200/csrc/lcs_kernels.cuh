@@ -226,61 +226,6 @@ __device__ __forceinline__ Vec3 shfl_xor1(const Vec3& v)
     return r;
 }
 
-// x and y lerps of one z-side: corners (i0,j0) (i1,j0) (i0,j1) (i1,j1)
-__device__ __forceinline__ Vec3 side_partial(const double* __restrict__ F4, const uint32_t idx[4], double fx, double fy)
-{
-    const Cell a = ld_cell(F4, idx[0]), b = ld_cell(F4, idx[1]), c = ld_cell(F4, idx[2]), d = ld_cell(F4, idx[3]);
-    Vec3 r;
-    r.x = lerp(lerp(a.u, b.u, fx), lerp(c.u, d.u, fx), fy);
-    r.y = lerp(lerp(a.v, b.v, fx), lerp(c.v, d.v, fx), fy);
-    r.z = lerp(lerp(a.w, b.w, fx), lerp(c.w, d.w, fx), fy);
-    return r;
-}
-
-// Fluid velocity at (x,y,z) of THIS lane's particle; must be called by all 32 lanes (converged).
-// Particle A is the even lane's, particle B the odd lane's.  Both lanes of a pair read A's stencil in
-// the first four loads (even lane: z0 side, odd lane: z1 side) and B's in the next four; the routing
-// is done by the source lane of the index shuffles, so no lane-parity selects are needed.
-__device__ __forceinline__ Vec3 gather_pair(const double* __restrict__ F4, int N, double inv_dx, double x, double y,
-                                            double z, int lane)
-{
-    int i0, i1, j0, j1, k0, k1;
-    double fx, fy, fz;
-    axis_stencil(x, inv_dx, N, i0, i1, fx);
-    axis_stencil(y, inv_dx, N, j0, j1, fy);
-    axis_stencil(z, inv_dx, N, k0, k1, fz);
-    const uint32_t Nu = (uint32_t)N;
-    const uint32_t a0 = Nu * (uint32_t)i0, a1 = Nu * (uint32_t)i1;
-    const uint32_t row[4] = {Nu * (a0 + (uint32_t)j0), Nu * (a1 + (uint32_t)j0), Nu * (a0 + (uint32_t)j1),
-                             Nu * (a1 + (uint32_t)j1)};
-    const uint32_t kk = (uint32_t)k0 | ((uint32_t)k1 << 16);          // N <= 1625 fits 16 bits
-    const int le = lane & ~1, lo = lane | 1;
-    const uint32_t sh = (uint32_t)(lane & 1) << 4;                    // this lane always fetches z-side (lane & 1)
-    const uint32_t kA = (__shfl_sync(0xffffffffu, kk, le) >> sh) & 0xffffu;
-    const uint32_t kB = (__shfl_sync(0xffffffffu, kk, lo) >> sh) & 0xffffu;
-    uint32_t ia[4], ib[4];
-#pragma unroll
-    for (int m = 0; m < 4; ++m) {
-        ia[m] = __shfl_sync(0xffffffffu, row[m], le) + kA;
-        ib[m] = __shfl_sync(0xffffffffu, row[m], lo) + kB;
-    }
-    const double fxA = __shfl_sync(0xffffffffu, fx, le), fyA = __shfl_sync(0xffffffffu, fy, le);
-    const double fxB = __shfl_sync(0xffffffffu, fx, lo), fyB = __shfl_sync(0xffffffffu, fy, lo);
-    const Vec3 pa = side_partial(F4, ia, fxA, fyA);
-    const Vec3 pb = side_partial(F4, ib, fxB, fyB);
-    // the even lane needs A's z1 side (the odd lane's pa); the odd lane needs B's z0 side (the even lane's pb)
-    const bool odd = lane & 1;
-    Vec3 give, keep;
-    give.x = odd ? pa.x : pb.x; give.y = odd ? pa.y : pb.y; give.z = odd ? pa.z : pb.z;
-    keep.x = odd ? pb.x : pa.x; keep.y = odd ? pb.y : pa.y; keep.z = odd ? pb.z : pa.z;
-    const Vec3 got = shfl_xor1(give);
-    Vec3 U;
-    U.x = lerp(odd ? got.x : keep.x, odd ? keep.x : got.x, fz);
-    U.y = lerp(odd ? got.y : keep.y, odd ? keep.y : got.y, fz);
-    U.z = lerp(odd ? got.z : keep.z, odd ? keep.z : got.z, fz);
-    return U;
-}
-
 // ---------------------------------------------------------------------------------------------
 // a2 / a3: advance, wrap, classify
 // ---------------------------------------------------------------------------------------------
@@ -310,27 +255,6 @@ __device__ __forceinline__ void advance_axis(double& a, double& v, double U, dou
     if (rel >= n_a) code += w;
     if (rel < 0) code -= w;
     jump |= !ok || (unsigned)(rel + n_a) >= 3u * (unsigned)n_a;
-}
-
-// a1-a3 for this lane's particle (all 32 lanes must call).  Returns the destination code.
-__device__ __forceinline__ int push_particle(Particle& p, const double* __restrict__ F4, const Geom& G,
-                                             const SubBox& B, double dt, int lane, bool& jump)
-{
-#ifdef LCS_X_NOGATHER
-    Vec3 U; U.x = U.y = U.z = 0.0;
-#else
-    const Vec3 U = gather_pair(F4, G.N, G.inv_dx, p.x, p.y, p.z, lane);
-#endif
-    double tau = (G.K_tau * p.d) * p.d;           // tau_p = (rho_p/rho) d^2 / (18 nu)
-    if (G.drag_model == 1) tau = tau / drag_factor(p.d, p.vx - U.x, p.vy - U.y, p.vz - U.z, G.inv_nu);   // DESIGN R-23
-    const double zz = dt / tau;
-    const double alpha = exp_neg(zz);
-    const double b = tau * (1.0 - alpha);
-    int code = kStay;
-    advance_axis(p.x, p.vx, U.x, G.gx, tau, alpha, b, dt, G, B.lox, G.nx, 1, code, jump);
-    advance_axis(p.y, p.vy, U.y, G.gy, tau, alpha, b, dt, G, B.loy, G.ny, 3, code, jump);
-    advance_axis(p.z, p.vz, U.z, G.gz, tau, alpha, b, dt, G, B.loz, G.nz, 9, code, jump);
-    return code;
 }
 
 __device__ __forceinline__ SubBox sub_box(const Geom& G, int s)
@@ -407,49 +331,6 @@ k_repack_fluid(int N, const double* __restrict__ u, const double* __restrict__ v
             *reinterpret_cast<double4*>(F4 + 4 * dst) = rec;
         }
     }
-}
-
-// ---------------------------------------------------------------------------------------------
-// K1: unfused push (a1-a4), lcs_particle_step.  One warp per tile; in place; codes + count table.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kBlock)
-k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
-{
-    const int s = blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int t = blockIdx.x * kWarps + warp;
-    const uint32_t cnt_s = T.count[s];
-    const int64_t first = (int64_t)t * kTile;
-    if (first >= (int64_t)cnt_s) return;
-    const SubBox B = sub_box(G, s);
-    uint32_t cnt_c = 0;
-    bool jump = false;
-#pragma unroll 1
-    for (int r = 0; r < kRows; ++r) {
-        const int64_t slot = first + 32 * r + lane;
-        if (first + 32 * r >= (int64_t)cnt_s) break;
-        const bool valid = slot < (int64_t)cnt_s;
-        const size_t at = (size_t)s * (size_t)G.cap + (size_t)slot;
-        Particle p{0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0};
-        if (valid) {
-            p.x = __longlong_as_double(ld_stream(S.f[0] + at)); p.y = __longlong_as_double(ld_stream(S.f[1] + at));
-            p.z = __longlong_as_double(ld_stream(S.f[2] + at)); p.vx = __longlong_as_double(ld_stream(S.f[3] + at));
-            p.vy = __longlong_as_double(ld_stream(S.f[4] + at)); p.vz = __longlong_as_double(ld_stream(S.f[5] + at));
-            p.d = __longlong_as_double(ld_stream(S.f[6] + at));
-        }
-        bool jmp = false;
-        int code = push_particle(p, F4, G, B, dt, lane, jmp);
-        if (valid) {
-            jump |= jmp;
-            st_stream(S.f[0] + at, __double_as_longlong(p.x)); st_stream(S.f[1] + at, __double_as_longlong(p.y));
-            st_stream(S.f[2] + at, __double_as_longlong(p.z)); st_stream(S.f[3] + at, __double_as_longlong(p.vx));
-            st_stream(S.f[4] + at, __double_as_longlong(p.vy)); st_stream(S.f[5] + at, __double_as_longlong(p.vz));
-            S.code[at] = (uint8_t)code;
-        } else code = kInvalid;
-        (void)row_rank(code, valid, lane, cnt_c);
-    }
-    if (jump) raise(T.status, -5);
-    if (lane < kNC && cnt_c) atomicAdd(&T.cnt[s * 32 + lane], cnt_c);      // a4
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -690,6 +571,65 @@ __device__ __forceinline__ uint32_t pack_xyz(const Geom& G, int s)
 {   // px | py << 10 | pz << 20 (each < 1024, checked at lcs_create)
     const int px = s % G.Px, py = (s / G.Px) % G.Py, pz = s / (G.Px * G.Py);
     return (uint32_t)px | ((uint32_t)py << 10) | ((uint32_t)pz << 20);
+}
+
+// a1-a3 for this lane's particle (all 32 lanes must call), unpipelined: the unfused push hides latency with
+// resident warps.  Same arithmetic, same order as the row pipeline of the tile pass.  Returns the destination code.
+__device__ __forceinline__ int push_particle(Particle& p, const double* __restrict__ F4, const Geom& G,
+                                             const SubBox& B, double dt, int lane, bool& jump)
+{
+    Gath Q;
+    gather_issue(Q, F4, G.N, G.inv_dx, p.x, p.y, p.z, lane);
+    Drag D;
+    if (G.drag_model == 0) D = drag_coeffs(p.d, dt, G);       // independent of the gather: issued under its latency
+    const Vec3 U = gather_reduce(Q, lane);
+    if (G.drag_model == 1)                                    // f needs the slip V - U(X) (DESIGN R-23)
+        D = drag_coeffs(p.d, dt, G, drag_factor(p.d, p.vx - U.x, p.vy - U.y, p.vz - U.z, G.inv_nu), true);
+    return advance_particle(p, U, D, G, B, dt, jump);
+}
+
+// ---------------------------------------------------------------------------------------------
+// K1: unfused push (a1-a4), lcs_particle_step.  One warp per tile; in place; codes + count table.
+// ---------------------------------------------------------------------------------------------
+constexpr int kPushWarps = 4;                      // 128-thread CTAs, four per SM (<= 128 registers)
+__global__ void __launch_bounds__(32 * kPushWarps, 4)
+k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
+{
+    const int s = blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int t = blockIdx.x * kPushWarps + warp;
+    const uint32_t cnt_s = T.count[s];
+    const int64_t first = (int64_t)t * kTile;
+    if (first >= (int64_t)cnt_s) return;
+    const SubBox B = sub_box(G, s);
+    uint32_t cnt_c = 0;
+    bool jump = false;
+#pragma unroll 1
+    for (int r = 0; r < kRows; ++r) {
+        const int64_t slot = first + 32 * r + lane;
+        if (first + 32 * r >= (int64_t)cnt_s) break;
+        const bool valid = slot < (int64_t)cnt_s;
+        const size_t at = (size_t)s * (size_t)G.cap + (size_t)slot;
+        Particle p{0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0};
+        if (valid) {
+            p.x = __longlong_as_double(ld_stream(S.f[0] + at)); p.y = __longlong_as_double(ld_stream(S.f[1] + at));
+            p.z = __longlong_as_double(ld_stream(S.f[2] + at)); p.vx = __longlong_as_double(ld_stream(S.f[3] + at));
+            p.vy = __longlong_as_double(ld_stream(S.f[4] + at)); p.vz = __longlong_as_double(ld_stream(S.f[5] + at));
+            p.d = __longlong_as_double(ld_stream(S.f[6] + at));
+        }
+        bool jmp = false;
+        int code = push_particle(p, F4, G, B, dt, lane, jmp);
+        if (valid) {
+            jump |= jmp;
+            st_stream(S.f[0] + at, __double_as_longlong(p.x)); st_stream(S.f[1] + at, __double_as_longlong(p.y));
+            st_stream(S.f[2] + at, __double_as_longlong(p.z)); st_stream(S.f[3] + at, __double_as_longlong(p.vx));
+            st_stream(S.f[4] + at, __double_as_longlong(p.vy)); st_stream(S.f[5] + at, __double_as_longlong(p.vz));
+            S.code[at] = (uint8_t)code;
+        } else code = kInvalid;
+        (void)row_rank(code, valid, lane, cnt_c);
+    }
+    if (jump) raise(T.status, -5);
+    if (lane < kNC && cnt_c) atomicAdd(&T.cnt[s * 32 + lane], cnt_c);      // a4
 }
 
 struct TileRef { int s, t; uint32_t cnt; bool ok; };     // a ticketed tile: subdomain, tile index, count[s]
