@@ -30,6 +30,7 @@ constexpr int kWarps = kBlock / 32;
 #endif
 constexpr int kRows = LCS_ROWS;              // rows (particles per lane) of a warp tile
 constexpr int kTile = 32 * kRows;            // particles per tile
+static_assert(kRows >= 1 && kRows <= 4, "row masks and the unfused pass's code bytes are packed four rows to a word");
 constexpr int kStay = 13;
 constexpr int kNC = 27;                      // destination codes
 constexpr int kInvalid = 31;                 // code of a lane beyond the slab's count
@@ -756,10 +757,15 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             const int nrows = (int)((nvalid + 31u) >> 5);
             SubBox B;
             B.lox = B.loy = B.loz = 0;
+            uint32_t codes_u = 0;          // unfused pass: the codes of this lane's particles, one byte per row
             if (kFused) {
                 const uint32_t c3 = xyz(s);
                 B.lox = (int)(c3 & 1023u) * G.nx; B.loy = (int)((c3 >> 10) & 1023u) * G.ny; B.loz = (int)(c3 >> 20) * G.nz;
             } else {
+                // the code bytes of the whole tile, requested before the wait for the tile's bulk copy (one byte per row and lane)
+#pragma unroll
+                for (int rr = 0; rr < kRows; ++rr)
+                    codes_u |= (uint32_t)S.code[(uint32_t)s * cap32 + first + min(32u * rr + (uint32_t)lane, nvalid - 1u)] << (8 * rr);
                 wait_buf(bc);
             }
             if (lane < kRows) W.stay_m[lane] = 0u;
@@ -820,7 +826,7 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     W.f[2][p] = __double_as_longlong(q.z); W.f[3][p] = __double_as_longlong(q.vx);
                     W.f[4][p] = __double_as_longlong(q.vy); W.f[5][p] = __double_as_longlong(q.vz);
                 } else {
-                    code = min((int)S.code[(uint32_t)s * cap32 + first + min(p, nvalid - 1u)], 26);
+                    code = min((int)((codes_u >> (8 * r)) & 0xffu), 26);
                 }
                 const unsigned stay_m = __ballot_sync(0xffffffffu, valid && code == kStay);
                 const unsigned mig_m = __ballot_sync(0xffffffffu, valid && code != kStay);
