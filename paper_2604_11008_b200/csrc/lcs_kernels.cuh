@@ -593,7 +593,10 @@ __device__ __forceinline__ int push_particle(Particle& p, const double* __restri
 // K1: unfused push (a1-a4), lcs_particle_step.  One warp per tile; in place; codes + count table.
 // ---------------------------------------------------------------------------------------------
 constexpr int kPushWarps = 4;                      // 128-thread CTAs, four per SM (<= 128 registers)
-__global__ void __launch_bounds__(32 * kPushWarps, 4)
+#ifndef LCS_PUSH_BLOCKS
+#define LCS_PUSH_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(32 * kPushWarps, LCS_PUSH_BLOCKS)
 k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
 {
     const int s = blockIdx.y;
