@@ -3,12 +3,14 @@
 // multiply-add happens only where fma() is written, so the push is bit-reproducible (DESIGN.md
 // section 4, rules R1-R7).
 //
-// Execution model of the hot kernel (k_tile_pass): WARP-AUTONOMOUS tiles.  A tile is 128
-// consecutive slots of one subdomain slab (4 rows of 32 lanes).  Every warp of a persistent grid
-// takes tiles from an atomic ticket and runs the whole path for its tile with warp-level
-// primitives only (ballot / shuffle / popc, a private shared-memory staging area, no block
-// barrier): the 24 resident warps of an SM drift apart in phase, so the DRAM stream, the L2
-// gather, the fp64 arithmetic, the look-back and the write-out of different tiles overlap.
+// Execution model of the hot kernel (k_tile_pass): WARP-AUTONOMOUS tiles in a latency pipeline.  A tile
+// is kTile = 64 consecutive slots of one subdomain slab (2 rows of 32 lanes).  Every warp of a
+// persistent grid (one CTA of 12 warps per SM) takes tiles from an atomic ticket and runs the whole
+// path for its tile with warp-level primitives only (ballot / shuffle / popc / redux, three private
+// shared-memory tile buffers fed by bulk tensor copies, no block barrier after the prologue); the
+// gather of the next row is in flight under the arithmetic of the current one.  The comment above
+// k_tile_pass has the details.  Macros LCS_X_* are ablation builds (wrong results on purpose), used
+// for the measurements quoted in DESIGN.md 6.5 and profiles/.
 #pragma once
 #include <cuda.h>            // CUtensorMap (the type only; the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
