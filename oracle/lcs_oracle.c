@@ -22,6 +22,8 @@
  *   orc_interp             constant / nodal / tri-affine closed forms; O(dx^2) convergence; seam
  *   orc_push (advance)     closed-form drag relaxation V(t), X(t) under constant U and g
  *   orc_push (classify)    hand-placed particles for all 27 codes, seams, Px in {1,2,3}
+ *   orc_classify_axis      hand-placed particles per axis incl. the seam and P_a in {1,2,3}; after the three sweeps every
+ *                          particle is in its owner's slab and the slabs hold the same id sets as the direct 27-way migrate
  *   orc_migrate            paper's worked example; global-sort brute force;
  *                          conservation; containment; idempotence
  *   contents after a sticky error: parity unpinned (by design)
@@ -347,6 +349,43 @@ int orc_push(orc_t *o, double dt)
             int c = (du[0] + 1) + 3 * (du[1] + 1) + 9 * (du[2] + 1);
             o->code[slot] = (uint8_t)c;
             o->cnt[s * 27 + c] += 1;                           /* a4 */
+        }
+    }
+    o->pushed = 1;
+    return o->status;
+}
+
+/* ---- axis-by-axis exchange (SURVEY.md 8(f) NEXT #3; PAPER.md:114-118 "mask", :191 "per direction", :243 "all three
+ * communications"; R-24).  One sweep = classify along ONE axis from the particle's current position relative
+ * to the slab it sits in, then the same ordered pack / compaction / append as orc_migrate with the three codes of that
+ * axis.  The direction is the minimum-image difference of subdomain indices: with P_a >= 3 a difference of +-(P_a - 1)
+ * is the periodic neighbour -+1; with P_a = 2 the difference is already in {-1, 0, +1}; with P_a = 1 nothing moves. ---- */
+int orc_classify_axis(orc_t *o, int axis)
+{
+    if (axis < 0 || axis > 2) return ORC_ERR_ARG;
+    if (o->status) return o->status;
+    const int64_t Pa[3] = { o->Px, o->Py, o->Pz };
+    const int64_t na[3] = { o->nx, o->ny, o->nz };
+    const int w[3] = { 1, 3, 9 };
+    memset(o->cnt, 0, (size_t)o->P * 27 * sizeof(int64_t));
+    for (int64_t s = 0; s < o->P; ++s) {
+        const int64_t pa[3] = { s % o->Px, (s / o->Px) % o->Py, s / ((int64_t)o->Px * o->Py) };
+        for (int64_t i = 0; i < o->count[s]; ++i) {
+            const int64_t slot = s * o->cap + i;
+            const double a = o->f[axis][slot];
+            int64_t dd = 0;
+            if (!(a >= 0.0 && a < o->L)) o->status = ORC_ERR_JUMP;
+            else {
+                dd = cell_of(o, a) / na[axis] - pa[axis];
+                if (Pa[axis] >= 3) {
+                    if (dd > 1) dd -= Pa[axis];
+                    else if (dd < -1) dd += Pa[axis];
+                }
+                if (dd < -1 || dd > 1) { o->status = ORC_ERR_JUMP; dd = dd < -1 ? -1 : 1; }
+            }
+            const int c = ORC_STAY + (int)dd * w[axis];
+            o->code[slot] = (uint8_t)c;
+            o->cnt[s * 27 + c] += 1;
         }
     }
     o->pushed = 1;

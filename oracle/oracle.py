@@ -63,6 +63,7 @@ def lib():
         L.orc_load_packed.argtypes = [C.c_void_p, _ip] + [_dp] * 7 + [_ip, _bp]
         L.orc_push.argtypes = [C.c_void_p, C.c_double]
         L.orc_migrate.argtypes = [C.c_void_p]
+        L.orc_classify_axis.argtypes = [C.c_void_p, C.c_int]
         L.orc_total.restype = C.c_int64
         L.orc_total.argtypes = [C.c_void_p]
         L.orc_status.argtypes = [C.c_void_p]
@@ -178,6 +179,21 @@ class Oracle:
     def step(self, dt):
         rc = self.push(dt)
         return rc if rc else self.migrate()
+
+    def classify_axis(self, axis):
+        """Codes of ONE axis (0: x, 1: y, 2: z) from the current positions, relative to the slab each particle sits in."""
+        return lib().orc_classify_axis(self._h, int(axis))
+
+    def migrate_sweeps(self):
+        """Axis-by-axis exchange (R-24): x, then y, then z; -> (rc, migrants moved in each sweep)."""
+        moved = []
+        for axis in range(3):
+            rc = self.classify_axis(axis)
+            rc = rc if rc else self.migrate()
+            if rc:
+                return rc, moved
+            moved.append(self.n_migrated_last)
+        return 0, moved
 
     @property
     def status(self):
