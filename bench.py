@@ -272,6 +272,17 @@ def run_cuda(args):
         if (err_u or n_tot_u != n) and not os.environ.get("LCS_BENCH_ABLATION"):
             print(f"bench.py: unfused step failed: sticky status {err_u}, total {n_tot_u}", file=sys.stderr)
             return 3
+        # axis-by-axis exchange: lcs_particle_step + lcs_migrate_sweeps, the sweeps timed
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(3)]
+        for k in range(3):
+            lcs.particle_step(dt)
+            evs[k][0].record(); lcs.migrate_sweeps(); evs[k][1].record()
+        torch.cuda.synchronize()
+        err_s, n_tot_s, _ = lcs.get_status()
+        if (err_s or n_tot_s != n) and not os.environ.get("LCS_BENCH_ABLATION"):
+            print(f"bench.py: sweep step failed: sticky status {err_s}, total {n_tot_s}", file=sys.stderr)
+            return 3
+        sweeps_ms = float(np.median([e[0].elapsed_time(e[1]) for e in evs]))
         # per-step fluid refresh (first half): lcs_set_fluid = the repack of the three x-fastest
         # arrays into the internal (u,v,w,0) z-fastest records, as a coupled solver would call it every step
         evf = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(3)]
@@ -294,6 +305,8 @@ def run_cuda(args):
                         "algorithmic_GBps": mig_bytes / (mig_ms * 1e-3) / 1e9,
                         "frac_of_measured_peak": mig_bytes / (mig_ms * 1e-3) / 1e9 / peak_p,
                         "migrant_fraction": m_u},
+            "migrate_sweeps": {"call": "lcs_migrate_sweeps", "ms": sweeps_ms, "particles_per_s": n / (sweeps_ms * 1e-3),
+                               "note": "x, y, z sweeps: three classify + unfused tile pass + scan + table + unpack rounds"},
             "set_fluid": {"call": "lcs_set_fluid", "ms": fluid_ms,
                           "GBps": (24.0 + 32.0) * N ** 3 / (fluid_ms * 1e-3) / 1e9,
                           "note": "reads 24 B and writes 32 B per cell; off the timed step (the fluid is frozen)"},

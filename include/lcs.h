@@ -98,6 +98,15 @@ int lcs_particle_step(lcs_t* h, double dt);
  * ascending (DESIGN R-12).  LCS_ERR_STATE if no lcs_particle_step preceded it. */
 int lcs_migrate(lcs_t* h);
 
+/* Axis-by-axis exchange (R-24): three sweeps x, y, z.  Each sweep classifies
+ * every particle along one axis from its CURRENT position relative to the slab it sits in (minimum-image difference of
+ * subdomain indices) and migrates with the three codes of that axis, in the order of lcs_migrate within the sweep.
+ * After the call every particle is in the slab that contains it -- the same slab contents as lcs_migrate delivers, in the
+ * sweeps' own (unique, deterministic) order.  May follow lcs_particle_step instead of lcs_migrate, or be called on its
+ * own.  lcs_get_status then reports the migrants of the LAST sweep.  LCS_ERR_STATE without particles; a particle more
+ * than one subdomain away from its slab along an axis raises the sticky LCS_ERR_JUMP. */
+int lcs_migrate_sweeps(lcs_t* h);
+
 /* lcs_particle_step followed by lcs_migrate in one pass that reads and writes each particle
  * once; the result is bit-identical to the two calls. */
 int lcs_step_fused(lcs_t* h, double dt);

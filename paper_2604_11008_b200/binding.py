@@ -10,7 +10,7 @@ LCS_ERR_CAPACITY, LCS_ERR_JUMP, LCS_ERR_RANGE = -4, -5, -6
 
 EXPORTED_SYMBOLS = (
     "lcs_workspace_bytes", "lcs_create", "lcs_destroy", "lcs_set_fluid", "lcs_set_particles",
-    "lcs_particle_step", "lcs_migrate", "lcs_step_fused", "lcs_get_counts", "lcs_get_particles",
+    "lcs_particle_step", "lcs_migrate", "lcs_migrate_sweeps", "lcs_step_fused", "lcs_get_counts", "lcs_get_particles",
     "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_step_fused_host",
     "lcs_profile_begin", "lcs_profile_end", "lcs_kernel_launches", "lcs_version")
 
@@ -58,6 +58,7 @@ def load_library(build_if_missing: bool = True):
     L.lcs_set_particles.argtypes = [vp, i64] + [vp] * 8
     L.lcs_particle_step.argtypes = [vp, dbl]
     L.lcs_migrate.argtypes = [vp]
+    L.lcs_migrate_sweeps.argtypes = [vp]
     L.lcs_step_fused.argtypes = [vp, dbl]
     L.lcs_get_counts.argtypes = [vp, vp]
     L.lcs_get_particles.argtypes = [vp] * 10
@@ -149,6 +150,10 @@ class LCS:
 
     def migrate(self):
         self._chk("lcs_migrate", self._L.lcs_migrate(self._h))
+
+    def migrate_sweeps(self):
+        """Axis-by-axis exchange: x, y, z sweeps (R-24)."""
+        self._chk("lcs_migrate_sweeps", self._L.lcs_migrate_sweeps(self._h))
 
     def step_fused(self, dt):
         self._chk("lcs_step_fused", self._L.lcs_step_fused(self._h, float(dt)))

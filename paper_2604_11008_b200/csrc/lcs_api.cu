@@ -330,6 +330,21 @@ int lcs_migrate(lcs_t* h)
     return enqueue_tile_pass(h, false, 0.0);
 }
 
+int lcs_migrate_sweeps(lcs_t* h)
+{
+    if (!h) return LCS_ERR_INVALID_ARG;
+    if (!h->have_particles) return LCS_ERR_STATE;
+    if (h->sticky) return h->sticky;
+    const Geom& G = h->G;
+    for (int axis = 0; axis < 3; ++axis) {
+        k_classify_axis<<<dim3((unsigned)((G.cap + 255) / 256), G.P), 256, 0, h->stream>>>(G, h->S, h->T, axis);
+        int rc = check_launch(h);
+        if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0);
+        if (rc != LCS_OK) return rc;
+    }
+    return LCS_OK;
+}
+
 int lcs_step_fused(lcs_t* h, double dt)
 {
     if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;

@@ -1122,6 +1122,39 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
 }
 
 // ---------------------------------------------------------------------------------------------
+// Axis-by-axis exchange (R-24): destination code along ONE axis from the particle's current
+// position relative to the slab it sits in (minimum-image difference of subdomain indices), written
+// as the code byte the unfused tile pass consumes.  One thread per slot.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_classify_axis(Geom G, Slabs S, Tables T, int axis)
+{
+    const int s = blockIdx.y;
+    const uint32_t cnt_s = T.count[s];
+    const uint32_t i = blockIdx.x * 256u + threadIdx.x;
+    if (i >= cnt_s) return;
+    const int Pa = axis == 0 ? G.Px : (axis == 1 ? G.Py : G.Pz);
+    const int n_a = axis == 0 ? G.nx : (axis == 1 ? G.ny : G.nz);
+    const int p_a = axis == 0 ? s % G.Px : (axis == 1 ? (s / G.Px) % G.Py : s / (G.Px * G.Py));
+    const int w = axis == 0 ? 1 : (axis == 1 ? 3 : 9);
+    const uint32_t at = (uint32_t)s * (uint32_t)G.cap + i;
+    const double a = S.f[axis][at];
+    int dd = 0;
+    if (!(a >= 0.0 && a < G.L)) raise(T.status, -5);
+    else {
+        int ic = __double2int_rd(a * G.inv_dx);
+        ic = max(0, min(ic, G.N - 1));
+        dd = ic / n_a - p_a;
+        if (Pa >= 3) {
+            if (dd > 1) dd -= Pa;
+            else if (dd < -1) dd += Pa;
+        }
+        if (dd < -1 || dd > 1) { raise(T.status, -5); dd = dd < -1 ? -1 : 1; }
+    }
+    S.code[at] = (uint8_t)(kStay + dd * w);
+}
+
+// ---------------------------------------------------------------------------------------------
 // accessors
 // ---------------------------------------------------------------------------------------------
 __global__ void k_counts_out(Geom G, Tables T, int64_t* out, int64_t* prefix)

@@ -206,6 +206,46 @@ def test_nonlinear_drag_model_matches_oracle(torch_cuda, oracle_lib, scale_d, P)
     dev.close(); dev2.close()
 
 
+@pytest.mark.parametrize("P,N", [((2, 2, 2), 16), ((3, 3, 3), 24), ((1, 2, 3), 12), ((5, 1, 3), 15), ((4, 4, 4), 32)])
+def test_axis_sweeps_match_oracle(torch_cuda, oracle_lib, P, N):
+    """lcs_migrate_sweeps (x, y, z sweeps, DESIGN R-24) after lcs_particle_step: ids, order, counts
+    and state bit-identical to the oracle's sweeps; slab contents equal to the direct migration's."""
+    rng = np.random.default_rng(P[0] * 31 + N)
+    nP = P[0] * P[1] * P[2]
+    n = 2500 * nP + 3
+    Ls = np.array([L / P[0], L / P[1], L / P[2]])
+    parts = random_parts(rng, n, 0.45 * Ls)
+    z = np.zeros(N ** 3)
+    cap = 2 * (int(1.6 * n / nP) // 2 + 200)
+    o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, cap, (z, z, z), parts)
+    _, dev_direct, _ = make_pair(torch_cuda, oracle_lib, N, P, cap, (z, z, z), parts)
+    for step in range(2):
+        assert o.push(0.7) == 0
+        rc, moved = o.migrate_sweeps()
+        assert rc == 0
+        dev.particle_step(0.7)
+        dev.migrate_sweeps()
+        assert dev.get_status() == (0, n, moved[2])
+        got, _ = compare_packed(dev, o, f"sweeps step {step}")
+        dev_direct.step_fused(0.7)
+        direct = to_np(dev_direct.get_particles())
+        assert np.array_equal(got["counts"], direct["counts"])
+        off = np.concatenate([[0], np.cumsum(got["counts"])])
+        for s in range(nP):
+            assert np.array_equal(np.sort(got["id"][off[s]:off[s + 1]]), np.sort(direct["id"][off[s]:off[s + 1]]))
+        # the two paths now hold different orders: bring the direct one to the sweeps' state for the next step
+        dp = to_dev(torch_cuda, {k: got[k] for k in F8})
+        dev_direct.set_particles(*(dp[k] for k in F8))
+    # on its own (no push before): nothing to move, nothing changes
+    before = to_np(dev.get_particles())
+    dev.migrate_sweeps()
+    after = to_np(dev.get_particles())
+    assert dev.get_status() == (0, n, 0)
+    for k in F8 + ("counts",):
+        assert np.array_equal(before[k], after[k])
+    dev.close(); dev_direct.close()
+
+
 def test_all_27_codes_hand_placed(torch_cuda, oracle_lib):
     for P in [(3, 3, 3), (2, 2, 2), (1, 2, 3), (1, 1, 1)]:
         N = 24
