@@ -368,7 +368,10 @@ k_repack_fluid(int N, const double* __restrict__ u, const double* __restrict__ v
 //   float reciprocals (prefetch shares); the ticket -> (s,t) map is an incremental search from the
 //   previous subdomain; particle slots are 32-bit indices (P*cap < 2^32 is checked at lcs_create).
 // ---------------------------------------------------------------------------------------------
-constexpr int kNBuf = 3;                     // tile buffers per warp: loading / being pushed / awaiting resolve
+#ifndef LCS_NBUF
+#define LCS_NBUF 3
+#endif
+constexpr int kNBuf = LCS_NBUF;                     // tile buffers per warp: loading / being pushed / awaiting resolve
 constexpr int kTableSmemMax = 1024;          // tile_start[] and the subdomain coordinates are mirrored in shared memory up to this P
 
 struct alignas(128) TileBuf {
