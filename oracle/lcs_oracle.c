@@ -22,6 +22,9 @@
  *   orc_interp             constant / nodal / tri-affine closed forms; O(dx^2) convergence; seam
  *   orc_push (advance)     closed-form drag relaxation V(t), X(t) under constant U and g
  *   orc_push (classify)    hand-placed particles for all 27 codes, seams, Px in {1,2,3}
+ *   orc_rk2_stage1/2       Heun amplification factor 1 - z + z^2/2 and the position polynomial under constant U, g;
+ *                          second-order convergence to the exact solution; decomposition independence (1x1x1 = 2x2x2 = 3x2x1
+ *                          by id, which fails unless all 17 arrays travel with the particle); containment
  *   orc_classify_axis      hand-placed particles per axis incl. the seam and P_a in {1,2,3}; after the three sweeps every
  *                          particle is in its owner's slab and the slabs hold the same id sets as the direct 27-way migrate
  *   orc_migrate            paper's worked example; global-sort brute force;
@@ -47,6 +50,7 @@ typedef struct orc {
     const double *u, *v, *w;            /* borrowed, N^3 each, x fastest */
     double *f[7];                       /* x y z vx vy vz d : P*cap each (SoA) */
     int64_t *id;                        /* P*cap */
+    double *ex[9];                      /* RK2 only: x0 y0 z0 vx0 vy0 vz0 and dV/dt of stage 1; NULL until used */
     uint8_t *code;                      /* P*cap, destination code of the last push */
     int64_t *send_slot;                 /* P*cap, storage position in the (s,c) send buffer, -1 = stay */
     int64_t *count;                     /* P   */
@@ -232,6 +236,7 @@ void orc_destroy(orc_t *o)
 {
     if (!o) return;
     for (int a = 0; a < 7; ++a) free(o->f[a]);
+    for (int a = 0; a < 9; ++a) free(o->ex[a]);
     free(o->id); free(o->code); free(o->send_slot); free(o->count); free(o->cnt);
     free(o);
 }
@@ -355,6 +360,88 @@ int orc_push(orc_t *o, double dt)
     return o->status;
 }
 
+/* ---- the paper's two-stage RK2 with per-stage migration ("explicit two-stage
+ * Runge-Kutta", :150-164 the 17 arrays, :175-177 one communication per stage; R-25: Heun).
+ *   stage 1: K1 = (U(X0) - V0)/tau + g ; X1 = X0 + dt V0 ; V1 = V0 + dt K1 ; keep X0, V0, K1 ; classify X1 ; migrate
+ *   stage 2: K2 = (U(X1) - V1)/tau + g ; X  = X0 + dt/2 (V0 + V1) ; V = V0 + dt/2 (K1 + K2) ; classify X ; migrate
+ * tau = tau_p / f with f evaluated at the start of each stage (f = 1 for drag_model 0).  The destination of a stage is
+ * the minimum-image direction from the slab the particle sits in to the owner of its new position, per axis (the
+ * particle of stage 2 no longer sits in the slab of X0, so the wrap of X0 + ... says nothing about it). ---- */
+static int min_image_code(orc_t *o, int64_t s, const double *pos3)
+{
+    const int64_t Pa[3] = { o->Px, o->Py, o->Pz };
+    const int64_t na[3] = { o->nx, o->ny, o->nz };
+    const int64_t pa[3] = { s % o->Px, (s / o->Px) % o->Py, s / ((int64_t)o->Px * o->Py) };
+    const int w[3] = { 1, 3, 9 };
+    int c = ORC_STAY;
+    for (int a = 0; a < 3; ++a) {
+        int64_t dd = 0;
+        if (!(pos3[a] >= 0.0 && pos3[a] < o->L)) o->status = ORC_ERR_JUMP;
+        else {
+            dd = cell_of(o, pos3[a]) / na[a] - pa[a];
+            if (Pa[a] >= 3) { if (dd > 1) dd -= Pa[a]; else if (dd < -1) dd += Pa[a]; }
+            if (dd < -1 || dd > 1) { o->status = ORC_ERR_JUMP; dd = dd < -1 ? -1 : 1; }
+        }
+        c += (int)dd * w[a];
+    }
+    return c;
+}
+
+static double wrap_once(const orc_t *o, double xu)
+{
+    if (xu < 0.0) { xu = xu + o->L; if (xu >= o->L) xu = o->L_below; }
+    else if (xu >= o->L) xu = xu - o->L;
+    return xu;                                      /* still outside [0, L): min_image_code raises ORC_ERR_JUMP */
+}
+
+static int rk2_stage(orc_t *o, double dt, int stage)
+{
+    if (!o->u) return ORC_ERR_STATE;
+    if (o->status) return o->status;
+    const size_t slots = (size_t)o->P * (size_t)o->cap;
+    for (int a = 0; a < 9; ++a)
+        if (!o->ex[a]) { o->ex[a] = (double *)calloc(slots, sizeof(double)); if (!o->ex[a]) return ORC_ERR_NOMEM; }
+    if (stage == 2 && o->pushed) return ORC_ERR_STATE;          /* stage 1's codes must have been migrated */
+    memset(o->cnt, 0, (size_t)o->P * 27 * sizeof(int64_t));
+    const double hdt = 0.5 * dt;
+    for (int64_t s = 0; s < o->P; ++s)
+        for (int64_t i = 0; i < o->count[s]; ++i) {
+            const int64_t slot = s * o->cap + i;
+            stencil1d sx = stencil_axis(o, o->f[0][slot]);
+            stencil1d sy = stencil_axis(o, o->f[1][slot]);
+            stencil1d sz = stencil_axis(o, o->f[2][slot]);
+            double U[3] = { tri(o->u, o->N, sx, sy, sz), tri(o->v, o->N, sx, sy, sz), tri(o->w, o->N, sx, sy, sz) };
+            double d = o->f[6][slot];
+            double tau = (o->K_tau * d) * d;
+            if (o->drag_model == 1)
+                tau = tau / orc_drag_factor(o, d, o->f[3][slot] - U[0], o->f[4][slot] - U[1], o->f[5][slot] - U[2]);
+            double pos[3];
+            for (int a = 0; a < 3; ++a) {
+                double v = o->f[3 + a][slot];
+                double k = (U[a] - v) / tau + o->g[a];              /* Eq. 6 + g (R-4) */
+                if (stage == 1) {
+                    double x = o->f[a][slot];
+                    o->ex[a][slot] = x; o->ex[3 + a][slot] = v; o->ex[6 + a][slot] = k;
+                    pos[a] = wrap_once(o, fma(dt, v, x));           /* X1 = X0 + dt V0 */
+                    o->f[3 + a][slot] = fma(dt, k, v);              /* V1 = V0 + dt K1 */
+                } else {
+                    double x0 = o->ex[a][slot], v0 = o->ex[3 + a][slot], k1 = o->ex[6 + a][slot];
+                    pos[a] = wrap_once(o, fma(hdt, v0 + v, x0));    /* X = X0 + dt/2 (V0 + V1) */
+                    o->f[3 + a][slot] = fma(hdt, k1 + k, v0);       /* V = V0 + dt/2 (K1 + K2) */
+                }
+                o->f[a][slot] = pos[a];
+            }
+            int c = min_image_code(o, s, pos);
+            o->code[slot] = (uint8_t)c;
+            o->cnt[s * 27 + c] += 1;
+        }
+    o->pushed = 1;
+    return o->status;
+}
+
+int orc_rk2_stage1(orc_t *o, double dt) { return rk2_stage(o, dt, 1); }
+int orc_rk2_stage2(orc_t *o, double dt) { return rk2_stage(o, dt, 2); }
+
 /* ---- axis-by-axis exchange (SURVEY.md 8(f) NEXT #3; PAPER.md:114-118 "mask", :191 "per direction", :243 "all three
  * communications"; R-24).  One sweep = classify along ONE axis from the particle's current position relative
  * to the slab it sits in, then the same ordered pack / compaction / append as orc_migrate with the three codes of that
@@ -404,9 +491,12 @@ int orc_migrate(orc_t *o)
     int64_t *seg_start = (int64_t *)malloc((size_t)P * 27 * sizeof(int64_t));
     int64_t *counter = (int64_t *)calloc((size_t)P * 27, sizeof(int64_t));   /* per-direction counter */
     double *sb[7]; int64_t *sbid;
+    double *sbe[9];                                   /* the RK2 arrays travel with the particle */
+    const int rk2 = o->ex[0] != NULL;
     size_t m = (size_t)(nmig > 0 ? nmig : 1);
     for (int a = 0; a < 7; ++a) sb[a] = (double *)malloc(m * sizeof(double));
     sbid = (int64_t *)malloc(m * sizeof(int64_t));
+    for (int a = 0; a < 9; ++a) sbe[a] = rk2 ? (double *)malloc(m * sizeof(double)) : NULL;
     int64_t *stay = (int64_t *)malloc((size_t)P * sizeof(int64_t));
     int64_t *fill = (int64_t *)malloc((size_t)P * sizeof(int64_t));
     {
@@ -428,6 +518,7 @@ int orc_migrate(orc_t *o)
                 o->send_slot[slot] = -1;
                 if (dst != slot) {
                     for (int a = 0; a < 7; ++a) o->f[a][dst] = o->f[a][slot];
+                    if (rk2) for (int a = 0; a < 9; ++a) o->ex[a][dst] = o->ex[a][slot];
                     o->id[dst] = o->id[slot];
                 }
                 ++nstay;
@@ -436,6 +527,7 @@ int orc_migrate(orc_t *o)
                 int64_t dst = seg_start[s * 27 + c] + k;
                 o->send_slot[slot] = k;
                 for (int a = 0; a < 7; ++a) sb[a][dst] = o->f[a][slot];
+                if (rk2) for (int a = 0; a < 9; ++a) sbe[a][dst] = o->ex[a][slot];
                 sbid[dst] = o->id[slot];
             }
         }
@@ -452,6 +544,7 @@ int orc_migrate(orc_t *o)
             if (fill[r] + len > cap) { overflow = 1; break; }
             int64_t src = seg_start[s * 27 + c], dst = r * cap + fill[r];
             for (int a = 0; a < 7; ++a) memcpy(o->f[a] + dst, sb[a] + src, (size_t)len * sizeof(double));
+            if (rk2) for (int a = 0; a < 9; ++a) memcpy(o->ex[a] + dst, sbe[a] + src, (size_t)len * sizeof(double));
             memcpy(o->id + dst, sbid + src, (size_t)len * sizeof(int64_t));
             fill[r] += len;
         }
@@ -467,6 +560,7 @@ int orc_migrate(orc_t *o)
     }
     o->pushed = 0;
     for (int a = 0; a < 7; ++a) free(sb[a]);
+    for (int a = 0; a < 9; ++a) free(sbe[a]);
     free(sbid); free(seg_start); free(counter); free(stay); free(fill);
     return o->status;
 }

@@ -64,6 +64,8 @@ def lib():
         L.orc_push.argtypes = [C.c_void_p, C.c_double]
         L.orc_migrate.argtypes = [C.c_void_p]
         L.orc_classify_axis.argtypes = [C.c_void_p, C.c_int]
+        L.orc_rk2_stage1.argtypes = [C.c_void_p, C.c_double]
+        L.orc_rk2_stage2.argtypes = [C.c_void_p, C.c_double]
         L.orc_total.restype = C.c_int64
         L.orc_total.argtypes = [C.c_void_p]
         L.orc_status.argtypes = [C.c_void_p]
@@ -179,6 +181,21 @@ class Oracle:
     def step(self, dt):
         rc = self.push(dt)
         return rc if rc else self.migrate()
+
+    def rk2_stage1(self, dt):
+        return lib().orc_rk2_stage1(self._h, float(dt))
+
+    def rk2_stage2(self, dt):
+        return lib().orc_rk2_stage2(self._h, float(dt))
+
+    def step_rk2(self, dt):
+        """The paper's two-stage RK2 (Heun) with one migration per stage (R-25)."""
+        for stage in (self.rk2_stage1, self.rk2_stage2):
+            rc = stage(dt)
+            rc = rc if rc else self.migrate()
+            if rc:
+                return rc
+        return 0
 
     def classify_axis(self, axis):
         """Codes of ONE axis (0: x, 1: y, 2: z) from the current positions, relative to the slab each particle sits in."""
