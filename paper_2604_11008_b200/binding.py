@@ -10,7 +10,7 @@ LCS_ERR_CAPACITY, LCS_ERR_JUMP, LCS_ERR_RANGE = -4, -5, -6
 
 EXPORTED_SYMBOLS = (
     "lcs_workspace_bytes", "lcs_create", "lcs_destroy", "lcs_set_fluid", "lcs_set_particles",
-    "lcs_particle_step", "lcs_migrate", "lcs_migrate_sweeps", "lcs_step_fused", "lcs_get_counts", "lcs_get_particles",
+    "lcs_particle_step", "lcs_migrate", "lcs_migrate_sweeps", "lcs_step_rk2", "lcs_step_fused", "lcs_get_counts", "lcs_get_particles",
     "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_step_fused_host",
     "lcs_profile_begin", "lcs_profile_end", "lcs_kernel_launches", "lcs_version")
 
@@ -25,7 +25,7 @@ class LcsError(RuntimeError):
 
 class LcsParams(C.Structure):
     _fields_ = [("nu", C.c_double), ("rho_ratio", C.c_double), ("g", C.c_double * 3),
-                ("send_capacity", C.c_int64), ("drag_model", C.c_int32)]
+                ("send_capacity", C.c_int64), ("drag_model", C.c_int32), ("enable_rk2", C.c_int32)]
 
 
 def lib_path() -> str:
@@ -59,6 +59,7 @@ def load_library(build_if_missing: bool = True):
     L.lcs_particle_step.argtypes = [vp, dbl]
     L.lcs_migrate.argtypes = [vp]
     L.lcs_migrate_sweeps.argtypes = [vp]
+    L.lcs_step_rk2.argtypes = [vp, C.c_double]
     L.lcs_step_fused.argtypes = [vp, dbl]
     L.lcs_get_counts.argtypes = [vp, vp]
     L.lcs_get_particles.argtypes = [vp] * 10
@@ -83,7 +84,7 @@ class LCS:
     Device tensors in, device tensors out; torch allocates, the library computes."""
 
     def __init__(self, N, Px, Py, Pz, capacity, nu=1.5e-5, rho_ratio=1000.0, g=(0.0, 0.0, 0.0),
-                 send_capacity=0, drag_model=0, device="cuda:0", stream=None):
+                 send_capacity=0, drag_model=0, rk2=False, device="cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2604_11008_b200 needs a CUDA device (no CPU fallback)")
@@ -92,7 +93,7 @@ class LCS:
         self.device = torch.device(device)
         self.N, self.Px, self.Py, self.Pz, self.capacity = N, Px, Py, Pz, int(capacity)
         self.P = Px * Py * Pz
-        self._prm = LcsParams(nu, rho_ratio, (C.c_double * 3)(*g), int(send_capacity), int(drag_model))
+        self._prm = LcsParams(nu, rho_ratio, (C.c_double * 3)(*g), int(send_capacity), int(drag_model), int(bool(rk2)))
         nbytes = self._L.lcs_workspace_bytes(N, Px, Py, Pz, int(capacity), C.byref(self._prm))
         if nbytes == 0:
             raise LcsError("lcs_workspace_bytes", LCS_ERR_INVALID_ARG)
@@ -150,6 +151,10 @@ class LCS:
 
     def migrate(self):
         self._chk("lcs_migrate", self._L.lcs_migrate(self._h))
+
+    def step_rk2(self, dt):
+        """The paper's two-stage RK2 with one migration per stage (needs rk2=True at construction; R-25)."""
+        self._chk("lcs_step_rk2", self._L.lcs_step_rk2(self._h, float(dt)))
 
     def migrate_sweeps(self):
         """Axis-by-axis exchange: x, y, z sweeps (R-24)."""

@@ -32,6 +32,9 @@ struct lcs_handle {
     int prof_steps, prof_max;
     int grid_fused, grid_pack;         // persistent grid sizes of the tile pass
     CUtensorMap slab_map;              // 2-D view [8 fields][P*cap slots] of the slabs, box 8 x kTile (bulk tile loads)
+    bool rk2;                          // the 9 extra arrays of the two-stage RK2 exist (lcs_params.enable_rk2)
+    Slabs SB, SC;                      // RK2: x0 y0 z0 vx0 vy0 vz0 k1x k1y | k1z + 7 spare arrays (groups of 8 for the tile pass)
+    CUtensorMap mapB, mapC;
     size_t gacc_bytes;
 };
 
@@ -42,6 +45,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t slab_f[7], slab_id, slab_code;
+    size_t rk2_b, rk2_c;               // RK2 groups B and C: 8 arrays each, stride as the slabs (0 = absent)
     size_t pool, pool_bytes, fluid4;
     size_t count, cnt, recv_off, new_count, desc, gacc, gacc_bytes, tile_start, tile_cnt, group_excl, misc, prefix;
     size_t total;
@@ -63,6 +67,7 @@ bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* pr
     if (prm->send_capacity < 0 || (prm->send_capacity & 1) || prm->send_capacity > cap) return false;
     if (!(prm->nu > 0.0) || !(prm->rho_ratio > 0.0)) return false;
     if (prm->drag_model != 0 && prm->drag_model != 1) return false;
+    if (prm->enable_rk2 != 0 && prm->enable_rk2 != 1) return false;
     if (!std::isfinite(prm->g[0]) || !std::isfinite(prm->g[1]) || !std::isfinite(prm->g[2])) return false;
     return true;
 }
@@ -81,6 +86,11 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     for (int a = 0; a < 7; ++a) { L.slab_f[a] = off; off = align_up(off + slots * 8); }
     L.slab_id = off;   off = align_up(off + slots * 8);
     L.slab_code = off; off = align_up(off + slots);
+    L.rk2_b = L.rk2_c = 0;
+    if (prm->enable_rk2) {
+        L.rk2_b = off; off += 8 * align_up(slots * 8);
+        L.rk2_c = off; off += 8 * align_up(slots * 8);
+    }
     // send pool: 8 arrays of P*send_cap slots; doubles as lcs_set_particles scratch
     const size_t send_bytes = 8 * align_up(P * (size_t)L.send_cap * 8);
     const size_t set_tiles = (slots + kSetTile - 1) / kSetTile;
@@ -103,6 +113,25 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     return L;
 }
 
+// Tensor map of one group of 8 arrays for the bulk tile loads: 2-D [8 fields][slots] of 8-byte words, rows `stride` bytes
+// apart, box 8 x kTile.  The encoder is fetched from the driver through the runtime (no link against libcuda).
+bool make_slab_map(CUtensorMap* out, void* base, size_t slots, size_t stride)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
+    const cuuint64_t gdim[2] = {(cuuint64_t)slots, 8};
+    const cuuint64_t gstride[1] = {(cuuint64_t)stride};
+    const cuuint32_t box[2] = {(cuuint32_t)kTile, 8};
+    const cuuint32_t estr[2] = {1, 1};
+    return reinterpret_cast<encode_fn>(fn)(out, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, base, gdim, gstride, box, estr,
+                                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                           CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 inline size_t tile_pass_smem(int P)
 {
     return kWarps * kNBuf * (sizeof(TileBuf) + sizeof(uint64_t)) + (P <= kTableSmemMax ? (size_t)(2 * P + 1) * sizeof(uint32_t) : 0);
@@ -116,9 +145,15 @@ inline int check_launch(lcs_t* h, int n = 1)
     return cudaPeekAtLastError() == cudaSuccess ? LCS_OK : LCS_ERR_CUDA;
 }
 
-int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
+// One round of the migration machinery on one group of 8 arrays (the slabs, or an RK2 group that travels with the same
+// codes): tile pass, per-code scan, table, unpack; `commit` also installs the new counts and the next tile index.  The
+// rounds of one migration see the same codes and the same counts, so they apply the same permutation.
+int enqueue_tile_pass(lcs_t* h, bool fused, double dt, const Slabs* grp = nullptr, const CUtensorMap* map = nullptr,
+                      bool commit = true)
 {
     const Geom& G = h->G;
+    const Slabs& S = grp ? *grp : h->S;
+    const CUtensorMap& M = map ? *map : h->slab_map;
     h->epoch = (h->epoch + 1u) & 0x3fffffffu;
     if (h->epoch == 0u) h->epoch = 1u;
     const bool rec = h->prof && h->prof_steps < h->prof_max;
@@ -129,7 +164,7 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
     const bool big = G.P > kTableSmemMax;
     const bool sn = fused && G.drag_model == 1;            // the unfused pass carries no push: one instantiation
 #define LCS_LAUNCH_TP(F, B, D, GRID) \
-    k_tile_pass<F, B, D><<<GRID, kBlock, smem, h->stream>>>(G, h->S, h->Snd, h->T, h->fluid4, dt, h->epoch, h->slab_map)
+    k_tile_pass<F, B, D><<<GRID, kBlock, smem, h->stream>>>(G, S, h->Snd, h->T, h->fluid4, dt, h->epoch, M)
     if (fused) {
         if (big) { if (sn) LCS_LAUNCH_TP(true, true, 1, h->grid_fused); else LCS_LAUNCH_TP(true, true, 0, h->grid_fused); }
         else     { if (sn) LCS_LAUNCH_TP(true, false, 1, h->grid_fused); else LCS_LAUNCH_TP(true, false, 0, h->grid_fused); }
@@ -141,10 +176,10 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt)
     k_code_scan<<<G.P, 256, 0, h->stream>>>(G, h->T);
     k_table<<<(G.P + 7) / 8, 256, 0, h->stream>>>(G, h->T);
     if (rec) cudaEventRecord(ev[2], h->stream);
-    k_unpack<<<dim3((G.groups_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, h->S, h->Snd, h->T);
-    k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, 1);
+    k_unpack<<<dim3((G.groups_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, S, h->Snd, h->T);
+    k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, commit ? 1 : 0);     // (also resets the tile ticket for the next round)
     if (rec) { cudaEventRecord(ev[3], h->stream); ++h->prof_steps; }
-    h->pushed = false;
+    if (commit) h->pushed = false;
     return check_launch(h, 5);
 }
 
@@ -214,20 +249,20 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     h->T.n_total = reinterpret_cast<unsigned long long*>(w + L.misc + 48);
     h->prefix = reinterpret_cast<int64_t*>(w + L.prefix);
     h->stream = static_cast<cudaStream_t>(cuda_stream);
-    {   // tensor map of the slabs for the bulk tile loads: 2-D [8 fields][P*cap slots] of 8-byte words, rows `stride` apart
-        typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                      const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                      CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-        void* fn = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) { delete h; return LCS_ERR_CUDA; }
-        const cuuint64_t gdim[2] = {(cuuint64_t)P * (cuuint64_t)capacity, 8};
-        const cuuint64_t gstride[1] = {(cuuint64_t)(L.slab_f[1] - L.slab_f[0])};
-        const cuuint32_t box[2] = {(cuuint32_t)kTile, 8};
-        const cuuint32_t estr[2] = {1, 1};
-        if (reinterpret_cast<encode_fn>(fn)(&h->slab_map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, w + L.slab_f[0], gdim, gstride, box, estr,
-                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { delete h; return LCS_ERR_CUDA; }
+    if (!make_slab_map(&h->slab_map, w + L.slab_f[0], (size_t)P * (size_t)capacity, L.slab_f[1] - L.slab_f[0])) { delete h; return LCS_ERR_CUDA; }
+    h->rk2 = prm->enable_rk2 == 1;
+    if (h->rk2) {   // the RK2 groups: same stride and shape as the slabs, so the same tile pass moves them
+        const size_t st = L.slab_f[1] - L.slab_f[0];
+        for (int a = 0; a < 7; ++a) {
+            h->SB.f[a] = reinterpret_cast<double*>(w + L.rk2_b + a * st);
+            h->SC.f[a] = reinterpret_cast<double*>(w + L.rk2_c + a * st);
+        }
+        h->SB.id = reinterpret_cast<int64_t*>(w + L.rk2_b + 7 * st);
+        h->SC.id = reinterpret_cast<int64_t*>(w + L.rk2_c + 7 * st);
+        h->SB.code = h->SC.code = h->S.code;
+        if (!make_slab_map(&h->mapB, w + L.rk2_b, (size_t)P * (size_t)capacity, st) ||
+            !make_slab_map(&h->mapC, w + L.rk2_c, (size_t)P * (size_t)capacity, st)) { delete h; return LCS_ERR_CUDA; }
+        if (cudaMemsetAsync(w + L.rk2_b, 0, 16 * st, h->stream) != cudaSuccess) { delete h; return LCS_ERR_CUDA; }
     }
     {   // persistent grids: one wave of resident CTAs
         int dev = 0, sms = 0, occ_f = 0, occ_p = 0;
@@ -343,6 +378,27 @@ int lcs_migrate_sweeps(lcs_t* h)
         if (rc != LCS_OK) return rc;
     }
     return LCS_OK;
+}
+
+int lcs_step_rk2(lcs_t* h, double dt)
+{
+    if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
+    if (!h->rk2 || !h->have_fluid || !h->have_particles) return LCS_ERR_STATE;
+    if (h->sticky) return h->sticky;
+    const Geom& G = h->G;
+    const dim3 grid((G.tiles_per_sub + kPushWarps - 1) / kPushWarps, G.P);
+    // stage 1, then all 17 arrays migrate: three rounds of 8 with the same codes, the counts committed by the last one
+    k_rk2_stage<1><<<grid, 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->SB, h->SC, h->T, h->fluid4, dt);
+    int rc = check_launch(h);
+    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0, &h->S, &h->slab_map, false);
+    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0, &h->SB, &h->mapB, false);
+    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0, &h->SC, &h->mapC, true);
+    if (rc != LCS_OK) return rc;
+    // stage 2 consumes X0, V0, K1; only X, V, d, id are live afterwards: one round
+    k_rk2_stage<2><<<grid, 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->SB, h->SC, h->T, h->fluid4, dt);
+    rc = check_launch(h);
+    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0);
+    return rc;
 }
 
 int lcs_step_fused(lcs_t* h, double dt)

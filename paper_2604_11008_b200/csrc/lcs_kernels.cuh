@@ -1125,6 +1125,104 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
 }
 
 // ---------------------------------------------------------------------------------------------
+// The paper's two-stage RK2 (Heun) with one migration per stage (R-25).
+//   stage 1: K1 = (U(X0) - V0)/tau + g ; X1 = X0 + dt V0 ; V1 = V0 + dt K1 ; X0, V0, K1 kept in groups B and C
+//   stage 2: K2 = (U(X1) - V1)/tau + g ; X  = X0 + dt/2 (V0 + V1) ; V = V0 + dt/2 (K1 + K2)
+// tau = tau_p / f, f at the start of the stage.  Destination: per axis the minimum-image direction from the slab the
+// particle sits in to the owner of its new position (R-24's rule).  One warp per tile, unpipelined like k_push.
+// Group B = x0 y0 z0 vx0 vy0 vz0 k1x k1y (its eighth array holds k1y's bits), group C = k1z + 7 spare arrays.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int min_image_dir(double a, const Geom& G, int Pa, int n_a, int p_a, bool& jump)
+{
+    if (!(a >= 0.0 && a < G.L)) { jump = true; return 0; }
+    int ic = __double2int_rd(a * G.inv_dx);
+    ic = max(0, min(ic, G.N - 1));
+    int dd = ic / n_a - p_a;
+    if (Pa >= 3) {
+        if (dd > 1) dd -= Pa;
+        else if (dd < -1) dd += Pa;
+    }
+    if (dd < -1 || dd > 1) { jump = true; dd = dd < -1 ? -1 : 1; }
+    return dd;
+}
+
+__device__ __forceinline__ double wrap_once(double xu, const Geom& G)
+{
+    if (xu < 0.0) { xu = xu + G.L; if (xu >= G.L) xu = G.L_below; }
+    else if (xu >= G.L) xu = xu - G.L;
+    return xu;                                     // still outside [0, L): min_image_dir raises the jump
+}
+
+template <int kStage>
+__global__ void __launch_bounds__(32 * kPushWarps, 3)
+k_rk2_stage(Geom G, Slabs S, Slabs SB, Slabs SC, Tables T, const double* __restrict__ F4, double dt)
+{
+    const int s = blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t first = (uint32_t)(blockIdx.x * kPushWarps + warp) * kTile;
+    const uint32_t cnt_s = T.count[s];
+    if (first >= cnt_s) return;
+    const int px = s % G.Px, py = (s / G.Px) % G.Py, pz = s / (G.Px * G.Py);
+    const uint32_t nvalid = min((uint32_t)kTile, cnt_s - first);
+    const double hdt = 0.5 * dt;
+    bool jump = false;
+#pragma unroll 1
+    for (int r = 0; r < kRows; ++r) {
+        if (32u * r >= nvalid) break;
+        const bool valid = 32u * r + (uint32_t)lane < nvalid;
+        const uint32_t at = (uint32_t)s * (uint32_t)G.cap + first + min(32u * r + (uint32_t)lane, nvalid - 1u);
+        double x[3], v[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { x[a] = S.f[a][at]; v[a] = S.f[3 + a][at]; }
+        const double d = S.f[6][at];
+        Gath Q;
+        gather_issue(Q, F4, G.N, G.inv_dx, x[0], x[1], x[2], lane);
+        double tau = (G.K_tau * d) * d;
+        const Vec3 Uv = gather_reduce(Q, lane);
+        const double U[3] = {Uv.x, Uv.y, Uv.z};
+        if (G.drag_model == 1) tau = tau / drag_factor(d, v[0] - U[0], v[1] - U[1], v[2] - U[2], G.inv_nu);
+        const double g[3] = {G.gx, G.gy, G.gz};
+        double k[3], pos[3], vn[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) k[a] = (U[a] - v[a]) / tau + g[a];          // Eq. 6 + g (R-4)
+        if (kStage == 1) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                pos[a] = wrap_once(fma(dt, v[a], x[a]), G);                     // X1 = X0 + dt V0
+                vn[a] = fma(dt, k[a], v[a]);                                    // V1 = V0 + dt K1
+            }
+            if (valid) {
+#pragma unroll
+                for (int a = 0; a < 3; ++a) { SB.f[a][at] = x[a]; SB.f[3 + a][at] = v[a]; }
+                SB.f[6][at] = k[0];
+                SB.id[at] = __double_as_longlong(k[1]);
+                SC.f[0][at] = k[2];
+            }
+        } else {
+            double x0[3], v0[3], k1[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { x0[a] = SB.f[a][at]; v0[a] = SB.f[3 + a][at]; }
+            k1[0] = SB.f[6][at]; k1[1] = __longlong_as_double(SB.id[at]); k1[2] = SC.f[0][at];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                pos[a] = wrap_once(fma(hdt, v0[a] + v[a], x0[a]), G);           // X = X0 + dt/2 (V0 + V1)
+                vn[a] = fma(hdt, k1[a] + k[a], v0[a]);                          // V = V0 + dt/2 (K1 + K2)
+            }
+        }
+        bool jmp = false;
+        const int code = kStay + min_image_dir(pos[0], G, G.Px, G.nx, px, jmp) + 3 * min_image_dir(pos[1], G, G.Py, G.ny, py, jmp)
+                       + 9 * min_image_dir(pos[2], G, G.Pz, G.nz, pz, jmp);
+        if (valid) {
+            jump |= jmp;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { S.f[a][at] = pos[a]; S.f[3 + a][at] = vn[a]; }
+            S.code[at] = (uint8_t)code;
+        }
+    }
+    if (jump) raise(T.status, -5);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Axis-by-axis exchange (R-24): destination code along ONE axis from the particle's current
 // position relative to the slab it sits in (minimum-image difference of subdomain indices), written
 // as the code byte the unfused tile pass consumes.  One thread per slot.

@@ -43,12 +43,13 @@ def assert_state_close(got, want, tag=""):
         assert ulps(got[k], want[k]) == 0, (tag, k, "ulp distance", ulps(got[k], want[k]))
 
 
-def make_pair(torch, oracle_lib, N, P, cap, fluid, parts, g=(0.0, 0.0, 0.0), rho=1000.0, send_capacity=0, drag_model=0):
+def make_pair(torch, oracle_lib, N, P, cap, fluid, parts, g=(0.0, 0.0, 0.0), rho=1000.0, send_capacity=0, drag_model=0,
+              rk2=False):
     from paper_2604_11008_b200 import LCS
     o = oracle_lib.Oracle(N, *P, cap, g=g, rho_ratio=rho, drag_model=drag_model)
     o.set_fluid(*fluid)
     rc = o.set_particles(*(parts[k] for k in F8))
-    dev = LCS(N, *P, cap, g=g, rho_ratio=rho, send_capacity=send_capacity, drag_model=drag_model)
+    dev = LCS(N, *P, cap, g=g, rho_ratio=rho, send_capacity=send_capacity, drag_model=drag_model, rk2=rk2)
     df = [torch.from_numpy(np.ascontiguousarray(f, dtype=np.float64)).cuda() for f in fluid]
     dev.set_fluid(*df)
     dp = to_dev(torch, parts)
@@ -244,6 +245,48 @@ def test_axis_sweeps_match_oracle(torch_cuda, oracle_lib, P, N):
     for k in F8 + ("counts",):
         assert np.array_equal(before[k], after[k])
     dev.close(); dev_direct.close()
+
+
+@pytest.mark.parametrize("P,drag_model", [((2, 2, 2), 0), ((3, 2, 1), 0), ((1, 1, 1), 0), ((4, 4, 2), 1), ((2, 2, 2), 1)])
+def test_two_stage_rk2_matches_oracle(torch_cuda, oracle_lib, P, drag_model):
+    """lcs_step_rk2 (the paper's two-stage RK2 with a migration of all 17 arrays after stage 1 and one after stage 2;
+    SURVEY 8(f) NEXT #1, DESIGN R-25) against the oracle: ids, order, counts exact, state 0 ulp, in the paper's regime
+    dt/tau <= 0.5 (300 um droplets, tau = 1.3 s) with a non-uniform field so that stage 2 really depends on X0, V0, K1."""
+    from workloads import gen
+    N = 24
+    cfg = gen.scaled_config(gen.get_config("Tiny"), n=24000, N=N)
+    wl = gen.make_workload(cfg)
+    fluid = [wl[k].numpy() for k in "uvw"]
+    parts = {k: v.numpy().copy() for k, v in wl["particles"].items()}
+    rng = np.random.default_rng(17)
+    parts["d"] = 300e-6 * np.exp(0.2 * rng.standard_normal(cfg["n"]))
+    for k in ("vx", "vy", "vz"):
+        parts[k] = parts[k] + 1.5 * rng.standard_normal(cfg["n"])
+    nP = P[0] * P[1] * P[2]
+    cap = 2 * (int(2.5 * cfg["n"] / nP) // 2 + 64)
+    dt = 0.1 if drag_model == 0 else 0.04
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, N, P, cap, fluid, parts, g=(0.0, 0.0, -9.81), drag_model=drag_model,
+                           rk2=True)
+    assert rc == 0
+    total_moved = 0
+    for step in range(4):
+        assert o.step_rk2(dt) == 0
+        dev.step_rk2(dt)
+        assert dev.get_status() == (0, cfg["n"], o.n_migrated_last)
+        total_moved += o.n_migrated_last
+        compare_packed(dev, o, f"rk2 P={P} step {step}")
+    assert nP == 1 or total_moved > 0
+    # the exponential step still works on the same handle afterwards (the RK2 arrays are scratch between the stages)
+    assert o.step(dt) == 0
+    dev.step_fused(dt)
+    compare_packed(dev, o, "fused after rk2")
+    dev.close()
+    # without enable_rk2 the call is a state error
+    from paper_2604_11008_b200 import LCS, LcsError
+    plain = LCS(N, *P, cap)
+    with pytest.raises(LcsError):
+        plain.step_rk2(dt)
+    plain.close()
 
 
 def test_all_27_codes_hand_placed(torch_cuda, oracle_lib):
