@@ -216,7 +216,7 @@ def run_cuda(args):
     cfg, wl = build_workload(args.workload, dev)
     n, N = cfg["n"], cfg["N"]
     P = cfg["P"][0] * cfg["P"][1] * cfg["P"][2]
-    lcs = LCS(N, *cfg["P"], cfg["capacity"], g=cfg["g"], drag_model=args.drag_model, device=dev)
+    lcs = LCS(N, *cfg["P"], cfg["capacity"], g=cfg["g"], drag_model=args.drag_model, rk2=args.rk2, device=dev)
     lcs.set_fluid(wl["u"], wl["v"], wl["w"])
     parts = wl["particles"]
     lcs.set_particles(*(parts[k] for k in F8))
@@ -283,6 +283,21 @@ def run_cuda(args):
             print(f"bench.py: sweep step failed: sticky status {err_s}, total {n_tot_s}", file=sys.stderr)
             return 3
         sweeps_ms = float(np.median([e[0].elapsed_time(e[1]) for e in evs]))
+        # the paper's two-stage RK2, in ITS regime: dt = 0.4 tau_p of the smallest droplet (explicit
+        # RK2 diverges at the dt of BASELINE.json's configs, R-1), so very few particles migrate per stage
+        rk2_ms = None
+        if args.rk2:
+            d_min = float(torch.min(wl["particles"]["d"]).item())       # the smallest droplet sets the explicit limit
+            dt_rk2 = 0.4 * 1000.0 * d_min * d_min / (18.0 * 1.5e-5)
+            evr = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(3)]
+            for k in range(3):
+                evr[k][0].record(); lcs.step_rk2(dt_rk2); evr[k][1].record()
+            torch.cuda.synchronize()
+            err_r, n_tot_r, n_mig_r = lcs.get_status()
+            if (err_r or n_tot_r != n) and not os.environ.get("LCS_BENCH_ABLATION"):
+                print(f"bench.py: rk2 step failed: sticky status {err_r}, total {n_tot_r}", file=sys.stderr)
+                return 3
+            rk2_ms = float(np.median([e[0].elapsed_time(e[1]) for e in evr]))
         # per-step fluid refresh (first half): lcs_set_fluid = the repack of the three x-fastest
         # arrays into the internal (u,v,w,0) z-fastest records, as a coupled solver would call it every step
         evf = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(3)]
@@ -307,6 +322,10 @@ def run_cuda(args):
                         "migrant_fraction": m_u},
             "migrate_sweeps": {"call": "lcs_migrate_sweeps", "ms": sweeps_ms, "particles_per_s": n / (sweeps_ms * 1e-3),
                                "note": "x, y, z sweeps: three classify + unfused tile pass + scan + table + unpack rounds"},
+            "rk2": None if rk2_ms is None else {
+                "call": "lcs_step_rk2", "ms": rk2_ms, "particles_per_s": n / (rk2_ms * 1e-3), "dt": dt_rk2,
+                "migrant_fraction_second_migration": n_mig_r / n,
+                "note": "two stages; 17 arrays migrate after stage 1 (three rounds of the 8-array tile pass), 8 after stage 2"},
             "set_fluid": {"call": "lcs_set_fluid", "ms": fluid_ms,
                           "GBps": (24.0 + 32.0) * N ** 3 / (fluid_ms * 1e-3) / 1e9,
                           "note": "reads 24 B and writes 32 B per cell; off the timed step (the fluid is frozen)"},
@@ -410,6 +429,8 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1 << 21, help="--impl reference: particles per timed step")
     ap.add_argument("--drag-model", type=int, default=0, choices=[0, 1],
                     help="0: Stokes drag (BASELINE.json's configs); 1: f = 1 + 0.15 Re^0.687 (SURVEY 8(f) NEXT #2)")
+    ap.add_argument("--rk2", action="store_true",
+                    help="also time lcs_step_rk2 (SURVEY 8(f) NEXT #1); reserves 16 more arrays of P*capacity doubles")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), reported as roofline.traffic")
     args = ap.parse_args()
