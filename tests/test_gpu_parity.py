@@ -339,6 +339,17 @@ def test_edge_cases(torch_cuda, oracle_lib):
     dev.particle_step(1.0); dev.migrate()
     assert dev.get_status() == (0, 0, 0)
     dev.close()
+    # empty box and a single particle through the sweeps and the two-stage RK2
+    for n in (0, 1):
+        parts = random_parts(rng, n, [0.3, 0.2, 0.1], d=3e-4)
+        o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, 64, (z, z, z), parts, rk2=True)
+        dev.particle_step(0.5); dev.migrate_sweeps()
+        assert o.push(0.5) == 0 and o.migrate_sweeps()[0] == 0
+        dev.step_rk2(0.25)
+        assert o.step_rk2(0.25) == 0
+        assert dev.get_status()[:2] == (0, n)
+        compare_packed(dev, o, f"sweeps + rk2, n = {n}")
+        dev.close()
 
 
 def test_sticky_errors(torch_cuda, oracle_lib):
