@@ -480,6 +480,33 @@ def test_stress_shape_sample(torch_cuda, oracle_lib):
 
 
 @pytest.mark.slow
+@pytest.mark.parametrize("name,steps", [("Medium", None), ("Clustered", 3), ("Large", 1), ("Stress", 1)])
+def test_full_size_free_running_P2(torch_cuda, oracle_lib, name, steps):
+    """BASELINE.json's configurations at FULL size run freely on both sides (protocol P2), every particle compared: final
+    ids, order and counts bit-identical, positions and velocities 0 ulp.  Medium (2,097,152 particles, 128^3, 4x4x4,
+    gravity): all its 100 steps.  Clustered (16.8 M, 4096 clumps): 3 steps.  Large (67.1 M, 512^3, 8x8x8): 1 step.
+    Stress (268 M, 1024^3, 30 % migrants): 1 step.  Bounded by single-core oracle time (10-30 s each, 3 min for Stress)."""
+    from workloads import gen
+    import psutil
+    cfg = gen.get_config(name)
+    if psutil.virtual_memory().available < 400 * cfg["n"] + 3 * 24 * cfg["N"] ** 3:
+        pytest.skip(f"{name} at full size needs more host memory for the oracle")
+    if steps is not None:
+        cfg["steps"] = steps
+    wl = gen.make_workload(cfg, device="cuda")
+    fluid = [wl[k].cpu().numpy() for k in "uvw"]
+    parts = {k: v.cpu().numpy() for k, v in wl["particles"].items()}
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, cfg["N"], cfg["P"], cfg["capacity"], fluid, parts, g=cfg["g"])
+    assert rc == 0
+    for step in range(cfg["steps"]):
+        assert o.step(cfg["dt"]) == 0, step
+        dev.step_fused(cfg["dt"])
+    assert dev.get_status() == (0, cfg["n"], o.n_migrated_last)
+    compare_packed(dev, o, f"{name}, {cfg['steps']} steps, free running")
+    dev.close()
+
+
+@pytest.mark.slow
 @pytest.mark.parametrize("name", ["Clustered", "Large", "Stress"])
 def test_full_size_properties(torch_cuda, oracle_lib, name):
     """BASELINE.json's configurations at FULL size (Large: 2^26 particles, 512^3, 8x8x8, capacity 1.25x; Stress: 2^28
