@@ -325,7 +325,7 @@ def run_cuda(args):
             "rk2": None if rk2_ms is None else {
                 "call": "lcs_step_rk2", "ms": rk2_ms, "particles_per_s": n / (rk2_ms * 1e-3), "dt": dt_rk2,
                 "migrant_fraction_second_migration": n_mig_r / n,
-                "note": "two stages; 17 arrays migrate after stage 1 (three rounds of the 8-array tile pass), 8 after stage 2"},
+                "note": "two stages; 16 arrays migrate after stage 1 (two rounds of the 8-array tile pass), 8 after stage 2"},
             "set_fluid": {"call": "lcs_set_fluid", "ms": fluid_ms,
                           "GBps": (24.0 + 32.0) * N ** 3 / (fluid_ms * 1e-3) / 1e9,
                           "note": "reads 24 B and writes 32 B per cell; off the timed step (the fluid is frozen)"},
@@ -430,7 +430,7 @@ def main():
     ap.add_argument("--drag-model", type=int, default=0, choices=[0, 1],
                     help="0: Stokes drag (BASELINE.json's configs); 1: f = 1 + 0.15 Re^0.687 (SURVEY 8(f) NEXT #2)")
     ap.add_argument("--rk2", action="store_true",
-                    help="also time lcs_step_rk2 (SURVEY 8(f) NEXT #1); reserves 16 more arrays of P*capacity doubles")
+                    help="also time lcs_step_rk2 (SURVEY 8(f) NEXT #1); reserves 8 more arrays of P*capacity doubles")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), reported as roofline.traffic")
     args = ap.parse_args()

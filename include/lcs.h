@@ -56,8 +56,8 @@ typedef struct {
     int32_t drag_model;     /* 0: Stokes drag, f = 1 (the hot path of BASELINE.json's configs);
                                1: f = 1 + 0.15 Re_p^0.687, Re_p = d|V-U|/nu (Eq. 7-8),
                                   frozen at the start of the step, tau_eff = tau_p / f (DESIGN R-23)  */
-    int32_t enable_rk2;     /* 1: reserve the 9 extra arrays of the paper's two-stage RK2 in the workspace (16 arrays of
-                               P*capacity doubles: they move in groups of 8) so that lcs_step_rk2 can be called     */
+    int32_t enable_rk2;     /* 1: reserve the extra arrays of the paper's two-stage RK2 in the workspace (one group of 8
+                               arrays of P*capacity doubles: X0, K1 and two spare) so that lcs_step_rk2 can be called */
 } lcs_params;
 
 /* Bytes of device workspace lcs_create needs; 0 if the arguments are invalid. */
@@ -102,7 +102,7 @@ int lcs_migrate(lcs_t* h);
 
 /* The paper's own integrator: explicit two-stage RK2 (Heun) with one particle communication per stage (PAPER.md:64,
  * :150-164, :175-177; R-25).  Stage 1: K1 = (U(X0)-V0)/tau + g, X1 = X0 + dt V0, V1 = V0 + dt K1; X0, V0, K1 are
- * kept, all 17 arrays (X, V, X0, V0, K1, d, id) migrate.  Stage 2: K2 = (U(X1)-V1)/tau + g, X = X0 + dt/2 (V0+V1),
+ * kept, everything live between the stages migrates (the paper's 17 arrays; here V1 is recomputed, so 14 + 2 spare).  Stage 2: K2 = (U(X1)-V1)/tau + g, X = X0 + dt/2 (V0+V1),
  * V = V0 + dt/2 (K1+K2); migrate.  tau = tau_p / f with f at the start of each stage (drag_model).  Explicit: meant for
  * dt/tau_p <= 0.5 (the paper's regime); BASELINE.json's configs need lcs_step_fused.  Needs lcs_params.enable_rk2 = 1
  * (LCS_ERR_STATE otherwise).  lcs_get_status then reports the migrants of the second migration. */

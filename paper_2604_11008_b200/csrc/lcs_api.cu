@@ -33,8 +33,8 @@ struct lcs_handle {
     int grid_fused, grid_pack;         // persistent grid sizes of the tile pass
     CUtensorMap slab_map;              // 2-D view [8 fields][P*cap slots] of the slabs, box 8 x kTile (bulk tile loads)
     bool rk2;                          // the 9 extra arrays of the two-stage RK2 exist (lcs_params.enable_rk2)
-    Slabs SB, SC;                      // RK2: x0 y0 z0 vx0 vy0 vz0 k1x k1y | k1z + 7 spare arrays (groups of 8 for the tile pass)
-    CUtensorMap mapB, mapC;
+    Slabs SB;                          // RK2: x0 y0 z0 k1x k1y k1z + 2 spare arrays (a group of 8 for the tile pass)
+    CUtensorMap mapB;
     size_t gacc_bytes;
 };
 
@@ -45,7 +45,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t slab_f[7], slab_id, slab_code;
-    size_t rk2_b, rk2_c;               // RK2 groups B and C: 8 arrays each, stride as the slabs (0 = absent)
+    size_t rk2_b;                      // RK2 group B: 8 arrays, stride as the slabs (0 = absent)
     size_t pool, pool_bytes, fluid4;
     size_t count, cnt, recv_off, new_count, desc, gacc, gacc_bytes, tile_start, tile_cnt, group_excl, misc, prefix;
     size_t total;
@@ -86,11 +86,8 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     for (int a = 0; a < 7; ++a) { L.slab_f[a] = off; off = align_up(off + slots * 8); }
     L.slab_id = off;   off = align_up(off + slots * 8);
     L.slab_code = off; off = align_up(off + slots);
-    L.rk2_b = L.rk2_c = 0;
-    if (prm->enable_rk2) {
-        L.rk2_b = off; off += 8 * align_up(slots * 8);
-        L.rk2_c = off; off += 8 * align_up(slots * 8);
-    }
+    L.rk2_b = 0;
+    if (prm->enable_rk2) { L.rk2_b = off; off += 8 * align_up(slots * 8); }
     // send pool: 8 arrays of P*send_cap slots; doubles as lcs_set_particles scratch
     const size_t send_bytes = 8 * align_up(P * (size_t)L.send_cap * 8);
     const size_t set_tiles = (slots + kSetTile - 1) / kSetTile;
@@ -251,18 +248,13 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     h->stream = static_cast<cudaStream_t>(cuda_stream);
     if (!make_slab_map(&h->slab_map, w + L.slab_f[0], (size_t)P * (size_t)capacity, L.slab_f[1] - L.slab_f[0])) { delete h; return LCS_ERR_CUDA; }
     h->rk2 = prm->enable_rk2 == 1;
-    if (h->rk2) {   // the RK2 groups: same stride and shape as the slabs, so the same tile pass moves them
+    if (h->rk2) {   // the RK2 group: same stride and shape as the slabs, so the same tile pass moves it
         const size_t st = L.slab_f[1] - L.slab_f[0];
-        for (int a = 0; a < 7; ++a) {
-            h->SB.f[a] = reinterpret_cast<double*>(w + L.rk2_b + a * st);
-            h->SC.f[a] = reinterpret_cast<double*>(w + L.rk2_c + a * st);
-        }
+        for (int a = 0; a < 7; ++a) h->SB.f[a] = reinterpret_cast<double*>(w + L.rk2_b + a * st);
         h->SB.id = reinterpret_cast<int64_t*>(w + L.rk2_b + 7 * st);
-        h->SC.id = reinterpret_cast<int64_t*>(w + L.rk2_c + 7 * st);
-        h->SB.code = h->SC.code = h->S.code;
-        if (!make_slab_map(&h->mapB, w + L.rk2_b, (size_t)P * (size_t)capacity, st) ||
-            !make_slab_map(&h->mapC, w + L.rk2_c, (size_t)P * (size_t)capacity, st)) { delete h; return LCS_ERR_CUDA; }
-        if (cudaMemsetAsync(w + L.rk2_b, 0, 16 * st, h->stream) != cudaSuccess) { delete h; return LCS_ERR_CUDA; }
+        h->SB.code = h->S.code;
+        if (!make_slab_map(&h->mapB, w + L.rk2_b, (size_t)P * (size_t)capacity, st)) { delete h; return LCS_ERR_CUDA; }
+        if (cudaMemsetAsync(w + L.rk2_b, 0, 8 * st, h->stream) != cudaSuccess) { delete h; return LCS_ERR_CUDA; }
     }
     {   // persistent grids: one wave of resident CTAs
         int dev = 0, sms = 0, occ_f = 0, occ_p = 0;
@@ -387,15 +379,15 @@ int lcs_step_rk2(lcs_t* h, double dt)
     if (h->sticky) return h->sticky;
     const Geom& G = h->G;
     const dim3 grid((G.tiles_per_sub + kPushWarps - 1) / kPushWarps, G.P);
-    // stage 1, then all 17 arrays migrate: three rounds of 8 with the same codes, the counts committed by the last one
-    k_rk2_stage<1><<<grid, 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->SB, h->SC, h->T, h->fluid4, dt);
+    // stage 1, then everything that is live between the stages migrates: two rounds of 8 arrays with the same codes
+    // (slabs: X1, V0, d, id; group B: X0, K1), the counts committed by the second one
+    k_rk2_stage<1><<<grid, 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->SB, h->T, h->fluid4, dt);
     int rc = check_launch(h);
     if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0, &h->S, &h->slab_map, false);
-    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0, &h->SB, &h->mapB, false);
-    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0, &h->SC, &h->mapC, true);
+    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0, &h->SB, &h->mapB, true);
     if (rc != LCS_OK) return rc;
-    // stage 2 consumes X0, V0, K1; only X, V, d, id are live afterwards: one round
-    k_rk2_stage<2><<<grid, 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->SB, h->SC, h->T, h->fluid4, dt);
+    // stage 2 consumes X0, K1; only X, V, d, id are live afterwards: one round
+    k_rk2_stage<2><<<grid, 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->SB, h->T, h->fluid4, dt);
     rc = check_launch(h);
     if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0);
     return rc;

@@ -1126,11 +1126,13 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
 
 // ---------------------------------------------------------------------------------------------
 // The paper's two-stage RK2 (Heun) with one migration per stage (R-25).
-//   stage 1: K1 = (U(X0) - V0)/tau + g ; X1 = X0 + dt V0 ; V1 = V0 + dt K1 ; X0, V0, K1 kept in groups B and C
-//   stage 2: K2 = (U(X1) - V1)/tau + g ; X  = X0 + dt/2 (V0 + V1) ; V = V0 + dt/2 (K1 + K2)
+//   stage 1: K1 = (U(X0) - V0)/tau + g ; X1 = X0 + dt V0 ; X0 and K1 kept in group B, V0 stays in the slabs
+//   stage 2: V1 = V0 + dt K1 (recomputed: the same fma the oracle stored) ; K2 = (U(X1) - V1)/tau + g ;
+//            X = X0 + dt/2 (V0 + V1) ; V = V0 + dt/2 (K1 + K2)
 // tau = tau_p / f, f at the start of the stage.  Destination: per axis the minimum-image direction from the slab the
 // particle sits in to the owner of its new position (R-24's rule).  One warp per tile, unpipelined like k_push.
-// Group B = x0 y0 z0 vx0 vy0 vz0 k1x k1y (its eighth array holds k1y's bits), group C = k1z + 7 spare arrays.
+// Of the paper's 17 arrays 14 travel between the stages (X1, V0, d, id in the slabs; X0, K1 in group B, whose two
+// spare arrays travel too): V1 never exists in memory.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ int min_image_dir(double a, const Geom& G, int Pa, int n_a, int p_a, bool& jump)
 {
@@ -1155,7 +1157,7 @@ __device__ __forceinline__ double wrap_once(double xu, const Geom& G)
 
 template <int kStage>
 __global__ void __launch_bounds__(32 * kPushWarps, 3)
-k_rk2_stage(Geom G, Slabs S, Slabs SB, Slabs SC, Tables T, const double* __restrict__ F4, double dt)
+k_rk2_stage(Geom G, Slabs S, Slabs SB, Tables T, const double* __restrict__ F4, double dt)
 {
     const int s = blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -1171,12 +1173,16 @@ k_rk2_stage(Geom G, Slabs S, Slabs SB, Slabs SC, Tables T, const double* __restr
         if (32u * r >= nvalid) break;
         const bool valid = 32u * r + (uint32_t)lane < nvalid;
         const uint32_t at = (uint32_t)s * (uint32_t)G.cap + first + min(32u * r + (uint32_t)lane, nvalid - 1u);
-        double x[3], v[3];
+        double x[3], v0[3], v[3], k1[3];
 #pragma unroll
-        for (int a = 0; a < 3; ++a) { x[a] = S.f[a][at]; v[a] = S.f[3 + a][at]; }
+        for (int a = 0; a < 3; ++a) { x[a] = S.f[a][at]; v0[a] = S.f[3 + a][at]; v[a] = v0[a]; k1[a] = 0.0; }
         const double d = S.f[6][at];
         Gath Q;
         gather_issue(Q, F4, G.N, G.inv_dx, x[0], x[1], x[2], lane);
+        if (kStage == 2) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { k1[a] = SB.f[3 + a][at]; v[a] = fma(dt, k1[a], v0[a]); }   // V1, recomputed (R-25)
+        }
         double tau = (G.K_tau * d) * d;
         const Vec3 Uv = gather_reduce(Q, lane);
         const double U[3] = {Uv.x, Uv.y, Uv.z};
@@ -1188,24 +1194,18 @@ k_rk2_stage(Geom G, Slabs S, Slabs SB, Slabs SC, Tables T, const double* __restr
         if (kStage == 1) {
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                pos[a] = wrap_once(fma(dt, v[a], x[a]), G);                     // X1 = X0 + dt V0
-                vn[a] = fma(dt, k[a], v[a]);                                    // V1 = V0 + dt K1
+                pos[a] = wrap_once(fma(dt, v0[a], x[a]), G);                    // X1 = X0 + dt V0
+                vn[a] = v0[a];                                                  // V0 stays; V1 = V0 + dt K1 is recomputed
             }
             if (valid) {
 #pragma unroll
-                for (int a = 0; a < 3; ++a) { SB.f[a][at] = x[a]; SB.f[3 + a][at] = v[a]; }
-                SB.f[6][at] = k[0];
-                SB.id[at] = __double_as_longlong(k[1]);
-                SC.f[0][at] = k[2];
+                for (int a = 0; a < 3; ++a) { SB.f[a][at] = x[a]; SB.f[3 + a][at] = k[a]; }
             }
         } else {
-            double x0[3], v0[3], k1[3];
-#pragma unroll
-            for (int a = 0; a < 3; ++a) { x0[a] = SB.f[a][at]; v0[a] = SB.f[3 + a][at]; }
-            k1[0] = SB.f[6][at]; k1[1] = __longlong_as_double(SB.id[at]); k1[2] = SC.f[0][at];
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                pos[a] = wrap_once(fma(hdt, v0[a] + v[a], x0[a]), G);           // X = X0 + dt/2 (V0 + V1)
+                const double x0 = SB.f[a][at];
+                pos[a] = wrap_once(fma(hdt, v0[a] + v[a], x0), G);              // X = X0 + dt/2 (V0 + V1)
                 vn[a] = fma(hdt, k1[a] + k[a], v0[a]);                          // V = V0 + dt/2 (K1 + K2)
             }
         }
@@ -1215,7 +1215,7 @@ k_rk2_stage(Geom G, Slabs S, Slabs SB, Slabs SC, Tables T, const double* __restr
         if (valid) {
             jump |= jmp;
 #pragma unroll
-            for (int a = 0; a < 3; ++a) { S.f[a][at] = pos[a]; S.f[3 + a][at] = vn[a]; }
+            for (int a = 0; a < 3; ++a) { S.f[a][at] = pos[a]; if (kStage == 2) S.f[3 + a][at] = vn[a]; }
             S.code[at] = (uint8_t)code;
         }
     }
