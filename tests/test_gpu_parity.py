@@ -493,10 +493,23 @@ def test_full_size_free_running_P2(torch_cuda, oracle_lib, name, steps):
         pytest.skip(f"{name} at full size needs more host memory for the oracle")
     if steps is not None:
         cfg["steps"] = steps
+    import gc
+    gc.collect()
+    torch_cuda.cuda.empty_cache()                      # the cached blocks of earlier tests count against this one
+    nP = cfg["P"][0] * cfg["P"][1] * cfg["P"][2]
+    need_dev = 97 * nP * cfg["capacity"] + 56 * cfg["N"] ** 3 + 80 * cfg["n"]
+    if torch_cuda.cuda.mem_get_info()[0] < need_dev:
+        pytest.skip(f"{name} at full size needs {need_dev / 2**30:.0f} GiB of free device memory")
     wl = gen.make_workload(cfg, device="cuda")
     fluid = [wl[k].cpu().numpy() for k in "uvw"]
     parts = {k: v.cpu().numpy() for k, v in wl["particles"].items()}
-    o, dev, rc = make_pair(torch_cuda, oracle_lib, cfg["N"], cfg["P"], cfg["capacity"], fluid, parts, g=cfg["g"])
+    del wl
+    gc.collect()
+    torch_cuda.cuda.empty_cache()
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, cfg["N"], cfg["P"], cfg["capacity"], fluid, parts, g=cfg["g"],
+                           send_capacity=cfg["capacity"] // 2)
+    gc.collect()
+    torch_cuda.cuda.empty_cache()
     assert rc == 0
     for step in range(cfg["steps"]):
         assert o.step(cfg["dt"]) == 0, step
@@ -519,7 +532,10 @@ def test_full_size_properties(torch_cuda, oracle_lib, name):
     n, N, P = cfg["n"], cfg["N"], cfg["P"]
     nP = P[0] * P[1] * P[2]
     # Stress needs about 140 GiB of device memory and 75 GB of host memory (two copies of the 1024^3 field)
+    import gc
     import psutil
+    gc.collect()
+    torch.cuda.empty_cache()                           # the cached blocks of earlier tests count against this one
     need_dev = 97 * nP * cfg["capacity"] + 56 * N ** 3 + 144 * n      # workspace + input field + particle copies
     if torch.cuda.mem_get_info()[0] < need_dev or psutil.virtual_memory().available < 3 * 24 * N ** 3:
         pytest.skip(f"{name} at full size needs {need_dev / 2**30:.0f} GiB of free device memory")
