@@ -84,7 +84,8 @@ class ClockSampler:
             self.thread = threading.Thread(target=poll, daemon=True)
             self.thread.start()
             return
-        except Exception:
+        except Exception as exc:
+            print(f"bench.py: NVML polling unavailable ({exc!r}); falling back to nvidia-smi", file=sys.stderr)
             self.thread = None
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
