@@ -65,7 +65,7 @@ size_t lcs_workspace_bytes(int N, int Px, int Py, int Pz, int64_t capacity, cons
 
 /* Create a handle.  N: fluid grid points per axis (2 <= N <= 1625, divisible by Px, Py and Pz);
  * Px, Py, Pz: 1..1024 each, Px*Py*Pz <= 8192; capacity: particle slots per subdomain slab (it must
- * be even, so that slab bases and tile runs stay 16-byte aligned, and P*capacity < 2^32: slots are
+ * be even, so that slab bases and tile runs stay 16-byte aligned, and P*capacity < 2^31: slots are
  * 32-bit indices); LCS_ERR_INVALID_ARG otherwise.  d_workspace: device block of at
  * least lcs_workspace_bytes(), 256-byte aligned, borrowed until lcs_destroy; cuda_stream: a
  * cudaStream_t (NULL = legacy default stream). */

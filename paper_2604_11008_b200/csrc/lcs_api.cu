@@ -63,7 +63,8 @@ bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* pr
     if (P > 8192) return false;                          // grid.y and shared-histogram limits
     if (cap < 2 || (cap & 1)) return false;               // even: slab bases stay 16-byte aligned
     if (cap > 0x7fffffff) return false;
-    if ((unsigned long long)P * (unsigned long long)cap >= (1ull << 32)) return false;   // 32-bit slot indices
+    if ((unsigned long long)P * (unsigned long long)cap >= (1ull << 31)) return false;   // slot indices are 32-bit, and the bulk
+                                                                                         // tensor copies take SIGNED 32-bit coordinates
     if (prm->send_capacity < 0 || (prm->send_capacity & 1) || prm->send_capacity > cap) return false;
     if (!(prm->nu > 0.0) || !(prm->rho_ratio > 0.0)) return false;
     if (prm->drag_model != 0 && prm->drag_model != 1) return false;

@@ -366,7 +366,7 @@ k_repack_fluid(int N, const double* __restrict__ u, const double* __restrict__ v
 //   larger ticket, which resolve after it has published -- so loading a tile early is safe too.
 //   All per-tile integer divisions are replaced by tables built once per CTA in shared memory or by
 //   float reciprocals (prefetch shares); the ticket -> (s,t) map is an incremental search from the
-//   previous subdomain; particle slots are 32-bit indices (P*cap < 2^32 is checked at lcs_create).
+//   previous subdomain; particle slots are 32-bit indices (P*cap < 2^31 is checked at lcs_create).
 // ---------------------------------------------------------------------------------------------
 #ifndef LCS_NBUF
 #define LCS_NBUF 3
@@ -922,7 +922,7 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             if (pend.n_mig) {
                 const bool fits = (long long)excl_mig + (long long)pend.n_mig <= G.send_cap;
                 if (!fits && lane == 0) raise(T.status, -4);
-                const uint32_t sendbase = (uint32_t)s * (uint32_t)G.send_cap + excl_mig;      // P*send_cap <= P*cap < 2^32
+                const uint32_t sendbase = (uint32_t)s * (uint32_t)G.send_cap + excl_mig;      // P*send_cap <= P*cap < 2^31
                 for (uint32_t a0 = 0; a0 < pend.n_mig; a0 += 32) {
                     const uint32_t a = a0 + lane;
                     const bool ok = a < pend.n_mig;

@@ -45,6 +45,7 @@ def test_version_and_workspace_size_checks(lib):
         (32, 2, 2, 2, 0, prm),                                   # no capacity
         (2048, 2, 2, 2, 4096, prm),                              # N > 1625 (32-bit record indices)
         (32, 2, 2, 2, 1 << 31, prm),                             # capacity beyond 2^31 - 1
+        (32, 2, 2, 2, 1 << 28, prm),                             # P * capacity = 2^31: slot indices and copy coordinates
         (32, 2, 2, 2, 4096, LcsParams(0.0, 1000.0, (C.c_double * 3)(0, 0, 0), 0, 0, 0)),        # nu <= 0
         (32, 2, 2, 2, 4096, LcsParams(1.5e-5, 1000.0, (C.c_double * 3)(0, 0, 0), 0, 2, 0)),     # unknown drag model
         (32, 2, 2, 2, 4096, LcsParams(1.5e-5, 1000.0, (C.c_double * 3)(0, 0, 0), 4098, 0, 0)),  # send region > capacity
