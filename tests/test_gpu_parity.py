@@ -289,6 +289,34 @@ def test_two_stage_rk2_matches_oracle(torch_cuda, oracle_lib, P, drag_model):
     plain.close()
 
 
+def test_host_buffer_entry_point_matches_oracle(torch_cuda, oracle_lib):
+    """lcs_step_fused_host (pinned host arrays in, packed result and counts out: the end-to-end call bench.py times):
+    three chained steps, the output of one the input of the next, against the oracle."""
+    torch = torch_cuda
+    N, P = 16, (2, 2, 2)
+    rng = np.random.default_rng(42)
+    n = 30011
+    Ls = np.array([L / P[0], L / P[1], L / P[2]])
+    parts = random_parts(rng, n, 0.45 * Ls)
+    z = np.zeros(N ** 3)
+    cap = 2 * (int(1.6 * n / 8) // 2 + 200)
+    o, dev, _ = make_pair(torch, oracle_lib, N, P, cap, (z, z, z), parts)
+    dtypes = {k: (torch.int64 if k == "id" else torch.float64) for k in F8}
+    h_in = {k: torch.from_numpy(np.ascontiguousarray(parts[k])).pin_memory() for k in F8}
+    h_out = {k: torch.empty(n, dtype=dtypes[k]).pin_memory() for k in F8}
+    h_counts = torch.empty(8, dtype=torch.int64).pin_memory()
+    staging = torch.empty(64 * n + 8 * 8 + 16384, dtype=torch.uint8, device="cuda")
+    for step in range(3):
+        assert o.step(0.7) == 0
+        dev.step_fused_host(0.7, h_in, h_out, h_counts, staging)       # synchronises: the result is on the host
+        want = o.get_particles()
+        assert np.array_equal(h_counts.numpy(), want["counts"]), step
+        for k in F8:
+            assert np.array_equal(h_out[k].numpy(), want[k]), (step, k)
+        h_in, h_out = h_out, h_in
+    dev.close()
+
+
 def test_all_27_codes_hand_placed(torch_cuda, oracle_lib):
     for P in [(3, 3, 3), (2, 2, 2), (1, 2, 3), (1, 1, 1)]:
         N = 24
