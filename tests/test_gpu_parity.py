@@ -394,6 +394,13 @@ def test_sticky_errors(torch_cuda, oracle_lib):
     with pytest.raises(LcsError):
         dev.step_fused(1.0)
     dev.close()
+    # jump in the two-stage RK2 (minimum-image classification, five subdomains along x: two away is detectable)
+    z20 = np.zeros(20 ** 3)
+    o, dev, _ = make_pair(torch_cuda, oracle_lib, 20, (5, 1, 1), 16, (z20, z20, z20),
+                          one(vx=np.array([L / 5 * 2.2]), d=np.array([1.0])), rk2=True)
+    dev.step_rk2(1.0)
+    assert dev.get_status()[0] == LCS_ERR_JUMP and o.step_rk2(1.0) == oracle_lib.ERR_JUMP
+    dev.close()
     # non-finite
     o, dev, _ = make_pair(torch_cuda, oracle_lib, N, P, 16, (z, z, z), one(vx=np.array([np.nan])))
     dev.particle_step(1.0)
