@@ -29,8 +29,8 @@ sys.path.insert(0, ROOT)
 METRIC = "particles/s (fused push + prefix-scan migrate step)"
 F8 = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
 # DRAM bytes of one k_tile_pass<fused> launch from the committed ncu --set full capture (profiles/r1c_tile_pass_full.md):
-# 9.081168 GB read + 4.309614 GB written.  --traffic-bytes overrides it after a new capture.
-NCU_TRAFFIC_BYTES = {"Large": 9.081168e9 + 4.309614e9}
+# 9.079250 GB read + 4.307880 GB written.  --traffic-bytes overrides it after a new capture.
+NCU_TRAFFIC_BYTES = {"Large": 9.079250e9 + 4.307880e9}
 
 
 def measured_peak_hbm():
