@@ -222,7 +222,7 @@ def run_cuda(args):
     parts = wl["particles"]
     lcs.set_particles(*(parts[k] for k in F8))
     err, n_tot, _ = lcs.get_status()
-    if (err or n_tot != n) and not os.environ.get("LCS_BENCH_ABLATION"):   # ablation builds (-DLCS_X_*) compute wrong results on purpose
+    if (err or n_tot != n):
         print(f"bench.py: set_particles failed: status {err}, total {n_tot}", file=sys.stderr)
         return 3
     dt = cfg["dt"]
@@ -250,7 +250,7 @@ def run_cuda(args):
     launches = lcs.kernel_launches - launches0
     clocks = sampler.stop() if sampler else None
     err, n_tot, n_mig = lcs.get_status()
-    if (err or n_tot != n) and not os.environ.get("LCS_BENCH_ABLATION"):   # ablation builds (-DLCS_X_*) compute wrong results on purpose
+    if (err or n_tot != n):
         print(f"bench.py: step failed: sticky status {err}, total {n_tot}", file=sys.stderr)
         return 3
     ms_total = max_over_ranks(ms_total, dist, dev)
@@ -270,7 +270,7 @@ def run_cuda(args):
             ev[k][2].record()
         torch.cuda.synchronize()
         err_u, n_tot_u, n_mig_u = lcs.get_status()
-        if (err_u or n_tot_u != n) and not os.environ.get("LCS_BENCH_ABLATION"):
+        if (err_u or n_tot_u != n):
             print(f"bench.py: unfused step failed: sticky status {err_u}, total {n_tot_u}", file=sys.stderr)
             return 3
         # axis-by-axis exchange: lcs_particle_step + lcs_migrate_sweeps, the sweeps timed
@@ -280,7 +280,7 @@ def run_cuda(args):
             evs[k][0].record(); lcs.migrate_sweeps(); evs[k][1].record()
         torch.cuda.synchronize()
         err_s, n_tot_s, _ = lcs.get_status()
-        if (err_s or n_tot_s != n) and not os.environ.get("LCS_BENCH_ABLATION"):
+        if (err_s or n_tot_s != n):
             print(f"bench.py: sweep step failed: sticky status {err_s}, total {n_tot_s}", file=sys.stderr)
             return 3
         sweeps_ms = float(np.median([e[0].elapsed_time(e[1]) for e in evs]))
@@ -295,7 +295,7 @@ def run_cuda(args):
                 evr[k][0].record(); lcs.step_rk2(dt_rk2); evr[k][1].record()
             torch.cuda.synchronize()
             err_r, n_tot_r, n_mig_r = lcs.get_status()
-            if (err_r or n_tot_r != n) and not os.environ.get("LCS_BENCH_ABLATION"):
+            if (err_r or n_tot_r != n):
                 print(f"bench.py: rk2 step failed: sticky status {err_r}, total {n_tot_r}", file=sys.stderr)
                 return 3
             rk2_ms = float(np.median([e[0].elapsed_time(e[1]) for e in evr]))
@@ -344,7 +344,7 @@ def run_cuda(args):
         for k in F8:
             h_in[k].copy_(state[k])
         del state
-        staging = torch.empty(64 * n + 8 * P + 16384, dtype=torch.uint8, device=dev)
+        staging = torch.empty(lcs.staging_bytes(n), dtype=torch.uint8, device=dev)
         lcs.step_fused_host(dt, h_in, h_out, h_counts, staging)       # warm-up
         barrier()
         t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)

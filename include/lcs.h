@@ -22,8 +22,13 @@
  *  - Return value: 0 = LCS_OK, negative = error found on the host at call time.  Errors found on
  *    the device are sticky in a status word that lcs_get_status reads (capacity overflow, a
  *    particle that moved more than one subdomain or became non-finite, an input position outside
- *    [0,L)).  After a sticky error memory safety still holds, particle contents are unspecified
- *    and every further call returns that code.  (The paper is silent on errors: DESIGN R-16/17.)
+ *    [0,L)).  After a sticky error memory safety still holds and particle contents are unspecified.
+ *    The calls never synchronise, so the host learns of a sticky error only through lcs_get_status:
+ *    once lcs_get_status has returned it, every further stepping call (lcs_particle_step,
+ *    lcs_migrate, lcs_migrate_sweeps, lcs_step_fused, lcs_step_rk2, lcs_step_fused_host) returns
+ *    that code without doing work, until lcs_set_particles loads a fresh particle set.  A caller
+ *    that never polls keeps stepping on unspecified contents.  (The paper is silent on errors:
+ *    DESIGN R-16/17.)
  */
 #ifndef LCS_B200_H
 #define LCS_B200_H
@@ -42,6 +47,7 @@ extern "C" {
 #define LCS_ERR_CAPACITY     (-4)   /* sticky: a receiver slab or a send region overflowed        */
 #define LCS_ERR_JUMP         (-5)   /* sticky: displacement > one subdomain, or non-finite        */
 #define LCS_ERR_RANGE        (-6)   /* sticky: lcs_set_particles saw a position outside [0, L)     */
+#define LCS_ERR_NOMEM        (-7)   /* host memory for the handle could not be allocated           */
 
 #define LCS_STAY_CODE 13
 
@@ -81,7 +87,8 @@ int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* 
 /* Load n particles given in any order; they are binned stably (input order kept inside each
  * slab) into the subdomain that contains them, all codes = stay.  Copies.  Positions must lie in
  * [0, L) (else sticky LCS_ERR_RANGE); a slab that would exceed capacity -> sticky LCS_ERR_CAPACITY.
- * PAPER.md:47 (3-D decomposition), DESIGN R-12. */
+ * LCS_ERR_INVALID_ARG for n < 0, n > P*capacity, a null pointer (n > 0) or one that is not 16-byte
+ * aligned.  PAPER.md:47 (3-D decomposition), DESIGN R-12. */
 int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y, const double* d_z,
                       const double* d_vx, const double* d_vy, const double* d_vz,
                       const double* d_diam, const int64_t* d_id);
@@ -89,7 +96,10 @@ int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y,
 /* a1-a4: per particle, interpolate U at X (trilinear), advance V then X under
  * dV/dt = -(V-U)/tau_p + g, dX/dt = V with U frozen over dt (Eq. 5-6, f = 1;
  * exponential integrator, DESIGN R-1), wrap into the box, classify into one of 27 destinations
- * ("mask computation") and count per (subdomain, destination).  In place. */
+ * ("mask computation") and count per (subdomain, destination).  In place.
+ * LCS_ERR_STATE without fluid or particles, or while the codes of an earlier lcs_particle_step
+ * are still waiting for lcs_migrate / lcs_migrate_sweeps (the same holds for lcs_step_fused and
+ * lcs_step_rk2: a pending push must be migrated first). */
 int lcs_particle_step(lcs_t* h, double dt);
 
 /* a5-a8: prefix-scan particle communication among the virtual
@@ -126,7 +136,7 @@ int lcs_get_counts(lcs_t* h, int64_t* d_counts);
 
 /* Packed copy-out: subdomain 0's particles in slot order, then subdomain 1's, ...  Each array
  * needs room for the current total (lcs_get_status gives it; <= P*capacity).  Any of the data
- * pointers may be NULL to skip that field. */
+ * pointers may be NULL to skip that field; the others must be 16-byte aligned (LCS_ERR_INVALID_ARG). */
 int lcs_get_particles(lcs_t* h, int64_t* d_counts, double* d_x, double* d_y, double* d_z,
                       double* d_vx, double* d_vy, double* d_vz, double* d_diam, int64_t* d_id);
 
@@ -143,7 +153,11 @@ int lcs_get_status(lcs_t* h, int* sticky_error, int64_t* n_total, int64_t* n_mig
  * CPU-delegated path): copies n particles host->device, bins them, runs
  * lcs_step_fused(dt), copies the packed result and the P counts device->host, synchronises.
  * h_in / h_out: 8 host pointers each in the order x,y,z,vx,vy,vz,d,id (8 bytes per element;
- * h_out arrays need room for n).  d_staging: device scratch of at least 64*n + 8*P bytes. */
+ * h_out arrays need room for n; 8-byte aligned).  d_staging: device scratch, 256-byte aligned, of at
+ * least lcs_staging_bytes(n, P) bytes (eight arrays of n words, each rounded up to 256 bytes, plus
+ * the P counts; 0 for n < 0 or P < 1).  LCS_ERR_INVALID_ARG for a null or misaligned pointer or a
+ * staging block that is too small. */
+size_t lcs_staging_bytes(int64_t n, int P);
 int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8], void* const h_out[8],
                         int64_t* h_counts, void* d_staging, size_t staging_bytes);
 
@@ -159,7 +173,8 @@ int lcs_profile_end(lcs_t* h, double* ms_tile_pass, double* ms_table, double* ms
 /* Number of kernels this library has launched on the handle since create (for bench accounting). */
 int64_t lcs_kernel_launches(lcs_t* h);
 
-/* Library build information: "lcs_b200 <version> sm_100a". */
+/* Library build information: "lcs_b200 <version> sm_100a".  There are no ablation or debug builds of this library:
+ * the kernels have no compile-time switches that change results. */
 const char* lcs_version(void);
 
 #ifdef __cplusplus

@@ -6,12 +6,12 @@ import ctypes as C
 import os
 
 LCS_OK, LCS_ERR_INVALID_ARG, LCS_ERR_STATE, LCS_ERR_CUDA = 0, -1, -2, -3
-LCS_ERR_CAPACITY, LCS_ERR_JUMP, LCS_ERR_RANGE = -4, -5, -6
+LCS_ERR_CAPACITY, LCS_ERR_JUMP, LCS_ERR_RANGE, LCS_ERR_NOMEM = -4, -5, -6, -7
 
 EXPORTED_SYMBOLS = (
     "lcs_workspace_bytes", "lcs_create", "lcs_destroy", "lcs_set_fluid", "lcs_set_particles",
     "lcs_particle_step", "lcs_migrate", "lcs_migrate_sweeps", "lcs_step_rk2", "lcs_step_fused", "lcs_get_counts", "lcs_get_particles",
-    "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_step_fused_host",
+    "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_staging_bytes", "lcs_step_fused_host",
     "lcs_profile_begin", "lcs_profile_end", "lcs_kernel_launches", "lcs_version")
 
 FIELDS = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
@@ -66,6 +66,8 @@ def load_library(build_if_missing: bool = True):
     L.lcs_get_codes.argtypes = [vp, vp]
     L.lcs_get_count_table.argtypes = [vp, vp]
     L.lcs_get_status.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(i64), C.POINTER(i64)]
+    L.lcs_staging_bytes.restype = C.c_size_t
+    L.lcs_staging_bytes.argtypes = [i64, C.c_int]
     L.lcs_step_fused_host.argtypes = [vp, dbl, i64, C.POINTER(vp), C.POINTER(vp), vp, vp, C.c_size_t]
     L.lcs_profile_begin.argtypes = [vp, C.c_int]
     L.lcs_profile_end.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl), C.POINTER(C.c_int)]
@@ -202,9 +204,13 @@ class LCS:
         self._chk("lcs_get_count_table", self._L.lcs_get_count_table(self._h, _ptr(out)))
         return out
 
+    def staging_bytes(self, n):
+        """Bytes of device scratch lcs_step_fused_host needs for n particles (+ 256 so that the block can be aligned)."""
+        return int(self._L.lcs_staging_bytes(int(n), self.P)) + 256
+
     def step_fused_host(self, dt, h_in, h_out, h_counts, staging):
         """h_in / h_out: dicts of pinned host tensors keyed x..id; h_counts: int64[P] host tensor;
-        staging: device uint8 tensor of at least 64*n + 8*P + 4096 bytes."""
+        staging: device uint8 tensor of at least staging_bytes(n) bytes."""
         n = h_in["id"].numel()
         pin = (C.c_void_p * 8)(*(h_in[k].data_ptr() for k in FIELDS))
         pout = (C.c_void_p * 8)(*(h_out[k].data_ptr() for k in FIELDS))

@@ -31,7 +31,7 @@ def stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
-        cmd = [nvcc(), *NVCC_FLAGS, *os.environ.get("LCS_NVCC_EXTRA", "").split(), "-o", LIB, SRC]
+        cmd = [nvcc(), *NVCC_FLAGS, "-o", LIB, SRC]
         res = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or res.returncode:
             print(res.stdout + res.stderr)

@@ -185,7 +185,13 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt, const Slabs* grp = nullpt
 
 extern "C" {
 
-const char* lcs_version(void) { return "lcs_b200 0.1 sm_100a"; }
+const char* lcs_version(void) { return "lcs_b200 0.2 sm_100a"; }
+
+size_t lcs_staging_bytes(int64_t n, int P)
+{
+    if (n < 0 || P < 1) return 0;
+    return 8 * align_up((size_t)n * 8) + align_up((size_t)P * 8);
+}
 
 size_t lcs_workspace_bytes(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params* prm)
 {
@@ -203,7 +209,7 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     const Layout L = make_layout(N, Px, Py, Pz, capacity, prm);
     if (workspace_bytes < L.total) return LCS_ERR_INVALID_ARG;
     lcs_t* h = new (std::nothrow) lcs_handle();
-    if (!h) return LCS_ERR_CUDA;
+    if (!h) return LCS_ERR_NOMEM;
     std::memset(static_cast<void*>(h), 0, sizeof(*h));
     Geom& G = h->G;
     G.N = N; G.Px = Px; G.Py = Py; G.Pz = Pz; G.P = Px * Py * Pz;
@@ -313,6 +319,8 @@ int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y,
     const Geom& G = h->G;
     if (n > (int64_t)G.P * G.cap) return LCS_ERR_INVALID_ARG;
     if (n > 0 && (!d_x || !d_y || !d_z || !d_vx || !d_vy || !d_vz || !d_diam || !d_id)) return LCS_ERR_INVALID_ARG;
+    if (!aligned16(d_x) || !aligned16(d_y) || !aligned16(d_z) || !aligned16(d_vx) || !aligned16(d_vy) || !aligned16(d_vz) ||
+        !aligned16(d_diam) || !aligned16(d_id)) return LCS_ERR_INVALID_ARG;
     // a fresh particle set clears the sticky error
     h->sticky = 0;
     h->pushed = false;
@@ -341,7 +349,7 @@ int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y,
 int lcs_particle_step(lcs_t* h, double dt)
 {
     if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
-    if (!h->have_fluid || !h->have_particles) return LCS_ERR_STATE;
+    if (!h->have_fluid || !h->have_particles || h->pushed) return LCS_ERR_STATE;   // a pending push must be migrated first
     if (h->sticky) return h->sticky;
     const Geom& G = h->G;
     cudaMemsetAsync(h->T.cnt, 0, (size_t)G.P * 32 * 4, h->stream);
@@ -376,7 +384,7 @@ int lcs_migrate_sweeps(lcs_t* h)
 int lcs_step_rk2(lcs_t* h, double dt)
 {
     if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
-    if (!h->rk2 || !h->have_fluid || !h->have_particles) return LCS_ERR_STATE;
+    if (!h->rk2 || !h->have_fluid || !h->have_particles || h->pushed) return LCS_ERR_STATE;
     if (h->sticky) return h->sticky;
     const Geom& G = h->G;
     const dim3 grid((G.tiles_per_sub + kPushWarps - 1) / kPushWarps, G.P);
@@ -397,7 +405,7 @@ int lcs_step_rk2(lcs_t* h, double dt)
 int lcs_step_fused(lcs_t* h, double dt)
 {
     if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
-    if (!h->have_fluid || !h->have_particles) return LCS_ERR_STATE;
+    if (!h->have_fluid || !h->have_particles || h->pushed) return LCS_ERR_STATE;   // a pending push must be migrated first
     if (h->sticky) return h->sticky;
     return enqueue_tile_pass(h, true, dt);
 }
@@ -421,6 +429,8 @@ int lcs_get_particles(lcs_t* h, int64_t* d_counts, double* d_x, double* d_y, dou
                       double* d_vy, double* d_vz, double* d_diam, int64_t* d_id)
 {
     if (!h) return LCS_ERR_INVALID_ARG;
+    if (!aligned16(d_counts) || !aligned16(d_x) || !aligned16(d_y) || !aligned16(d_z) || !aligned16(d_vx) || !aligned16(d_vy) ||
+        !aligned16(d_vz) || !aligned16(d_diam) || !aligned16(d_id)) return LCS_ERR_INVALID_ARG;      // NULL (= skip) is aligned
     OutPtrs O;
     O.f[0] = d_x; O.f[1] = d_y; O.f[2] = d_z; O.f[3] = d_vx; O.f[4] = d_vy; O.f[5] = d_vz; O.f[6] = d_diam;
     O.id = d_id; O.code = nullptr;
@@ -466,11 +476,13 @@ int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8
 {
     if (!h || !h_in || !h_out || !h_counts || !d_staging || n < 0) return LCS_ERR_INVALID_ARG;
     const size_t arr = align_up((size_t)n * 8);
-    if (staging_bytes < 8 * arr + align_up((size_t)h->G.P * 8)) return LCS_ERR_INVALID_ARG;
+    if (staging_bytes < lcs_staging_bytes(n, h->G.P)) return LCS_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(h_counts) & 7u) return LCS_ERR_INVALID_ARG;
     if (reinterpret_cast<uintptr_t>(d_staging) % kAlign) return LCS_ERR_INVALID_ARG;
     char* st = static_cast<char*>(d_staging);
     for (int a = 0; a < 8; ++a) {
         if (!h_in[a] || !h_out[a]) return LCS_ERR_INVALID_ARG;
+        if ((reinterpret_cast<uintptr_t>(h_in[a]) | reinterpret_cast<uintptr_t>(h_out[a])) & 7u) return LCS_ERR_INVALID_ARG;
         if (cudaMemcpyAsync(st + a * arr, h_in[a], (size_t)n * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
             return LCS_ERR_CUDA;
     }

@@ -9,8 +9,7 @@
 // path for its tile with warp-level primitives only (ballot / shuffle / popc / redux, three private
 // shared-memory tile buffers fed by bulk tensor copies, no block barrier after the prologue); the
 // gather of the next row is in flight under the arithmetic of the current one.  The comment above
-// k_tile_pass has the details.  Macros LCS_X_* are ablation builds (wrong results on purpose), used
-// for the measurements quoted in DESIGN.md 6.5 and profiles/.
+// k_tile_pass has the details.
 #pragma once
 #include <cuda.h>            // CUtensorMap (the type only; the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
@@ -79,11 +78,7 @@ struct Tables {
 // ---------------------------------------------------------------------------------------------
 // small helpers
 // ---------------------------------------------------------------------------------------------
-#ifdef LCS_X_NOSTATUS               // experiment builds only: errors are not recorded
-__device__ __forceinline__ void raise(int*, int) {}
-#else
 __device__ __forceinline__ void raise(int* status, int code) { atomicCAS(status, 0, code); }
-#endif
 
 __device__ __forceinline__ uint64_t ld_relaxed_u64(const void* p)
 {
@@ -193,18 +188,8 @@ struct alignas(32) Cell { double u, v, w, pad; };
 __device__ __forceinline__ Cell ld_cell(const double* __restrict__ F4, uint32_t cell)
 {
     Cell r;
-#ifdef LCS_X_NOGATHER            // experiment: no fluid loads at all
-    r.u = r.v = r.w = r.pad = 0.0;
-    return r;
-#endif
-#ifdef LCS_X_GATHER_SMALL        // experiment: all gathers fall into the first 8 MB of the field
-    cell &= 0x3ffffu;
-#endif
     asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
                  : "=d"(r.u), "=d"(r.v), "=d"(r.w), "=d"(r.pad) : "l"(F4 + 4 * (size_t)cell));
-#ifdef LCS_X_ZEROU                // experiment: loads kept, values zeroed (same dynamics as LCS_X_NOGATHER)
-    r.u *= 0.0; r.v *= 0.0; r.w *= 0.0;
-#endif
     return r;
 }
 
@@ -438,15 +423,6 @@ __device__ __forceinline__ void gather_issue(Gath& Q, const double* __restrict__
     const uint32_t a0 = Nu * (uint32_t)i0, a1 = Nu * (uint32_t)i1;
     const uint32_t row[4] = {Nu * (a0 + (uint32_t)j0), Nu * (a1 + (uint32_t)j0), Nu * (a0 + (uint32_t)j1),
                              Nu * (a1 + (uint32_t)j1)};
-#ifdef LCS_X_NOPAIR               // experiment: every lane gathers its own eight corners, no exchange
-    (void)lane;
-#pragma unroll
-    for (int m = 0; m < 4; ++m) Q.a[m] = ld_cell(F4, row[m] + (uint32_t)k0);
-#pragma unroll
-    for (int m = 0; m < 4; ++m) Q.b[m] = ld_cell(F4, row[m] + (uint32_t)k1);
-    Q.fxA = Q.fxB = fx; Q.fyA = Q.fyB = fy;
-    return;
-#endif
     const uint32_t kk = (uint32_t)k0 | ((uint32_t)k1 << 16);          // N <= 1625 fits 16 bits
     const int le = lane & ~1, lo = lane | 1;
     const uint32_t sh = (uint32_t)(lane & 1) << 4;                    // this lane always fetches z-side (lane & 1)
@@ -473,13 +449,6 @@ __device__ __forceinline__ Vec3 gather_reduce(const Gath& Q, int lane)
 {
     const Vec3 pa = side_reduce(Q.a, Q.fxA, Q.fyA);
     const Vec3 pb = side_reduce(Q.b, Q.fxB, Q.fyB);
-#ifdef LCS_X_NOPAIR
-    {
-        Vec3 U0;
-        U0.x = lerp(pa.x, pb.x, Q.fz); U0.y = lerp(pa.y, pb.y, Q.fz); U0.z = lerp(pa.z, pb.z, Q.fz);
-        return U0;
-    }
-#endif
     // the even lane needs A's z1 side (the odd lane's pa); the odd lane needs B's z0 side (the even lane's pb)
     const bool odd = lane & 1;
     Vec3 give, keep;
@@ -560,11 +529,7 @@ __device__ __forceinline__ void sum_descs(const uint64_t* base, int n, int lane,
     const bool need = lane < n;
     const uint64_t* pd = base + 2 * (need ? lane : 0);
     for (unsigned ns = 64;; ns = min(ns * 2u, 1024u)) {
-#ifdef LCS_X_NOWAIT                // experiment: never wait for a predecessor (wrong results)
-        const bool ready = true;
-#else
         const bool ready = !need || ((uint32_t)(w.x >> 34) == epoch && (uint32_t)(w.y >> 34) == epoch);
-#endif
         if (__all_sync(0xffffffffu, ready)) break;
         __nanosleep(ns);
         if (need) w = ld_relaxed_desc(pd);
@@ -777,6 +742,7 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 wait_buf(bc);
             }
             if (lane < kRows) W.stay_m[lane] = 0u;
+            __syncwarp();                  // lane 0 rewrites these words row by row
             uint32_t cnt_c = 0;            // lane c: migrants of the tile so far with code c
             uint32_t n_mig = 0, n_stay = 0;
             g_early = 0u;
@@ -888,11 +854,7 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 unsigned long long w = lb_g;
                 if (g0 > 0 && need) w = ld_relaxed_u64(ga + g0 + lane);
                 for (unsigned ns = 64;; ns = min(ns * 2u, 1024u)) {
-#ifdef LCS_X_NOWAIT
-                    const bool ready = true;
-#else
                     const bool ready = !need || (w >> 40) == 32ull;
-#endif
                     if (__all_sync(0xffffffffu, ready)) break;
                     __nanosleep(ns);
                     if (need) w = ld_relaxed_u64(ga + g0 + lane);
@@ -902,9 +864,6 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             }
             // copy-out, stayers: in place, compacted; the stayers of a row are consecutive lanes -> consecutive slots
             uint32_t base = (uint32_t)s * cap32 + excl_stay;
-#ifdef LCS_X_NOSTORE             // experiment: no stayer stores
-            if (excl_stay == 0xffffffffu)
-#endif
 #pragma unroll 1
             for (int rr = 0; rr < kRows; ++rr) {
                 const unsigned m = W.stay_m[rr];

@@ -55,6 +55,17 @@ def test_version_and_workspace_size_checks(lib):
     assert lib.lcs_workspace_bytes(32, 2, 2, 2, 4096, None) == 0
 
 
+def test_staging_size_formula(lib):
+    """lcs_staging_bytes is what lcs_step_fused_host checks against: eight arrays of n words, each rounded up to 256
+    bytes, plus the P counts rounded up to 256 bytes (include/lcs.h)."""
+    up = lambda v: (v + 255) // 256 * 256
+    lib.lcs_staging_bytes.restype = C.c_size_t
+    lib.lcs_staging_bytes.argtypes = [C.c_int64, C.c_int]
+    for n, P in ((0, 1), (1, 8), (30011, 8), (1 << 26, 512)):
+        assert lib.lcs_staging_bytes(n, P) == 8 * up(8 * n) + up(8 * P)
+    assert lib.lcs_staging_bytes(-1, 8) == 0 and lib.lcs_staging_bytes(10, 0) == 0
+
+
 def test_null_handles_are_rejected(lib):
     from paper_2604_11008_b200 import LCS_ERR_INVALID_ARG
     for name in ("lcs_destroy", "lcs_migrate", "lcs_migrate_sweeps"):

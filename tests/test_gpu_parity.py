@@ -305,7 +305,7 @@ def test_host_buffer_entry_point_matches_oracle(torch_cuda, oracle_lib):
     h_in = {k: torch.from_numpy(np.ascontiguousarray(parts[k])).pin_memory() for k in F8}
     h_out = {k: torch.empty(n, dtype=dtypes[k]).pin_memory() for k in F8}
     h_counts = torch.empty(8, dtype=torch.int64).pin_memory()
-    staging = torch.empty(64 * n + 8 * 8 + 16384, dtype=torch.uint8, device="cuda")
+    staging = torch.empty(dev.staging_bytes(n), dtype=torch.uint8, device="cuda")
     for step in range(3):
         assert o.step(0.7) == 0
         dev.step_fused_host(0.7, h_in, h_out, h_counts, staging)       # synchronises: the result is on the host
@@ -436,6 +436,15 @@ def test_sticky_errors(torch_cuda, oracle_lib):
     with pytest.raises(LcsError) as ei:
         dev.migrate()
     assert ei.value.code == LCS_ERR_STATE
+    # a second push (of any kind) while the codes of the first are still waiting for their migration
+    dev.particle_step(0.1)
+    for again in (lambda: dev.particle_step(0.1), lambda: dev.step_fused(0.1)):
+        with pytest.raises(LcsError) as ei:
+            again()
+        assert ei.value.code == LCS_ERR_STATE
+    dev.migrate()
+    dev.step_fused(0.1)                # fine again
+    assert dev.get_status()[:2] == (0, 1)
     dev.close()
     with pytest.raises(LcsError):
         LCS(15, 2, 2, 2, 16)          # N not divisible
@@ -514,21 +523,36 @@ def test_stress_shape_sample(torch_cuda, oracle_lib):
     dev.close()
 
 
+def _reload_oracle_from_gpu(o, dev):
+    """Protocol P1: the oracle takes over the GPU's current packed state (all codes = stay)."""
+    st = to_np(dev.get_particles())
+    assert o.load_packed(st["counts"], *(st[k] for k in F8)) == 0
+    return st
+
+
 @pytest.mark.slow
-@pytest.mark.parametrize("name,steps", [("Medium", None), ("Clustered", 3), ("Large", 1), ("Stress", 1)])
-def test_full_size_free_running_P2(torch_cuda, oracle_lib, name, steps):
-    """BASELINE.json's configurations at FULL size run freely on both sides (protocol P2), every particle compared: final
-    ids, order and counts bit-identical, positions and velocities 0 ulp.  Medium (2,097,152 particles, 128^3, 4x4x4,
-    gravity): all its 100 steps.  Clustered (16.8 M, 4096 clumps): 3 steps.  Large (67.1 M, 512^3, 8x8x8): 1 step.
-    Stress (268 M, 1024^3, 30 % migrants): 1 step.  Bounded by single-core oracle time (10-30 s each, 3 min for Stress)."""
+@pytest.mark.parametrize("name,first,last", [("Medium", None, None), ("Clustered", 3, 50), ("Large", 1, 20), ("Stress", 1, 10)])
+def test_full_size_free_running_P2_then_last_step_lockstep_P1(torch_cuda, oracle_lib, name, first, last):
+    """BASELINE.json's configurations at FULL size, in the launch configuration bench.py times, every particle compared:
+    ids, order and counts bit-identical, positions and velocities 0 ulp.
+    (1) Protocol P2, both sides free-running from the initial state: Medium (2,097,152 particles, 128^3, 4x4x4, gravity)
+        all its 100 steps; Clustered (16.8 M, 4096 clumps) 3 steps; Large (67.1 M, 512^3, 8x8x8) 1 step; Stress (268 M,
+        1024^3, 30 % migrants) 1 step -- bounded by single-core oracle time.
+    (2) Protocol P1 at the LAST step of the config (50 / 20 / 10): the GPU runs steps first+1 .. K-1 alone, the oracle
+        loads that evolved state (slabs no longer in id order, uneven counts, send regions reused K-1 times -- the state
+        bench.py times), both run step K, everything is compared again.
+    (3) Large only, continuing from that state: the SURVEY 8(f) paths at P = 512 with 163,840-slot slabs -- axis-by-axis
+        sweeps after an unfused push; a fused step with drag_model = 1; one lcs_step_rk2 (two stages, 16 arrays through
+        the second tensor map) with drag_model = 1."""
     from workloads import gen
+    from paper_2604_11008_b200 import LCS
+    import gc
     import psutil
     cfg = gen.get_config(name)
     if psutil.virtual_memory().available < 400 * cfg["n"] + 3 * 24 * cfg["N"] ** 3:
         pytest.skip(f"{name} at full size needs more host memory for the oracle")
-    if steps is not None:
-        cfg["steps"] = steps
-    import gc
+    K = cfg["steps"] if last is None else last
+    first = K if first is None else first
     gc.collect()
     torch_cuda.cuda.empty_cache()                      # the cached blocks of earlier tests count against this one
     nP = cfg["P"][0] * cfg["P"][1] * cfg["P"][2]
@@ -543,15 +567,62 @@ def test_full_size_free_running_P2(torch_cuda, oracle_lib, name, steps):
     torch_cuda.cuda.empty_cache()
     o, dev, rc = make_pair(torch_cuda, oracle_lib, cfg["N"], cfg["P"], cfg["capacity"], fluid, parts, g=cfg["g"],
                            send_capacity=cfg["capacity"] // 2)
+    del parts
     gc.collect()
     torch_cuda.cuda.empty_cache()
     assert rc == 0
-    for step in range(cfg["steps"]):
-        assert o.step(cfg["dt"]) == 0, step
-        dev.step_fused(cfg["dt"])
-    assert dev.get_status() == (0, cfg["n"], o.n_migrated_last)
-    compare_packed(dev, o, f"{name}, {cfg['steps']} steps, free running")
-    dev.close()
+    dt, n = cfg["dt"], cfg["n"]
+    for step in range(first):
+        assert o.step(dt) == 0, step
+        dev.step_fused(dt)
+    assert dev.get_status() == (0, n, o.n_migrated_last)
+    compare_packed(dev, o, f"{name}, {first} steps, free running")
+    if K > first:
+        for step in range(first, K - 1):
+            dev.step_fused(dt)
+        assert dev.get_status()[:2] == (0, n)
+        st = _reload_oracle_from_gpu(o, dev)
+        assert not np.array_equal(st["id"][:4096], np.sort(st["id"][:4096]))      # the evolved state really is reordered
+        del st
+        gc.collect()
+        assert o.step(dt) == 0
+        dev.step_fused(dt)
+        assert dev.get_status() == (0, n, o.n_migrated_last)
+        compare_packed(dev, o, f"{name}, step {K} in lock step")
+    if name == "Large":
+        # (3a) unfused push + axis-by-axis sweeps
+        assert o.push(dt) == 0
+        rc, moved = o.migrate_sweeps()
+        assert rc == 0
+        dev.particle_step(dt)
+        dev.migrate_sweeps()
+        assert dev.get_status() == (0, n, moved[2])
+        got, _ = compare_packed(dev, o, "Large, sweeps")
+        dev.close()
+        del dev
+        gc.collect()
+        torch_cuda.cuda.empty_cache()
+        # (3b) drag_model = 1: one fused step, then one two-stage RK2 step, on a handle with the RK2 arrays
+        devR = LCS(cfg["N"], *cfg["P"], cfg["capacity"], g=cfg["g"], send_capacity=cfg["capacity"] // 2, drag_model=1, rk2=True)
+        df = [torch_cuda.from_numpy(f).cuda() for f in fluid]
+        devR.set_fluid(*df)
+        dp = to_dev(torch_cuda, {k: got[k] for k in F8})
+        devR.set_particles(*(dp[k] for k in F8))
+        d_min = float(got["d"].min())
+        del dp, got
+        assert oracle_lib.lib().orc_set_drag_model(o._h, 1) == 0
+        assert o.step(dt) == 0
+        devR.step_fused(dt)
+        assert devR.get_status() == (0, n, o.n_migrated_last)
+        compare_packed(devR, o, "Large, drag_model 1 fused")
+        dt_rk2 = 0.25 * 1000.0 * d_min ** 2 / (18.0 * 1.5e-5)      # explicit scheme: a fraction of the smallest droplet's tau_p
+        assert o.step_rk2(dt_rk2) == 0
+        devR.step_rk2(dt_rk2)
+        assert devR.get_status() == (0, n, o.n_migrated_last)
+        compare_packed(devR, o, "Large, two-stage RK2 with drag_model 1")
+        devR.close()
+    else:
+        dev.close()
 
 
 @pytest.mark.slow

@@ -128,3 +128,49 @@ def test_stage2_needs_the_migration_of_stage1(oracle_lib):
     o.set_particles([1.0], [1.0], [1.0], [0.1], [0.0], [0.0], [3e-4], [0])
     assert o.rk2_stage1(0.1) == 0
     assert o.rk2_stage2(0.1) != 0            # ORC_ERR_STATE: the codes of stage 1 have not been migrated
+
+
+@pytest.mark.parametrize("d,dt", [(300e-6, 0.02), (600e-6, 0.05)])
+def test_heun_with_nonlinear_drag_reevaluates_f_per_stage(oracle_lib, d, dt):
+    """drag_model = 1 inside the two-stage RK2 (f = 1 + 0.15 Re_p^0.687 is part of Eq. 6, and the
+    integrator has two stages, so each stage evaluates f from ITS slip): one particle, uniform U, gravity on, Heun
+    written out here with libm pow -- f1 from |V0 - U|, f2 from |V1 - U|.  The variant that reuses the slip of V0 in
+    stage 2 (a plausible mistake the decomposition-independence pin cannot see) must be far outside the tolerance."""
+    N = 8
+    g = np.array([0.0, 0.0, -9.81])
+    U = np.array([0.6, -0.3, 0.2])
+    tau_p = RHO * d * d / (18 * NU)
+    o = oracle_lib.Oracle(N, 1, 1, 1, 8, nu=NU, rho_ratio=RHO, g=tuple(g), drag_model=1)
+    o.set_fluid(*(np.full(N ** 3, c) for c in U))
+    x0 = np.array([1.0, 2.0, 3.0])
+    v0 = np.array([2.5, -1.5, 1.0])
+    o.set_particles([x0[0]], [x0[1]], [x0[2]], [v0[0]], [v0[1]], [v0[2]], [d], [0])
+
+    def f_of(v):
+        return 1.0 + 0.15 * (d * float(np.linalg.norm(v - U)) / NU) ** 0.687
+
+    assert f_of(v0) > 1.5                      # Re_p = O(10..100): the correction matters
+    assert dt * f_of(v0) / tau_p < 0.5         # the paper's regime for an explicit scheme
+    x, v = x0.copy(), v0.copy()
+    xw, vw = x0.copy(), v0.copy()              # the wrong variant: stage 2 with the f of stage 1
+    K = 6
+    for _ in range(K):
+        assert o.step_rk2(dt) == 0
+        k1 = (U - v) * (f_of(v) / tau_p) + g
+        v1 = v + dt * k1
+        k2 = (U - v1) * (f_of(v1) / tau_p) + g
+        x = x + 0.5 * dt * (v + v1)
+        v = v + 0.5 * dt * (k1 + k2)
+        k1w = (U - vw) * (f_of(vw) / tau_p) + g
+        v1w = vw + dt * k1w
+        k2w = (U - v1w) * (f_of(vw) / tau_p) + g
+        xw = xw + 0.5 * dt * (vw + v1w)
+        vw = vw + 0.5 * dt * (k1w + k2w)
+    out = o.get_particles()
+    got_v = np.array([out["vx"][0], out["vy"][0], out["vz"][0]])
+    got_x = np.array([out["x"][0], out["y"][0], out["z"][0]])
+    assert np.all(np.abs(got_v - v) <= 1e-12 * np.maximum(1.0, np.abs(v)))
+    dx = np.abs(got_x - np.mod(x, L))
+    assert np.all(np.minimum(dx, L - dx) <= 1e-12 * L)
+    assert np.max(np.abs(got_v - vw)) > 1e-6   # the pin discriminates: frozen-f Heun is not what the oracle computes
+    o.close()
