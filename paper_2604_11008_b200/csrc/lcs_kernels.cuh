@@ -26,6 +26,11 @@ namespace lcs {
 constexpr int kBlock = LCS_BLOCK;            // threads per CTA of the tile pass
 constexpr int kMinBlocks = LCS_MIN_BLOCKS;   // CTAs per SM the tile pass is compiled for
 constexpr int kWarps = kBlock / 32;
+#ifdef LCS_MAXREG
+#define LCS_TP_BOUNDS __maxnreg__(LCS_MAXREG)
+#else
+#define LCS_TP_BOUNDS __launch_bounds__(kBlock, kMinBlocks)
+#endif
 #ifndef LCS_ROWS
 #define LCS_ROWS 2
 #endif
@@ -183,13 +188,15 @@ __device__ __forceinline__ double lerp(double p, double q, double f) { return fm
 // exchange of three doubles then feeds the z lerp.  Operation order per particle is exactly
 // lerp x, then y, then z (rule R3).
 // ---------------------------------------------------------------------------------------------
-struct alignas(32) Cell { double u, v, w, pad; };
+struct Cell { double u, v, w; };
 
 __device__ __forceinline__ Cell ld_cell(const double* __restrict__ F4, uint32_t cell)
 {
     Cell r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
-                 : "=d"(r.u), "=d"(r.v), "=d"(r.w), "=d"(r.pad) : "l"(F4 + 4 * (size_t)cell));
+    // one 256-bit load per record; the sink operand keeps the pad word out of the register file (24 in-flight registers
+    // per corner pair instead of 32)
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,_}, [%3];"
+                 : "=d"(r.u), "=d"(r.v), "=d"(r.w) : "l"(F4 + 4 * (size_t)cell));
     return r;
 }
 
@@ -609,7 +616,7 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
 struct TileRef { int s, t; uint32_t cnt; bool ok; };     // a ticketed tile: subdomain, tile index, count[s]
 
 template <bool kFused, bool kBig, int kDrag>
-__global__ void __launch_bounds__(kBlock, kMinBlocks)
+__global__ void LCS_TP_BOUNDS
 k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch,
             const __grid_constant__ CUtensorMap slab_map)
 {
