@@ -47,9 +47,9 @@ struct Layout {
     size_t slab_f[7], slab_id, slab_code;
     size_t rk2_b;                      // RK2 group B: 8 arrays, stride as the slabs (0 = absent)
     size_t pool, pool_bytes, fluid4;
-    size_t count, cnt, recv_off, new_count, desc, gacc, gacc_bytes, tile_start, tile_cnt, group_excl, misc, prefix;
+    size_t count, cnt, recv_off, new_count, desc, gacc, gacc_bytes, tile_start, send_count, chunk_excl, misc, prefix;
     size_t total;
-    int tiles_per_sub, groups_per_sub, lbgroups_per_sub;
+    int tiles_per_sub, chunks_per_sub, lbgroups_per_sub;
     int64_t send_cap;
 };
 
@@ -80,7 +80,7 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     const size_t slots = P * (size_t)cap;
     L.send_cap = prm->send_capacity ? prm->send_capacity : cap;
     L.tiles_per_sub = (int)((cap + kTile - 1) / kTile);
-    L.groups_per_sub = (L.tiles_per_sub + kGroup - 1) / kGroup;
+    L.chunks_per_sub = (int)((L.send_cap + kChunk - 1) / kChunk);
     L.lbgroups_per_sub = (L.tiles_per_sub + 31) / 32;
     const size_t ntiles = P * (size_t)L.tiles_per_sub;
     size_t off = 0;
@@ -89,8 +89,8 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     L.slab_code = off; off = align_up(off + slots);
     L.rk2_b = 0;
     if (prm->enable_rk2) { L.rk2_b = off; off += 8 * align_up(slots * 8); }
-    // send pool: 8 arrays of P*send_cap slots; doubles as lcs_set_particles scratch
-    const size_t send_bytes = 8 * align_up(P * (size_t)L.send_cap * 8);
+    // send pool: 8 arrays of P*send_cap slots + one code byte per slot; doubles as lcs_set_particles scratch
+    const size_t send_bytes = 8 * align_up(P * (size_t)L.send_cap * 8) + align_up(P * (size_t)L.send_cap);
     const size_t set_tiles = (slots + kSetTile - 1) / kSetTile;
     const size_t set_bytes = align_up(slots * 4) + align_up(set_tiles * P * 4);
     L.pool = off; L.pool_bytes = send_bytes > set_bytes ? send_bytes : set_bytes;
@@ -100,11 +100,11 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     L.cnt = off;       off = align_up(off + P * 32 * 4);
     L.recv_off = off;  off = align_up(off + P * 32 * 4);
     L.new_count = off; off = align_up(off + P * 4);
-    L.desc = off;      off = align_up(off + ntiles * 2 * 8);
+    L.desc = off;      off = align_up(off + ntiles * 8);
     L.gacc = off;      L.gacc_bytes = P * (size_t)L.lbgroups_per_sub * 8; off = align_up(off + L.gacc_bytes);
     L.tile_start = off; off = align_up(off + (P + 1) * 4);
-    L.tile_cnt = off;  off = align_up(off + ntiles * 32);
-    L.group_excl = off; off = align_up(off + P * (size_t)L.groups_per_sub * 32 * 4);
+    L.send_count = off; off = align_up(off + P * 4);
+    L.chunk_excl = off; off = align_up(off + P * (size_t)L.chunks_per_sub * 32 * 4);
     L.misc = off;      off = align_up(off + 256);
     L.prefix = off;    off = align_up(off + (P + 1) * 8);
     L.total = off;
@@ -152,8 +152,11 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt, const Slabs* grp = nullpt
     const Geom& G = h->G;
     const Slabs& S = grp ? *grp : h->S;
     const CUtensorMap& M = map ? *map : h->slab_map;
-    h->epoch = (h->epoch + 1u) & 0x3fffffffu;
-    if (h->epoch == 0u) h->epoch = 1u;
+    h->epoch = (h->epoch + 1u) & 0xffffffu;                // 24 bits: the count field of a look-back word
+    if (h->epoch == 0u) {                                  // wrapped: no word of 2^24 launches ago may look current
+        h->epoch = 1u;
+        cudaMemsetAsync(h->T.desc, 0, (size_t)G.P * (size_t)G.tiles_per_sub * 8, h->stream);
+    }
     const bool rec = h->prof && h->prof_steps < h->prof_max;
     cudaEvent_t* ev = rec ? h->prof->data() + 4 * h->prof_steps : nullptr;
     if (rec) cudaEventRecord(ev[0], h->stream);
@@ -171,10 +174,10 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt, const Slabs* grp = nullpt
     }
 #undef LCS_LAUNCH_TP
     if (rec) cudaEventRecord(ev[1], h->stream);
-    k_code_scan<<<G.P, 256, 0, h->stream>>>(G, h->T);
+    k_send_scan<<<G.P, 256, 0, h->stream>>>(G, h->Snd, h->T);
     k_table<<<(G.P + 7) / 8, 256, 0, h->stream>>>(G, h->T);
     if (rec) cudaEventRecord(ev[2], h->stream);
-    k_unpack<<<dim3((G.groups_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, S, h->Snd, h->T);
+    k_unpack<<<dim3((G.chunks_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, S, h->Snd, h->T);
     k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, commit ? 1 : 0);     // (also resets the tile ticket for the next round)
     if (rec) { cudaEventRecord(ev[3], h->stream); ++h->prof_steps; }
     if (commit) h->pushed = false;
@@ -215,7 +218,7 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     G.N = N; G.Px = Px; G.Py = Py; G.Pz = Pz; G.P = Px * Py * Pz;
     G.nx = N / Px; G.ny = N / Py; G.nz = N / Pz;
     G.tiles_per_sub = L.tiles_per_sub;
-    G.groups_per_sub = L.groups_per_sub;
+    G.chunks_per_sub = L.chunks_per_sub;
     G.lbgroups_per_sub = L.lbgroups_per_sub;
     G.cap = capacity; G.send_cap = L.send_cap;
     // all doubles are computed once on the host and passed as data (rule R6)
@@ -235,7 +238,7 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     const size_t send_arr = align_up(P * (size_t)L.send_cap * 8);
     for (int a = 0; a < 7; ++a) h->Snd.f[a] = reinterpret_cast<double*>(w + L.pool + a * send_arr);
     h->Snd.id = reinterpret_cast<int64_t*>(w + L.pool + 7 * send_arr);
-    h->Snd.code = nullptr;
+    h->Snd.code = reinterpret_cast<uint8_t*>(w + L.pool + 8 * send_arr);
     h->fluid4 = reinterpret_cast<double*>(w + L.fluid4);
     h->T.count = reinterpret_cast<uint32_t*>(w + L.count);
     h->T.cnt = reinterpret_cast<uint32_t*>(w + L.cnt);
@@ -245,8 +248,8 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     h->T.gacc = reinterpret_cast<unsigned long long*>(w + L.gacc);
     h->gacc_bytes = L.gacc_bytes;
     h->T.tile_start = reinterpret_cast<uint32_t*>(w + L.tile_start);
-    h->T.tile_cnt = reinterpret_cast<uint8_t*>(w + L.tile_cnt);
-    h->T.group_excl = reinterpret_cast<uint32_t*>(w + L.group_excl);
+    h->T.send_count = reinterpret_cast<uint32_t*>(w + L.send_count);
+    h->T.chunk_excl = reinterpret_cast<uint32_t*>(w + L.chunk_excl);
     h->T.ticket = reinterpret_cast<unsigned int*>(w + L.misc);
     h->T.status = reinterpret_cast<int*>(w + L.misc + 16);
     h->T.n_migrated = reinterpret_cast<unsigned long long*>(w + L.misc + 32);

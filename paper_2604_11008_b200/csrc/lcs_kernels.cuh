@@ -40,17 +40,17 @@ static_assert(kRows >= 1 && kRows <= 4, "row masks and the unfused pass's code b
 constexpr int kStay = 13;
 constexpr int kNC = 27;                      // destination codes
 constexpr int kInvalid = 31;                 // code of a lane beyond the slab's count
-#ifndef LCS_GROUP
-#define LCS_GROUP 8
-#endif
-constexpr int kGroup = LCS_GROUP;            // tiles per unpack warp
+constexpr int kChunk = 256;                  // migrants of one send region handled by one warp of the scan / unpack kernels
 
-// Look-back descriptor word: [ epoch:30 | valid:2 | value:32 ]
+// Look-back words (all 64-bit): [ count:24 | migrants:20 | stayers:20 ]
+//   desc[tile]   count = epoch of the launch that wrote it (1 .. 2^24-1); written once by the tile's push
+//   gacc[group]  count = tiles of the group of 32 that have published; zeroed per launch, accumulated by atomics
+constexpr unsigned long long kField20 = 0xfffffull;
 
 struct Geom {
     int N, Px, Py, Pz, P, nx, ny, nz;
     int tiles_per_sub;                 // ceil(cap / kTile)
-    int groups_per_sub;                // ceil(tiles_per_sub / kGroup)
+    int chunks_per_sub;                // ceil(send_cap / kChunk): chunks of a send region
     int lbgroups_per_sub;              // ceil(tiles_per_sub / 32): look-back groups
     int64_t cap, send_cap;
     double inv_dx, K_tau, L, L_below, gx, gy, gz;
@@ -58,10 +58,10 @@ struct Geom {
     int drag_model;                    // 0 = Stokes, 1 = f = 1 + 0.15 Re_p^0.687 (DESIGN R-23)
 };
 
-struct Slabs {                         // SoA particle storage, P*cap slots each
+struct Slabs {                         // SoA particle storage, P*cap slots each (send pool: P*send_cap)
     double* f[7];                      // x y z vx vy vz d
     int64_t* id;
-    uint8_t* code;
+    uint8_t* code;                     // slabs: destination code of the last unfused push; send pool: code of each migrant
 };
 
 struct Tables {
@@ -69,11 +69,11 @@ struct Tables {
     uint32_t* cnt;                     // [P*32] per-(s,c) totals of the last step (27 used per row)
     uint32_t* recv_off;                // [P*32] slot in the receiver slab where segment (s,c) starts
     uint32_t* new_count;               // [P]
-    uint64_t* desc;                    // [P*tiles_per_sub*2] tile aggregates: (stay, migrant) words
+    uint64_t* desc;                    // [P*tiles_per_sub] tile aggregates
     unsigned long long* gacc;          // [P*lbgroups_per_sub] accumulators of groups of 32 tiles (zeroed per launch)
     uint32_t* tile_start;              // [P+1] compact prefix of non-empty tiles per subdomain
-    uint8_t* tile_cnt;                 // [P*tiles_per_sub*32] per-code count of each tile (<= 128 fits a byte)
-    uint32_t* group_excl;              // [P*groups_per_sub*32] exclusive per-code prefix at each group of kGroup tiles
+    uint32_t* send_count;              // [P] migrants in each send region after the tile pass
+    uint32_t* chunk_excl;              // [P*chunks_per_sub*32] per-code count of each chunk, then its exclusive prefix over the chunks
     unsigned int* ticket;              // tile ticket counter
     int* status;                       // sticky error word
     unsigned long long* n_migrated;    // migrants of the last migrate
@@ -111,6 +111,21 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
+}
+
+// Selects that stay selects: ptxas turns nested ?: on doubles into branches (BSSY / BRA / BSYNC per use), which costs
+// more instructions and cuts the basic blocks the scheduler can interleave.
+__device__ __forceinline__ double sel(bool c, double a, double b)
+{
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %3, 0;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b), "r"((int)c));
+    return r;
+}
+__device__ __forceinline__ int seli(bool c, int a, int b)
+{
+    int r;
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %3, 0;\n\tselp.s32 %0, %1, %2, p;\n\t}" : "=r"(r) : "r"(a), "r"(b), "r"((int)c));
+    return r;
 }
 
 // exp(-z), z >= 0: range reduction by ln2 (hi/lo), degree-14 Taylor polynomial in Horner form with
@@ -368,8 +383,7 @@ constexpr int kTableSmemMax = 1024;          // tile_start[] and the subdomain c
 
 struct alignas(128) TileBuf {
     unsigned long long f[8][kTile];     // x y z vx vy vz d id of the tile's slots, raw 64-bit words; x..vz updated in place
-    uint32_t mlist[kTile];              // migrants in arrival order: position | code << 8 | rank-in-code << 16
-    uint32_t stay_m[4];                 // per row: lanes that stay
+    uint16_t mlist[kTile];              // migrants in slot order: position in the tile | code << 8
 };
 
 // ---- mbarrier / bulk-copy primitives (sm_90+; one elected lane issues, all lanes wait) ----
@@ -495,54 +509,36 @@ __device__ __forceinline__ int advance_particle(Particle& p, const Vec3& U, cons
     return code;
 }
 
-// Stable rank-in-code of the MIGRANTS of one row (code != stay); lane c owns the running count of code c.
-// One warp-uniform iteration per distinct migrant code present in the row (usually 0 to 2).
-__device__ __forceinline__ uint32_t migrant_rank(int code, unsigned mig_m, int lane, uint32_t& cnt_c)
-{
-    const unsigned lt = (1u << lane) - 1u;
-    uint32_t rank = 0;
-    unsigned todo = mig_m;
-    while (todo) {
-        const int leader = __ffs(todo) - 1;
-        const int c = __shfl_sync(0xffffffffu, code, leader);
-        const unsigned m = __ballot_sync(0xffffffffu, code == c) & mig_m;
-        const uint32_t base = __shfl_sync(0xffffffffu, cnt_c, c);
-        if (code == c) rank = base + __popc(m & lt);
-        if (lane == c) cnt_c += __popc(m);
-        todo &= ~m;
-    }
-    return rank;
-}
-
 // What a pushed tile carries from its push to its resolve one iteration later.
 struct TileInfo {
     int s, t;
-    uint32_t n_stay, n_mig;
-    uint32_t run_start;                 // lane c: start of code c's run inside the tile's send chunk
+    uint32_t n_mig;
+    uint32_t stay[kRows];               // per row: lanes that stay
 };
 
-__device__ __forceinline__ ulonglong2 ld_relaxed_desc(const uint64_t* p)
-{   // both words (stay, migrant) of a descriptor in one 128-bit load
-    ulonglong2 v;
-    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0,%1}, [%2];" : "=l"(v.x), "=l"(v.y) : "l"(p) : "memory");
-    return v;
+// The look-back of one tile, two levels of aggregates (no prefix chain): the exclusive prefix of tile t of a slab is
+//     sum of desc over the earlier tiles of its group of 32  +  sum of gacc over the earlier groups,
+// one lane per word: one desc and (up to 64 earlier groups = 4096 tiles) two gacc words per lane, more in a loop.  A lane
+// that has nothing to load holds a word that already looks complete (count field set, value fields zero), so "all
+// ready" is one test of the three count fields.
+struct Poll { unsigned long long a, b, c; };
+
+__device__ __forceinline__ void poll_issue(Poll& w, const Geom& G, const Tables& T, int s, int t, int lane, uint32_t epoch)
+{
+    const int r = t & 31, g = t >> 5;
+    w.a = (unsigned long long)epoch << 40;
+    w.b = w.c = 32ull << 40;
+    const unsigned long long* ga = T.gacc + (size_t)s * G.lbgroups_per_sub + lane;
+    if (lane < r) w.a = ld_relaxed_u64(T.desc + ((size_t)s * G.tiles_per_sub + (t - r) + lane));
+    if (lane < g) w.b = ld_relaxed_u64(ga);
+    if (lane + 32 < g) w.c = ld_relaxed_u64(ga + 32);
 }
 
-// Sum of the (stay, migrant) aggregates desc[first .. first+n), n <= 32, one lane per descriptor; spins until
-// all of them carry this launch's epoch.  `w` is the first poll, loaded early by the caller (lanes < n).
-__device__ __forceinline__ void sum_descs(const uint64_t* base, int n, int lane, uint32_t epoch, ulonglong2 w,
-                                          uint32_t& stay, uint32_t& mig)
-{
-    const bool need = lane < n;
-    const uint64_t* pd = base + 2 * (need ? lane : 0);
-    for (unsigned ns = 64;; ns = min(ns * 2u, 1024u)) {
-        const bool ready = !need || ((uint32_t)(w.x >> 34) == epoch && (uint32_t)(w.y >> 34) == epoch);
-        if (__all_sync(0xffffffffu, ready)) break;
-        __nanosleep(ns);
-        if (need) w = ld_relaxed_desc(pd);
-    }
-    stay += __reduce_add_sync(0xffffffffu, need ? (uint32_t)w.x : 0u);
-    mig += __reduce_add_sync(0xffffffffu, need ? (uint32_t)w.y : 0u);
+__device__ __forceinline__ bool poll_ready(const Poll& w, uint32_t epoch)
+{   // the count fields are the top 24 bits of each word
+    const uint32_t x = ((uint32_t)(w.a >> 32) ^ (epoch << 8)) | ((uint32_t)(w.b >> 32) ^ (32u << 8)) |
+                       ((uint32_t)(w.c >> 32) ^ (32u << 8));
+    return (x >> 8) == 0u;
 }
 
 __device__ __forceinline__ uint32_t pack_xyz(const Geom& G, int s)
@@ -645,7 +641,6 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
     auto xyz = [&](int s) -> uint32_t { return big ? pack_xyz(G, s) : s_xyz[s]; };
     const unsigned lt = (1u << lane) - 1u;
     const unsigned int n_active = ts(G.P);
-    const uint64_t tag = ((uint64_t)(epoch << 2) << 32) | (1ull << 32);
     const uint32_t cap32 = (uint32_t)G.cap;
     int s_hint = 0;
     uint32_t phase = 0;                                    // bit b: parity of the next completion of buffer b's mbarrier
@@ -710,7 +705,9 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                      __longlong_as_double(px[2 * kTile + lane]), lane);
     }
     TileInfo pend;
-    pend.s = pend.t = 0; pend.n_stay = pend.n_mig = pend.run_start = 0;
+    pend.s = pend.t = 0; pend.n_mig = 0;
+#pragma unroll
+    for (int rr = 0; rr < kRows; ++rr) pend.stay[rr] = 0u;
     bool have_pend = false;
     int bc = 0, bp = 0;                                    // buffers of the current and of the pending tile
     for (;;) {
@@ -719,15 +716,11 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
         TileInfo ti = pend;
         nn.ok = false;
         unsigned int g_early = 0u;
-        ulonglong2 lb_w = make_ulonglong2(0ull, 0ull);     // first look-back poll of the pending tile (early, see the row loop)
-        unsigned long long lb_g = 0ull;
-        if (!have && have_pend) {                          // drain: no row loop ran, poll now
-            const int pr = pend.t & 31, pgrp = pend.t >> 5;
-            if (lane < pr) lb_w = ld_relaxed_desc(T.desc + ((size_t)pend.s * G.tiles_per_sub + (pend.t - pr) + lane) * 2);
-            if (lane < pgrp) lb_g = ld_relaxed_u64(T.gacc + (size_t)pend.s * G.lbgroups_per_sub + lane);
-        }
+        Poll lb;                                           // first look-back poll of the pending tile (early, see the row loop)
+        lb.a = lb.b = lb.c = 0ull;
+        if (!have && have_pend) poll_issue(lb, G, T, pend.s, pend.t, lane, epoch);      // drain: no row loop ran, poll now
 
-        // ================= push of the current tile: (push,) rank, update in place, publish the aggregate =================
+        // ================= push of the current tile: (push,) masks, update in place, publish the aggregate =================
         if (have) {
             TileBuf& W = my[bc];
             const int bn = bc + 1 == kNBuf ? 0 : bc + 1;
@@ -748,10 +741,9 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     codes_u |= (uint32_t)S.code[(uint32_t)s * cap32 + first + min(32u * rr + (uint32_t)lane, nvalid - 1u)] << (8 * rr);
                 wait_buf(bc);
             }
-            if (lane < kRows) W.stay_m[lane] = 0u;
-            __syncwarp();                  // lane 0 rewrites these words row by row
-            uint32_t cnt_c = 0;            // lane c: migrants of the tile so far with code c
             uint32_t n_mig = 0, n_stay = 0;
+#pragma unroll
+            for (int rr = 0; rr < kRows; ++rr) ti.stay[rr] = 0u;
             g_early = 0u;
             bool jump = false;
 #pragma unroll 1
@@ -767,16 +759,10 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     U = gather_reduce(Q, lane);
                 }
                 if (r + 1 == nrows) {
-                    // long-latency requests of the tile end, issued under the arithmetic of the last row (and BEFORE the
-                    // gather of the next row: ptxas tracks all of them on one scoreboard, so a load issued after the gather
-                    // would first wait for it): the ticket
-                    // of the tile after next, and the first look-back poll of the pending tile
-                    if (have_pend) {
-                        const int pr = pend.t & 31, pgrp = pend.t >> 5;
-                        if (lane < pr) lb_w = ld_relaxed_desc(T.desc + ((size_t)pend.s * G.tiles_per_sub + (pend.t - pr) + lane) * 2);
-                        if (lane < pgrp) lb_g = ld_relaxed_u64(T.gacc + (size_t)pend.s * G.lbgroups_per_sub + lane);
-                    }
-                    if (nxt.ok) g_early = take_issue();       // after the polls: they would wait on the atomic's scoreboard
+                    // long-latency requests of the tile end, issued under the arithmetic of the last row: the ticket of the
+                    // tile after next, and the first look-back poll of the pending tile
+                    if (have_pend) poll_issue(lb, G, T, pend.s, pend.t, lane, epoch);
+                    if (nxt.ok) g_early = take_issue();
                 }
                 if (kFused) {
                     // gather of the next row: of this tile, or row 0 of the next tile (whose bulk copy must have landed)
@@ -809,72 +795,64 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 } else {
                     code = min((int)((codes_u >> (8 * r)) & 0xffu), 26);
                 }
+                // a3/a4 at tile level: who stays (a mask per row, kept in registers) and who leaves (listed in slot order
+                // with its code; the per-code ranks are worked out where the migrants are dense, in k_send_scan / k_unpack)
                 const unsigned stay_m = __ballot_sync(0xffffffffu, valid && code == kStay);
                 const unsigned mig_m = __ballot_sync(0xffffffffu, valid && code != kStay);
-                if (mig_m) {
-                    const uint32_t rank = migrant_rank(code, mig_m, lane, cnt_c);
-                    if ((mig_m >> lane) & 1u)
-                        W.mlist[n_mig + __popc(mig_m & lt)] = p | ((uint32_t)code << 8) | (rank << 16);
-                    n_mig += __popc(mig_m);
-                }
-                if (lane == 0) W.stay_m[r] = stay_m;
+                if ((mig_m >> lane) & 1u) W.mlist[n_mig + __popc(mig_m & lt)] = (uint16_t)(p | ((uint32_t)code << 8));
+                n_mig += __popc(mig_m);
+#pragma unroll
+                for (int rr = 0; rr < kRows; ++rr) if (rr == r) ti.stay[rr] = stay_m;
                 n_stay += __popc(stay_m);
             }
             if (jump) raise(T.status, -5);
             __syncwarp();
-            // tile totals; publish the aggregate and the per-code byte counts
-            if (lane == kStay) cnt_c = n_stay;
-            const uint32_t magg = (lane < kNC && lane != kStay) ? cnt_c : 0u;
-            uint32_t inc = magg;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += nb;
+            // publish the tile aggregate: one word per level, [count : 24 | migrants : 20 | stayers : 20]; the group
+            // accumulators were zeroed before the launch
+            {
+                const size_t tile_row = (size_t)s * G.tiles_per_sub + t;
+                const unsigned long long agg = ((unsigned long long)n_mig << 20) | (unsigned long long)n_stay;
+                if (lane == 0) st_relaxed_u64(T.desc + tile_row, ((unsigned long long)epoch << 40) | agg);
+                if (lane == 1) atomicAdd(T.gacc + (size_t)s * G.lbgroups_per_sub + (t >> 5), (1ull << 40) | agg);
             }
-            const size_t tile_row = (size_t)s * G.tiles_per_sub + t;
-            T.tile_cnt[tile_row * 32 + lane] = (uint8_t)cnt_c;
-            if (lane < 2) st_relaxed_u64(T.desc + tile_row * 2 + lane, tag | (lane == 0 ? n_stay : n_mig));
-            if (lane == 2)      // group accumulator [tiles done : 24 | migrants : 20 | stayers : 20], zeroed before the launch
-                atomicAdd(T.gacc + (size_t)s * G.lbgroups_per_sub + (t >> 5),
-                          (1ull << 40) | ((unsigned long long)n_mig << 20) | (unsigned long long)n_stay);
-            ti.s = s; ti.t = t; ti.n_stay = n_stay; ti.n_mig = n_mig; ti.run_start = inc - magg;
+            ti.s = s; ti.t = t; ti.n_mig = n_mig;
             // ticket of the tile after next: taken right after this tile's aggregate is out
             if (nxt.ok) take_finish(nn, g_early);
         }
 
         // ================= resolve of the previous tile: look-back, then copy-out =================
-        // Two-level aggregate look-back (no prefix chain): exclusive prefix of tile t = aggregates of the
-        // earlier tiles of its group of 32 + accumulators of the earlier groups (every tile adds its
-        // aggregate to its group's accumulator with one 64-bit atomic right after its push).  Every word
-        // waited for is produced by the PUSH of a tile with a smaller ticket -- never by another tile's
-        // resolve -- and this warp has pushed a whole tile in between.
+        // Two-level aggregate look-back (no prefix chain, see poll_issue): every tile adds its aggregate to
+        // its group's accumulator with one 64-bit atomic right after its push.  Every word waited for is
+        // produced by the PUSH of a tile with a smaller ticket -- never by another tile's resolve -- and
+        // this warp has pushed a whole tile in between.
         if (have_pend) {
             const TileBuf& W = my[bp];
             const int s = pend.s, t = pend.t;
-            const size_t tile_row = (size_t)s * G.tiles_per_sub + t;
-            const int r = t & 31, grp = t >> 5;
-            uint32_t excl_stay = 0, excl_mig = 0;
-            if (r > 0) sum_descs(T.desc + (tile_row - r) * 2, r, lane, epoch, lb_w, excl_stay, excl_mig);
-            const unsigned long long* ga = T.gacc + (size_t)s * G.lbgroups_per_sub;
-            for (int g0 = 0; g0 < grp; g0 += 32) {
-                const bool need = g0 + lane < grp;
-                unsigned long long w = lb_g;
-                if (g0 > 0 && need) w = ld_relaxed_u64(ga + g0 + lane);
-                for (unsigned ns = 64;; ns = min(ns * 2u, 1024u)) {
-                    const bool ready = !need || (w >> 40) == 32ull;
-                    if (__all_sync(0xffffffffu, ready)) break;
-                    __nanosleep(ns);
-                    if (need) w = ld_relaxed_u64(ga + g0 + lane);
-                }
-                excl_stay += __reduce_add_sync(0xffffffffu, need ? (uint32_t)(w & 0xfffffull) : 0u);
-                excl_mig += __reduce_add_sync(0xffffffffu, need ? (uint32_t)((w >> 20) & 0xfffffull) : 0u);
+            for (unsigned ns = 32;; ns = min(ns * 2u, 512u)) {
+                if (__all_sync(0xffffffffu, poll_ready(lb, epoch))) break;
+                __nanosleep(ns);
+                poll_issue(lb, G, T, s, t, lane, epoch);
             }
+            uint32_t st = (uint32_t)(lb.a & kField20) + (uint32_t)(lb.b & kField20) + (uint32_t)(lb.c & kField20);
+            uint32_t mg = (uint32_t)((lb.a >> 20) & kField20) + (uint32_t)((lb.b >> 20) & kField20) +
+                          (uint32_t)((lb.c >> 20) & kField20);
+            for (int g0 = 64; g0 < (t >> 5); g0 += 32) {       // slabs of more than 64 full groups (> 4096 tiles): rare
+                const bool need = g0 + lane < (t >> 5);
+                const unsigned long long* pc = T.gacc + ((size_t)s * G.lbgroups_per_sub + g0 + (need ? lane : 0));
+                unsigned long long w = ld_relaxed_u64(pc);
+                for (unsigned ns = 32; !__all_sync(0xffffffffu, !need || (w >> 40) == 32ull); ns = min(ns * 2u, 512u)) {
+                    __nanosleep(ns);
+                    w = ld_relaxed_u64(pc);
+                }
+                if (need) { st += (uint32_t)(w & kField20); mg += (uint32_t)((w >> 20) & kField20); }
+            }
+            const uint32_t excl_stay = __reduce_add_sync(0xffffffffu, st);
+            const uint32_t excl_mig = __reduce_add_sync(0xffffffffu, mg);
             // copy-out, stayers: in place, compacted; the stayers of a row are consecutive lanes -> consecutive slots
             uint32_t base = (uint32_t)s * cap32 + excl_stay;
-#pragma unroll 1
+#pragma unroll
             for (int rr = 0; rr < kRows; ++rr) {
-                const unsigned m = W.stay_m[rr];
-                if (m == 0u) continue;
+                const unsigned m = pend.stay[rr];
                 if ((m >> lane) & 1u) {
                     const uint32_t dst = base + __popc(m & lt);
                     const uint32_t src = 32u * (uint32_t)rr + (uint32_t)lane;
@@ -884,22 +862,21 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 }
                 base += __popc(m);
             }
-            // copy-out, migrants: to the send region of s, grouped by code inside the tile's chunk
+            // copy-out, migrants: to the send region of s in slot order, each with its code byte
             if (pend.n_mig) {
                 const bool fits = (long long)excl_mig + (long long)pend.n_mig <= G.send_cap;
                 if (!fits && lane == 0) raise(T.status, -4);
                 const uint32_t sendbase = (uint32_t)s * (uint32_t)G.send_cap + excl_mig;      // P*send_cap <= P*cap < 2^31
                 for (uint32_t a0 = 0; a0 < pend.n_mig; a0 += 32) {
                     const uint32_t a = a0 + lane;
-                    const bool ok = a < pend.n_mig;
-                    const uint32_t e = ok ? W.mlist[a] : 0u;
-                    const uint32_t off = __shfl_sync(0xffffffffu, pend.run_start, (e >> 8) & 31u) + (e >> 16);
-                    if (ok && fits) {
-                        const uint32_t dst = sendbase + off;
+                    if (a < pend.n_mig && fits) {
+                        const uint32_t e = W.mlist[a];
+                        const uint32_t dst = sendbase + a;
                         const uint32_t src = e & 0xffu;
 #pragma unroll
                         for (int q = 0; q < 7; ++q) st_stream(Snd.f[q] + dst, W.f[q][src]);
                         st_stream(Snd.id + dst, W.f[7][src]);
+                        Snd.code[dst] = (uint8_t)(e >> 8);
                     }
                 }
             }
@@ -916,35 +893,78 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2b: per-(subdomain, code) exclusive scan of tile_cnt over the tiles of the subdomain, kept at
-// group granularity (kGroup tiles) for the unpack, and the count table totals cnt[s][c] (a4/a5).
-// One CTA per subdomain, lane c owns code c.
+// K2b (a4/a5 for the migrants): the send region of a subdomain holds its migrants in slot order, each with its code.
+// Per chunk of kChunk migrants: the per-code counts, then their exclusive prefix over the chunks of the region (what
+// the unpack needs to turn "k-th migrant with code c of the region" into a slot of the receiver), and the totals
+// cnt[s][c] of the count table; cnt[s][13] = stayers.  One CTA of 8 warps per subdomain, lane c owns code c; each warp
+// takes a contiguous range of chunks.  The totals of the region come from the look-back accumulators of the tile pass.
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t chunk_hist(const uint8_t* __restrict__ codes, uint32_t n, int lane)
+{   // lane c: how many of the n <= kChunk codes are c
+    uint32_t cnt = 0;
+    for (uint32_t i0 = 0; i0 < n; i0 += 32) {
+        const uint32_t i = i0 + lane;
+        const int code = i < n ? (int)codes[i] : kInvalid;
+        unsigned todo = __ballot_sync(0xffffffffu, code != kInvalid);
+        while (todo) {
+            const int c = __shfl_sync(0xffffffffu, code, __ffs(todo) - 1);
+            const unsigned m = __ballot_sync(0xffffffffu, code == c);
+            if (lane == c) cnt += __popc(m);
+            todo &= ~m;
+        }
+    }
+    return cnt;
+}
+
 __global__ void __launch_bounds__(256)
-k_code_scan(Geom G, Tables T)
+k_send_scan(Geom G, Slabs Snd, Tables T)
 {
     __shared__ uint32_t s_part[8][32];
+    __shared__ uint32_t s_tot[2];
     const int s = blockIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint32_t cnt_s = T.count[s];
-    const int nt = (int)((cnt_s + kTile - 1) / kTile);
-    const int ng = (nt + kGroup - 1) / kGroup;
-    const int gchunk = (ng + 7) / 8;
-    const int g0 = min(ng, warp * gchunk), g1 = min(ng, g0 + gchunk);
-    const int t0 = g0 * kGroup, t1 = min(nt, g1 * kGroup);
-    const size_t row0 = (size_t)s * G.tiles_per_sub;
+    // totals of the slab: sum of the group accumulators [count : 24 | migrants : 20 | stayers : 20]
+    if (threadIdx.x < 2) s_tot[threadIdx.x] = 0u;
+    __syncthreads();
+    {
+        const uint32_t cnt_s = T.count[s];
+        const int nt = (int)((cnt_s + kTile - 1) / kTile);
+        const int ngrp = (nt + 31) / 32;
+        uint32_t st = 0, mg = 0;
+        for (int g = threadIdx.x; g < ngrp; g += 256) {
+            const unsigned long long w = T.gacc[(size_t)s * G.lbgroups_per_sub + g];
+            st += (uint32_t)(w & kField20); mg += (uint32_t)((w >> 20) & kField20);
+        }
+        st = warp_sum(st); mg = warp_sum(mg);
+        if (lane == 0 && (st | mg)) { atomicAdd(&s_tot[0], st); atomicAdd(&s_tot[1], mg); }
+    }
+    __syncthreads();
+    const uint32_t n_stay = s_tot[0];
+    const uint32_t n_mig = (uint32_t)min((unsigned long long)s_tot[1], (unsigned long long)G.send_cap);   // overflow: already raised
+    const int nch = (int)((n_mig + kChunk - 1) / kChunk);
+    const int per = (nch + 7) / 8;
+    const int q0 = min(nch, warp * per), q1 = min(nch, q0 + per);
+    const uint8_t* codes = Snd.code + (size_t)s * (size_t)G.send_cap;
+    uint32_t* ce = T.chunk_excl + (size_t)s * G.chunks_per_sub * 32;
     uint32_t sum = 0;
-    for (int t = t0; t < t1; ++t) sum += T.tile_cnt[(row0 + t) * 32 + lane];
+    for (int q = q0; q < q1; ++q) {
+        const uint32_t c = chunk_hist(codes + (size_t)q * kChunk, min((uint32_t)kChunk, n_mig - (uint32_t)q * kChunk), lane);
+        ce[(size_t)q * 32 + lane] = c;
+        sum += c;
+    }
     s_part[warp][lane] = sum;
     __syncthreads();
     uint32_t run = 0, total = 0;
     for (int w = 0; w < 8; ++w) { const uint32_t v = s_part[w][lane]; if (w < warp) run += v; total += v; }
-    for (int g = g0; g < g1; ++g) {
-        T.group_excl[((size_t)s * G.groups_per_sub + g) * 32 + lane] = run;
-        const int te = min(nt, (g + 1) * kGroup);
-        for (int t = g * kGroup; t < te; ++t) run += T.tile_cnt[(row0 + t) * 32 + lane];
+    for (int q = q0; q < q1; ++q) {                       // counts -> exclusive prefix, in place (this warp wrote them)
+        const uint32_t c = ce[(size_t)q * 32 + lane];
+        ce[(size_t)q * 32 + lane] = run;
+        run += c;
     }
-    if (warp == 0) T.cnt[s * 32 + lane] = total;
+    if (warp == 0) {
+        T.cnt[s * 32 + lane] = (lane == kStay) ? n_stay : total;
+        if (lane == 0) T.send_count[s] = n_mig;
+    }
     if (s == 0 && threadIdx.x == 0) { *T.n_migrated = 0ull; *T.n_total = 0ull; }   // k_table accumulates them
 }
 
@@ -1023,67 +1043,76 @@ k_table(Geom G, Tables T)
 }
 
 // ---------------------------------------------------------------------------------------------
-// K4: unpack / append (a8).  One warp per group of kGroup tiles of one subdomain's send region;
-// lane c owns code c: it carries the exclusive prefix of its code and copies its run of every
-// tile chunk to slab[receiver(s,c)] + recv_off[s][c] + prefix.
+// K4: unpack / append (a8).  One warp per chunk of kChunk migrants of one subdomain's send region.  Lane c owns code c:
+// it carries the slot of the next code-c migrant in slab[receiver(s,c)], i.e. recv_off[s][c] + the exclusive prefix of
+// the chunk.  The migrants of the chunk are ranked row by row (stable: slot order inside a code) and at the same time
+// sorted by code in shared memory, so that the copy that follows writes runs: consecutive lanes, consecutive slots of one
+// receiver.  The reads from the send region are scattered only inside the chunk's 2 KB per array.
 // ---------------------------------------------------------------------------------------------
 #ifndef LCS_UNPACK_WARPS
-#define LCS_UNPACK_WARPS 2
+#define LCS_UNPACK_WARPS 4
 #endif
 constexpr int kUnpackWarps = LCS_UNPACK_WARPS;
 
 __global__ void __launch_bounds__(32 * kUnpackWarps)
 k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
 {
+    __shared__ uint32_t s_dst[kUnpackWarps][kChunk];      // sorted by code: destination slot (global index)
+    __shared__ uint8_t s_src[kUnpackWarps][kChunk];       // sorted by code: position in the chunk
     const int s = blockIdx.y;
-    const int lane = threadIdx.x & 31;
-    const int grp = blockIdx.x * kUnpackWarps + (threadIdx.x >> 5);
-    const uint32_t cnt_s = T.count[s];
-    const int nt = (int)((cnt_s + kTile - 1) / kTile);
-    const int t0 = grp * kGroup;
-    if (t0 >= nt) return;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int q = blockIdx.x * kUnpackWarps + w;
+    const uint32_t n_mig = T.send_count[s];
+    if ((uint32_t)q * kChunk >= n_mig) return;
     if (*T.status != 0) return;                                 // contents unspecified after an error
-    const int t1 = min(nt, t0 + kGroup);
+    const uint32_t n = min((uint32_t)kChunk, n_mig - (uint32_t)q * kChunk);
     const bool mig = lane < kNC && lane != kStay;
-    const size_t row0 = (size_t)s * G.tiles_per_sub;
-    uint32_t n[kGroup];
+    const uint32_t* ce = T.chunk_excl + ((size_t)s * G.chunks_per_sub + q) * 32;
+    const uint32_t pre = mig ? ce[lane] : 0u;
+    // per-code count of THIS chunk = next chunk's prefix - this one's (or the region total for the last chunk)
+    const uint32_t nextpre = mig ? (((uint32_t)(q + 1) * kChunk < n_mig) ? ce[32 + lane] : T.cnt[s * 32 + lane]) : 0u;
+    const uint32_t mine = nextpre - pre;
+    uint32_t sorted_at = mine;                                  // exclusive scan over the codes: start of code c's run in the sorted chunk
 #pragma unroll
-    for (int q = 0; q < kGroup; ++q) n[q] = (mig && t0 + q < t1) ? T.tile_cnt[(row0 + t0 + q) * 32 + lane] : 0u;
-    uint32_t pre = mig ? T.group_excl[((size_t)s * G.groups_per_sub + grp) * 32 + lane] : 0u;
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t nb = __shfl_up_sync(0xffffffffu, sorted_at, o);
+        if (lane >= o) sorted_at += nb;
+    }
+    sorted_at -= mine;
     const uint32_t roff = mig ? T.recv_off[s * 32 + lane] : 0u;
-    const size_t recv0 = mig ? (size_t)receiver_of(G, s, lane) * (size_t)G.cap + roff : 0;
-    // phase 1: destination slot of every migrant of the group, in send-region order (shared memory list)
-    __shared__ unsigned long long s_dst[kUnpackWarps][kGroup * kTile];
-    unsigned long long* dstl = s_dst[threadIdx.x >> 5];
-    const size_t send0 = (size_t)s * (size_t)G.send_cap + warp_sum(pre);
-    uint32_t nlist = 0;
-#pragma unroll
-    for (int q = 0; q < kGroup; ++q) {
-        if (t0 + q >= t1) break;
-        uint32_t inc = n[q];
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += nb;
+    // memory safety if counts were clamped after an overflow: such migrants are dropped (the status word is set then)
+    const bool fits = (unsigned long long)roff + pre + mine <= (unsigned long long)G.cap;
+    uint32_t next_dst = mig ? (uint32_t)receiver_of(G, s, lane) * (uint32_t)G.cap + roff + pre : 0u;   // < P*cap < 2^31
+    const size_t send0 = (size_t)s * (size_t)G.send_cap + (size_t)q * kChunk;
+    const unsigned lt = (1u << lane) - 1u;
+    for (uint32_t i0 = 0; i0 < n; i0 += 32) {
+        const uint32_t i = i0 + lane;
+        const int code = i < n ? min((int)Snd.code[send0 + i], 26) : kInvalid;
+        unsigned todo = __ballot_sync(0xffffffffu, code != kInvalid);
+        while (todo) {
+            const int c = __shfl_sync(0xffffffffu, code, __ffs(todo) - 1);
+            const unsigned m = __ballot_sync(0xffffffffu, code == c);
+            const uint32_t d0 = __shfl_sync(0xffffffffu, next_dst, c);
+            const uint32_t a0 = __shfl_sync(0xffffffffu, sorted_at, c);
+            const bool ok = __shfl_sync(0xffffffffu, (int)fits, c) != 0;
+            if (code == c) {
+                const uint32_t k = __popc(m & lt);
+                s_dst[w][a0 + k] = ok ? d0 + k : 0xffffffffu;
+                s_src[w][a0 + k] = (uint8_t)i;
+            }
+            if (lane == c) { next_dst += __popc(m); sorted_at += __popc(m); }
+            todo &= ~m;
         }
-        const uint32_t ntile = __shfl_sync(0xffffffffu, inc, 31);
-        // memory safety if counts were clamped after an overflow: such migrants are dropped
-        const bool fits = (uint64_t)roff + pre + n[q] <= (uint64_t)G.cap;
-        const uint32_t at = nlist + (inc - n[q]);
-        for (uint32_t k = 0; k < n[q]; ++k) dstl[at + k] = fits ? (unsigned long long)(recv0 + pre + k) : ~0ull;
-        pre += n[q];
-        nlist += ntile;
     }
     __syncwarp();
-    // phase 2: one lane per migrant; the reads from the send region are contiguous across lanes
-    for (uint32_t i = lane; i < nlist; i += 32) {
-        const unsigned long long dst = dstl[i];
-        if (dst == ~0ull) continue;
-        const size_t src = send0 + i;
+    for (uint32_t j = lane; j < n; j += 32) {
+        const uint32_t dst = s_dst[w][j];
+        if (dst == 0xffffffffu) continue;
+        const size_t src = send0 + s_src[w][j];
         unsigned long long v[8];
 #pragma unroll
-        for (int a = 0; a < 7; ++a) v[a] = ld_stream(Snd.f[a] + src);
-        v[7] = ld_stream(Snd.id + src);
+        for (int a = 0; a < 7; ++a) v[a] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.f[a] + src));
+        v[7] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.id + src));
 #pragma unroll
         for (int a = 0; a < 7; ++a) S.f[a][dst] = __longlong_as_double(v[a]);
         S.id[dst] = (int64_t)v[7];
