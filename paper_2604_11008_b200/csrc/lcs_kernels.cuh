@@ -899,27 +899,28 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
 // cnt[s][c] of the count table; cnt[s][13] = stayers.  One CTA of 8 warps per subdomain, lane c owns code c; each warp
 // takes a contiguous range of chunks.  The totals of the region come from the look-back accumulators of the tile pass.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t chunk_hist(const uint8_t* __restrict__ codes, uint32_t n, int lane)
-{   // lane c: how many of the n <= kChunk codes are c
-    uint32_t cnt = 0;
+__device__ __forceinline__ uint32_t chunk_hist(const uint8_t* __restrict__ codes, uint32_t n, int lane, uint32_t* s_cnt)
+{   // lane c: how many of the n <= kChunk codes are c.  Integer shared-memory atomics on the warp's 32 counters (counts
+    // do not depend on the order of the additions); lanes with the same code are combined first (match)
+    s_cnt[lane] = 0u;
+    __syncwarp();
     for (uint32_t i0 = 0; i0 < n; i0 += 32) {
         const uint32_t i = i0 + lane;
-        const int code = i < n ? (int)codes[i] : kInvalid;
-        unsigned todo = __ballot_sync(0xffffffffu, code != kInvalid);
-        while (todo) {
-            const int c = __shfl_sync(0xffffffffu, code, __ffs(todo) - 1);
-            const unsigned m = __ballot_sync(0xffffffffu, code == c);
-            if (lane == c) cnt += __popc(m);
-            todo &= ~m;
-        }
+        const int code = i < n ? min((int)codes[i], 26) : kInvalid;
+        const unsigned m = __match_any_sync(0xffffffffu, code);
+        if (code != kInvalid && (m & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_cnt[code], (uint32_t)__popc(m));
     }
-    return cnt;
+    __syncwarp();
+    const uint32_t c = s_cnt[lane];
+    __syncwarp();
+    return c;
 }
 
 __global__ void __launch_bounds__(256)
 k_send_scan(Geom G, Slabs Snd, Tables T)
 {
     __shared__ uint32_t s_part[8][32];
+    __shared__ uint32_t s_hist[8][32];
     __shared__ uint32_t s_tot[2];
     const int s = blockIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -948,7 +949,7 @@ k_send_scan(Geom G, Slabs Snd, Tables T)
     uint32_t* ce = T.chunk_excl + (size_t)s * G.chunks_per_sub * 32;
     uint32_t sum = 0;
     for (int q = q0; q < q1; ++q) {
-        const uint32_t c = chunk_hist(codes + (size_t)q * kChunk, min((uint32_t)kChunk, n_mig - (uint32_t)q * kChunk), lane);
+        const uint32_t c = chunk_hist(codes + (size_t)q * kChunk, min((uint32_t)kChunk, n_mig - (uint32_t)q * kChunk), lane, s_hist[warp]);
         ce[(size_t)q * 32 + lane] = c;
         sum += c;
     }
@@ -1059,14 +1060,18 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
 {
     __shared__ uint32_t s_dst[kUnpackWarps][kChunk];      // sorted by code: destination slot (global index)
     __shared__ uint8_t s_src[kUnpackWarps][kChunk];       // sorted by code: position in the chunk
+    __shared__ uint32_t s_next[kUnpackWarps][32], s_at[kUnpackWarps][32];
     const int s = blockIdx.y;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int q = blockIdx.x * kUnpackWarps + w;
     const uint32_t n_mig = T.send_count[s];
+    const int q = blockIdx.x * kUnpackWarps + w;                // one chunk per warp: the copy needs many warps in flight
     if ((uint32_t)q * kChunk >= n_mig) return;
     if (*T.status != 0) return;                                 // contents unspecified after an error
-    const uint32_t n = min((uint32_t)kChunk, n_mig - (uint32_t)q * kChunk);
     const bool mig = lane < kNC && lane != kStay;
+    const uint32_t roff = mig ? T.recv_off[s * 32 + lane] : 0u;
+    const uint32_t recv0 = mig ? (uint32_t)receiver_of(G, s, lane) * (uint32_t)G.cap + roff : 0u;     // < P*cap < 2^31
+    const unsigned lt = (1u << lane) - 1u;
+    const uint32_t n = min((uint32_t)kChunk, n_mig - (uint32_t)q * kChunk);
     const uint32_t* ce = T.chunk_excl + ((size_t)s * G.chunks_per_sub + q) * 32;
     const uint32_t pre = mig ? ce[lane] : 0u;
     // per-code count of THIS chunk = next chunk's prefix - this one's (or the region total for the last chunk)
@@ -1079,43 +1084,61 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
         if (lane >= o) sorted_at += nb;
     }
     sorted_at -= mine;
-    const uint32_t roff = mig ? T.recv_off[s * 32 + lane] : 0u;
     // memory safety if counts were clamped after an overflow: such migrants are dropped (the status word is set then)
     const bool fits = (unsigned long long)roff + pre + mine <= (unsigned long long)G.cap;
-    uint32_t next_dst = mig ? (uint32_t)receiver_of(G, s, lane) * (uint32_t)G.cap + roff + pre : 0u;   // < P*cap < 2^31
+    // running state per code, in shared memory: slot of the next code-c migrant in its receiver (0xffffffff = dropped)
+    // and its place in the chunk sorted by code
+    s_next[w][lane] = (mig && fits) ? recv0 + pre : 0xffffffffu;
+    s_at[w][lane] = sorted_at;
+    __syncwarp();
     const size_t send0 = (size_t)s * (size_t)G.send_cap + (size_t)q * kChunk;
-    const unsigned lt = (1u << lane) - 1u;
     for (uint32_t i0 = 0; i0 < n; i0 += 32) {
         const uint32_t i = i0 + lane;
         const int code = i < n ? min((int)Snd.code[send0 + i], 26) : kInvalid;
-        unsigned todo = __ballot_sync(0xffffffffu, code != kInvalid);
-        while (todo) {
-            const int c = __shfl_sync(0xffffffffu, code, __ffs(todo) - 1);
-            const unsigned m = __ballot_sync(0xffffffffu, code == c);
-            const uint32_t d0 = __shfl_sync(0xffffffffu, next_dst, c);
-            const uint32_t a0 = __shfl_sync(0xffffffffu, sorted_at, c);
-            const bool ok = __shfl_sync(0xffffffffu, (int)fits, c) != 0;
-            if (code == c) {
-                const uint32_t k = __popc(m & lt);
-                s_dst[w][a0 + k] = ok ? d0 + k : 0xffffffffu;
-                s_src[w][a0 + k] = (uint8_t)i;
+        const unsigned m = __match_any_sync(0xffffffffu, code);           // the lanes of this row with my code
+        const int leader = __ffs(m) - 1;
+        uint32_t d0 = 0u, a0 = 0u;
+        if (lane == leader && code != kInvalid) { d0 = s_next[w][code]; a0 = s_at[w][code]; }
+        d0 = __shfl_sync(0xffffffffu, d0, leader);
+        a0 = __shfl_sync(0xffffffffu, a0, leader);
+        if (code != kInvalid) {
+            const uint32_t k = __popc(m & lt);                            // stable: slot order inside a code
+            s_dst[w][a0 + k] = d0 == 0xffffffffu ? d0 : d0 + k;
+            s_src[w][a0 + k] = (uint8_t)i;
+            if (lane == leader) {
+                const uint32_t c = __popc(m);
+                if (d0 != 0xffffffffu) s_next[w][code] = d0 + c;
+                s_at[w][code] = a0 + c;
             }
-            if (lane == c) { next_dst += __popc(m); sorted_at += __popc(m); }
-            todo &= ~m;
         }
+        __syncwarp();
     }
     __syncwarp();
-    for (uint32_t j = lane; j < n; j += 32) {
-        const uint32_t dst = s_dst[w][j];
-        if (dst == 0xffffffffu) continue;
-        const size_t src = send0 + s_src[w][j];
-        unsigned long long v[8];
+    // copy: two migrants per lane and iteration (16 loads in flight), consecutive lanes on consecutive slots of a receiver
+    for (uint32_t j0 = 0; j0 < n; j0 += 64) {
+        uint32_t dst[2];
+        size_t src[2];
+        unsigned long long v[2][8];
 #pragma unroll
-        for (int a = 0; a < 7; ++a) v[a] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.f[a] + src));
-        v[7] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.id + src));
+        for (int u = 0; u < 2; ++u) {
+            const uint32_t j = j0 + 32u * u + lane;
+            dst[u] = j < n ? s_dst[w][j] : 0xffffffffu;
+            src[u] = send0 + (j < n ? s_src[w][j] : 0);
+        }
 #pragma unroll
-        for (int a = 0; a < 7; ++a) S.f[a][dst] = __longlong_as_double(v[a]);
-        S.id[dst] = (int64_t)v[7];
+        for (int u = 0; u < 2; ++u)
+            if (dst[u] != 0xffffffffu) {
+#pragma unroll
+                for (int a = 0; a < 7; ++a) v[u][a] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.f[a] + src[u]));
+                v[u][7] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.id + src[u]));
+            }
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+            if (dst[u] != 0xffffffffu) {
+#pragma unroll
+                for (int a = 0; a < 7; ++a) S.f[a][dst[u]] = __longlong_as_double(v[u][a]);
+                S.id[dst[u]] = (int64_t)v[u][7];
+            }
     }
 }
 
