@@ -335,16 +335,17 @@ int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y,
     uint32_t* tilehist = reinterpret_cast<uint32_t*>(static_cast<char*>(h->pool) + align_up((size_t)G.P * (size_t)G.cap * 4));
     if (ntiles > 0)
         k_set_owner<<<ntiles, 256, (size_t)G.P * 4, h->stream>>>(G, h->T, n, d_x, d_y, d_z, owner, tilehist);
-    k_set_scan<<<(G.P + 127) / 128, 128, 0, h->stream>>>(G, h->T, ntiles, tilehist, n);
+    k_set_scan<<<(G.P + 31) / 32, 1024, 0, h->stream>>>(G, h->T, ntiles, tilehist, n);
     k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, 0);
     if (ntiles > 0) {
-        int wpb = (int)(32768 / ((size_t)G.P * 4));
-        wpb = wpb < 1 ? 1 : (wpb > 4 ? 4 : wpb);
+        int W = 8;                                                           // warps per tile, a power of two: W * P 16-bit
+        while (W > 1 && W * G.P > 16384) W >>= 1;                             // counters in shared memory
+        const size_t smem = ((size_t)(W + 1) * G.P + 2 * kSetTile + 1) * 2 + (size_t)kSetTile * 4 + 16;
+        cudaFuncSetAttribute(k_set_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         InPtrs I;
         I.f[0] = d_x; I.f[1] = d_y; I.f[2] = d_z; I.f[3] = d_vx; I.f[4] = d_vy; I.f[5] = d_vz; I.f[6] = d_diam;
         I.id = d_id;
-        k_set_scatter<<<(ntiles + wpb - 1) / wpb, 32 * wpb, (size_t)wpb * G.P * 4, h->stream>>>(G, h->S, n, I, owner,
-                                                                                                 tilehist, wpb);
+        k_set_scatter<<<ntiles, 32 * W, smem, h->stream>>>(G, h->S, n, I, owner, tilehist, W);
     }
     return check_launch(h, ntiles > 0 ? 4 : 2);
 }

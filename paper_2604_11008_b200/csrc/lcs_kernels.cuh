@@ -1370,54 +1370,141 @@ k_set_owner(Geom G, Tables T, int64_t n, const double* __restrict__ x, const dou
     for (int p = threadIdx.x; p < G.P; p += blockDim.x) tilehist[(size_t)blockIdx.x * G.P + p] = s_hist[p];
 }
 
-__global__ void k_set_scan(Geom G, Tables T, int ntiles, uint32_t* __restrict__ tilehist, int64_t n)
-{   // thread p: exclusive scan of bucket p over tiles (in place), total -> count[p]
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p == 0) *T.n_total = (unsigned long long)n;
-    if (p >= G.P) return;
-    uint64_t run = 0;
-    for (int t = 0; t < ntiles; ++t) {
-        const uint32_t v = tilehist[(size_t)t * G.P + p];
-        tilehist[(size_t)t * G.P + p] = (uint32_t)min(run, (uint64_t)0xffffffffu);
-        run += v;
+// Exclusive scan of every bucket's count over the tiles (in place in tilehist[tile][bucket]), totals -> count[].
+// One CTA of 32 warps per 32 consecutive buckets (lane = bucket, so every row read is one 128-byte line); warp w owns a
+// contiguous range of tiles: sum, exchange through shared memory, then prefix.
+__global__ void __launch_bounds__(1024)
+k_set_scan(Geom G, Tables T, int ntiles, uint32_t* __restrict__ tilehist, int64_t n)
+{
+    __shared__ unsigned long long s_part[32][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int p = blockIdx.x * 32 + lane;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *T.n_total = (unsigned long long)n;
+    const bool ok = p < G.P;
+    const int per = (ntiles + 31) / 32;
+    const int t0 = min(ntiles, warp * per), t1 = min(ntiles, t0 + per);
+    unsigned long long sum = 0;
+    if (ok)
+        for (int t = t0; t < t1; ++t) sum += tilehist[(size_t)t * G.P + p];
+    s_part[warp][lane] = sum;
+    __syncthreads();
+    unsigned long long run = 0, total = 0;
+    for (int w = 0; w < 32; ++w) { const unsigned long long v = s_part[w][lane]; if (w < warp) run += v; total += v; }
+    if (ok)
+        for (int t = t0; t < t1; ++t) {
+            const uint32_t v = tilehist[(size_t)t * G.P + p];
+            tilehist[(size_t)t * G.P + p] = (uint32_t)min(run, 0xffffffffull);
+            run += v;
+        }
+    if (ok && warp == 0) {
+        if (total > (unsigned long long)G.cap) { raise(T.status, -4); total = (unsigned long long)G.cap; }
+        T.count[p] = (uint32_t)total;
+        for (int c = 0; c < 32; ++c) T.cnt[p * 32 + c] = (c == kStay) ? (uint32_t)total : 0u;
     }
-    if (run > (uint64_t)G.cap) { raise(T.status, -4); run = (uint64_t)G.cap; }
-    T.count[p] = (uint32_t)run;
-    for (int c = 0; c < 32; ++c) T.cnt[p * 32 + c] = (c == kStay) ? (uint32_t)run : 0u;
 }
 
 struct InPtrs { const double* f[7]; const int64_t* id; };
 
-__global__ void __launch_bounds__(128)
+// Stable scatter of one tile of kSetTile particles (a block-level counting sort): W warps, each owning a contiguous
+// part of the tile.  (1) per-warp stable rank of every particle among those of the same owner (match + a 16-bit
+// counter per (warp, owner) in shared memory); (2) the counters become exclusive prefixes across the warps, and the
+// tile's per-owner counts an exclusive prefix over the owners: the position of every particle in the tile SORTED BY
+// OWNER; (3) the copy walks the sorted order, so consecutive threads write the run of one owner to consecutive slots of
+// its slab.  Shared memory (dynamic): cntw[W][P] u16, sbase[P] u16, rk[kSetTile] u16, src[kSetTile] u16, dst[kSetTile] u32.
+__global__ void __launch_bounds__(256)
 k_set_scatter(Geom G, Slabs S, int64_t n, InPtrs I, const int32_t* __restrict__ owner,
-              const uint32_t* __restrict__ tileoff, int warps_per_block)
-{   // one warp per tile, sequential 32-particle rounds: stable rank = running bucket counter + match rank
-    extern __shared__ uint32_t s_run[];
+              const uint32_t* __restrict__ tileoff, int W)
+{
+    extern __shared__ __align__(16) unsigned char s_set[];
+    const int P = G.P;
+    uint16_t* cntw = reinterpret_cast<uint16_t*>(s_set);                       // [W][P]
+    uint16_t* sbase = cntw + (size_t)W * P;                                    // [P]
+    uint16_t* rk = sbase + P;                                                  // [kSetTile]
+    uint16_t* srcl = rk + kSetTile;                                            // [kSetTile]
+    uint32_t* dstl = reinterpret_cast<uint32_t*>(srcl + kSetTile + ((P * (W + 1)) & 1));   // [kSetTile], 4-byte aligned
+    __shared__ uint32_t s_scan[256];
+    const int nthr = 32 * W;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t tile = (int64_t)blockIdx.x * warps_per_block + warp;
-    const int64_t first = tile * kSetTile;
-    if (first >= n) return;
-    uint32_t* run = s_run + (size_t)warp * G.P;
-    for (int p = lane; p < G.P; p += 32) run[p] = tileoff[(size_t)tile * G.P + p];
-    __syncwarp();
-    const int64_t end = min(first + kSetTile, n);
-    for (int64_t i0 = first; i0 < end; i0 += 32) {
-        const int64_t i = i0 + lane;
-        const bool valid = i < end;
-        const int ow = valid ? owner[i] : -1 - lane;            // distinct dummies never match
+    const int64_t first = (int64_t)blockIdx.x * kSetTile;
+    const int ntile = (int)min((int64_t)kSetTile, n - first);
+    const int perw = kSetTile / W;                                             // particles per warp (a multiple of 32)
+    for (int i = threadIdx.x; i < W * P; i += nthr) cntw[i] = 0;
+    __syncthreads();
+    // (1) stable rank inside the warp's part
+    const unsigned lt = (1u << lane) - 1u;
+    for (int r0 = 0; r0 < perw; r0 += 32) {
+        const int l = warp * perw + r0 + lane;                                 // index in the tile
+        const int ow = l < ntile ? owner[first + l] : -1 - lane;               // distinct dummies never match
         const unsigned m = __match_any_sync(0xffffffffu, ow);
-        const uint32_t rank = __popc(m & ((1u << lane) - 1u));
-        uint32_t slot = 0;
-        if (valid) slot = run[ow] + rank;
-        __syncwarp();
-        if (valid && rank == (uint32_t)__popc(m) - 1u) run[ow] = slot + 1u;   // last lane of the group
-        __syncwarp();
-        if (valid && (int64_t)slot < G.cap) {
-            const size_t dst = (size_t)ow * (size_t)G.cap + slot;
-#pragma unroll
-            for (int a = 0; a < 7; ++a) S.f[a][dst] = I.f[a][i];
-            S.id[dst] = I.id[i];
+        const int leader = __ffs(m) - 1;
+        uint32_t old = 0;
+        if (lane == leader && ow >= 0) {
+            old = cntw[(size_t)warp * P + ow];
+            cntw[(size_t)warp * P + ow] = (uint16_t)(old + __popc(m));
         }
+        old = __shfl_sync(0xffffffffu, old, leader);
+        if (ow >= 0) rk[l] = (uint16_t)(old + __popc(m & lt));
+        __syncwarp();
+    }
+    __syncthreads();
+    // (2) per owner: exclusive prefix across the warps; tile total -> sbase, then exclusive scan of sbase over the owners
+    for (int p = threadIdx.x; p < P; p += nthr) {
+        uint32_t run = 0;
+        for (int w = 0; w < W; ++w) { const uint32_t c = cntw[(size_t)w * P + p]; cntw[(size_t)w * P + p] = (uint16_t)run; run += c; }
+        sbase[p] = (uint16_t)run;                                              // <= kSetTile = 4096
+    }
+    __syncthreads();
+    {
+        const int per = (P + nthr - 1) / nthr;
+        const int p0 = min(P, (int)threadIdx.x * per), p1 = min(P, p0 + per);
+        uint32_t sum = 0;
+        for (int p = p0; p < p1; ++p) sum += sbase[p];
+        s_scan[threadIdx.x] = sum;
+        __syncthreads();
+        uint32_t run = 0;
+        for (int t = 0; t < (int)threadIdx.x; ++t) run += s_scan[t];
+        for (int p = p0; p < p1; ++p) { const uint32_t c = sbase[p]; sbase[p] = (uint16_t)run; run += c; }
+    }
+    __syncthreads();
+    // (3) sorted lists
+    const uint32_t* toff = tileoff + (size_t)blockIdx.x * P;
+    for (int r0 = 0; r0 < perw; r0 += 32) {
+        const int l = warp * perw + r0 + lane;
+        if (l < ntile) {
+            const int ow = owner[first + l];
+            const uint32_t inw = (uint32_t)cntw[(size_t)warp * P + ow] + rk[l];   // rank among the tile's particles of this owner
+            const uint32_t pos = (uint32_t)sbase[ow] + inw;
+            const unsigned long long slot = (unsigned long long)toff[ow] + inw;
+            srcl[pos] = (uint16_t)l;
+            dstl[pos] = slot < (unsigned long long)G.cap ? (uint32_t)ow * (uint32_t)G.cap + (uint32_t)slot : 0xffffffffu;
+        }
+    }
+    __syncthreads();
+    // copy in sorted order, two particles per thread and iteration
+    for (int j0 = 0; j0 < ntile; j0 += 2 * nthr) {
+        uint32_t dst[2];
+        int64_t src[2];
+        unsigned long long v[2][8];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int j = j0 + u * nthr + (int)threadIdx.x;
+            dst[u] = j < ntile ? dstl[j] : 0xffffffffu;
+            src[u] = first + (j < ntile ? srcl[j] : 0);
+        }
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+            if (dst[u] != 0xffffffffu) {
+#pragma unroll
+                for (int a = 0; a < 7; ++a) v[u][a] = __ldg(reinterpret_cast<const unsigned long long*>(I.f[a] + src[u]));
+                v[u][7] = __ldg(reinterpret_cast<const unsigned long long*>(I.id + src[u]));
+            }
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+            if (dst[u] != 0xffffffffu) {
+#pragma unroll
+                for (int a = 0; a < 7; ++a) S.f[a][dst[u]] = __longlong_as_double(v[u][a]);
+                S.id[dst[u]] = (int64_t)v[u][7];
+            }
     }
 }
 
