@@ -29,6 +29,9 @@
  *                          particle is in its owner's slab and the slabs hold the same id sets as the direct 27-way migrate
  *   orc_migrate            paper's worked example; global-sort brute force;
  *                          conservation; containment; idempotence
+ *   orc_rk2_stage x drag 1 Heun written out with libm pow, f re-evaluated from the slip of each stage
+ *   orc_pair_count         hand-countable lattices, pairs across the periodic seam, shell edges, uniform random
+ *                          particles -> g = 1 within the statistical error, independence of the decomposition
  *   contents after a sticky error: parity unpinned (by design)
  */
 #include <math.h>
@@ -599,4 +602,44 @@ void orc_get_particles(const orc_t *o, int64_t *counts, double *x, double *y, do
 void orc_get_last_send_slots(const orc_t *o, int64_t s, int64_t n, int64_t *out)
 {
     memcpy(out, o->send_slot + (size_t)s * (size_t)o->cap, (size_t)n * sizeof(int64_t));
+}
+
+/* ---- statistics hook: the pair count behind the radial distribution function g(r)
+ * ("radial distribution function at contact g(r=R) ... unity indicates a uniform distribution"; the
+ * statistic the heterogeneous run offloads to a GPU).  Plain definition, O(n^2): the number of
+ * unordered pairs {i, j}, i != j, of ALL particles in the box whose periodic (minimum-image) separation r satisfies
+ * r_lo <= r < r_hi.  The paper gives no formula for it; R-26 fixes the arithmetic so that two independent
+ * implementations agree on every pair, also at the edges of the shell:
+ *   per axis  d = a_i - a_j;  if (d > L/2) d = d - L;  else if (d < -L/2) d = d + L;        (L/2 = 0.5 * L, exact)
+ *   r2 = fma(dz, dz, fma(dy, dy, dx * dx));   counted iff  r_lo * r_lo <= r2  and  r2 < r_hi * r_hi.
+ * (d and -d give the same r2 bit for bit, so the count does not depend on which of the two particles comes first.)
+ * g over the shell = count / (n (n-1) / 2 * V_shell / L^3), V_shell = 4/3 pi (r_hi^3 - r_lo^3): left to the caller.
+ * Pins: tests/test_oracle_pairs.py (hand-countable lattice, seam pairs, uniform random -> g = 1 within the
+ * statistical error, shell edges). ---- */
+int64_t orc_pair_count(const orc_t *o, double r_lo, double r_hi)
+{
+    if (!(r_lo >= 0.0) || !(r_hi > r_lo)) return -1;
+    const double half = 0.5 * o->L;
+    const double lo2 = r_lo * r_lo, hi2 = r_hi * r_hi;
+    int64_t n = 0, pairs = 0;
+    for (int64_t s = 0; s < o->P; ++s) n += o->count[s];
+    double *xs = (double *)malloc((size_t)(n > 0 ? n : 1) * 3 * sizeof(double));
+    if (!xs) return -1;
+    int64_t q = 0;
+    for (int64_t s = 0; s < o->P; ++s)
+        for (int64_t i = 0; i < o->count[s]; ++i, ++q)
+            for (int a = 0; a < 3; ++a) xs[3 * q + a] = o->f[a][s * o->cap + i];
+    for (int64_t i = 0; i < n; ++i)
+        for (int64_t j = i + 1; j < n; ++j) {
+            double d[3];
+            for (int a = 0; a < 3; ++a) {
+                d[a] = xs[3 * i + a] - xs[3 * j + a];
+                if (d[a] > half) d[a] = d[a] - o->L;
+                else if (d[a] < -half) d[a] = d[a] + o->L;
+            }
+            const double r2 = fma(d[2], d[2], fma(d[1], d[1], d[0] * d[0]));
+            if (lo2 <= r2 && r2 < hi2) ++pairs;
+        }
+    free(xs);
+    return pairs;
 }

@@ -79,6 +79,8 @@ def lib():
         L.orc_get_particles.restype = None
         L.orc_get_last_send_slots.argtypes = [C.c_void_p, C.c_int64, C.c_int64, _ip]
         L.orc_get_last_send_slots.restype = None
+        L.orc_pair_count.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.orc_pair_count.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -244,6 +246,13 @@ class Oracle:
         lib().orc_get_particles(self._h, _i(out["counts"]), *(_d(out[k]) for k in FIELDS[:7]),
                                 _i(out["id"]), out["code"].ctypes.data_as(_bp))
         return out
+
+    def pair_count(self, r_lo, r_hi):
+        """Unordered pairs of all particles with periodic separation in [r_lo, r_hi) (O(n^2); R-26)."""
+        c = lib().orc_pair_count(self._h, float(r_lo), float(r_hi))
+        if c < 0:
+            raise ValueError("orc_pair_count: need 0 <= r_lo < r_hi")
+        return c
 
     def last_send_slots(self, s, n):
         o = np.empty(n, dtype=np.int64)
