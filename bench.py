@@ -306,6 +306,15 @@ def run_cuda(args):
             evf[k][0].record(); lcs.set_fluid(wl["u"], wl["v"], wl["w"]); evf[k][1].record()
         torch.cuda.synchronize()
         fluid_ms = float(np.median([e[0].elapsed_time(e[1]) for e in evf]))
+        # statistics hook (second half): the pair count behind g(r), on a thin shell
+        r_hi_pc = 2.0 * np.pi / N * 0.25
+        evp = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        pc_dev = lcs.pair_count(0.0, r_hi_pc)                                 # warm-up
+        evp[0].record(); pc_dev = lcs.pair_count(0.0, r_hi_pc); evp[1].record()
+        torch.cuda.synchronize()
+        pair_ms = evp[0].elapsed_time(evp[1])
+        pairs = int(pc_dev.item())
+        g_of_r = pairs / (0.5 * n * (n - 1) * (4.0 / 3.0) * np.pi * r_hi_pc ** 3 / (2.0 * np.pi) ** 3)
         push_ms = float(np.median([e[0].elapsed_time(e[1]) for e in ev]))
         mig_ms = float(np.median([e[1].elapsed_time(e[2]) for e in ev]))
         m_u = n_mig_u / n
@@ -330,6 +339,9 @@ def run_cuda(args):
             "set_fluid": {"call": "lcs_set_fluid", "ms": fluid_ms,
                           "GBps": (24.0 + 32.0) * N ** 3 / (fluid_ms * 1e-3) / 1e9,
                           "note": "reads 24 B and writes 32 B per cell; off the timed step (the fluid is frozen)"},
+            "pair_count": {"call": "lcs_pair_count", "ms": pair_ms, "r_lo": 0.0, "r_hi": r_hi_pc, "pairs": pairs, "g": g_of_r,
+                           "particles_per_s": n / (pair_ms * 1e-3),
+                           "note": "cell list of all particles + 27-cell neighbourhood; g = 1 for a uniform distribution"},
             "fused": {"call": "lcs_step_fused", "ms": ms_total / args.steps,
                       "particles_per_s": n / (ms_total / args.steps * 1e-3)},
         }

@@ -145,6 +145,17 @@ int lcs_get_particles(lcs_t* h, int64_t* d_counts, double* d_x, double* d_y, dou
 int lcs_get_codes(lcs_t* h, uint8_t* d_codes);
 int lcs_get_count_table(lcs_t* h, int64_t* d_table);
 
+/* Statistics hook: the pair count behind the radial distribution function g(r) ("radial distribution
+ * function at contact g(r=R) ... unity indicates a uniform distribution"; the statistic the paper's heterogeneous run
+ * offloads to a GPU; R-26).  Writes to *d_count (device, int64, 8-byte aligned) the number
+ * of unordered pairs of ALL particles in the box whose periodic (minimum-image) separation r satisfies
+ * r_lo <= r < r_hi; g over the shell = count / (n (n-1) / 2 * 4/3 pi (r_hi^3 - r_lo^3) / L^3).  Arithmetic per pair as
+ * DESIGN.md R-26 fixes it, so the count is bit-exact against the O(n^2) definition.  Uses the send pool as scratch
+ * (slot indices sorted by cell + a cell list of up to 256^3 cells): call it between steps, not between
+ * lcs_particle_step and lcs_migrate.  LCS_ERR_INVALID_ARG unless 0 <= r_lo < r_hi <= L/3; LCS_ERR_STATE without
+ * particles or with a pending push. */
+int lcs_pair_count(lcs_t* h, double r_lo, double r_hi, int64_t* d_count);
+
 /* Synchronises the stream and reads the status word.  Any out pointer may be NULL.
  * Returns the sticky error (0 if none). */
 int lcs_get_status(lcs_t* h, int* sticky_error, int64_t* n_total, int64_t* n_migrated_last);

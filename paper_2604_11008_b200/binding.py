@@ -11,7 +11,7 @@ LCS_ERR_CAPACITY, LCS_ERR_JUMP, LCS_ERR_RANGE, LCS_ERR_NOMEM = -4, -5, -6, -7
 EXPORTED_SYMBOLS = (
     "lcs_workspace_bytes", "lcs_create", "lcs_destroy", "lcs_set_fluid", "lcs_set_particles",
     "lcs_particle_step", "lcs_migrate", "lcs_migrate_sweeps", "lcs_step_rk2", "lcs_step_fused", "lcs_get_counts", "lcs_get_particles",
-    "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_staging_bytes", "lcs_step_fused_host",
+    "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_staging_bytes", "lcs_step_fused_host", "lcs_pair_count",
     "lcs_profile_begin", "lcs_profile_end", "lcs_kernel_launches", "lcs_version")
 
 FIELDS = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
@@ -66,6 +66,7 @@ def load_library(build_if_missing: bool = True):
     L.lcs_get_codes.argtypes = [vp, vp]
     L.lcs_get_count_table.argtypes = [vp, vp]
     L.lcs_get_status.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(i64), C.POINTER(i64)]
+    L.lcs_pair_count.argtypes = [vp, dbl, dbl, vp]
     L.lcs_staging_bytes.restype = C.c_size_t
     L.lcs_staging_bytes.argtypes = [i64, C.c_int]
     L.lcs_step_fused_host.argtypes = [vp, dbl, i64, C.POINTER(vp), C.POINTER(vp), vp, vp, C.c_size_t]
@@ -202,6 +203,12 @@ class LCS:
     def get_count_table(self):
         out = self._torch.empty((self.P, 27), dtype=self._torch.int64, device=self.device)
         self._chk("lcs_get_count_table", self._L.lcs_get_count_table(self._h, _ptr(out)))
+        return out
+
+    def pair_count(self, r_lo, r_hi):
+        """-> device int64 tensor (1 element): unordered pairs with periodic separation in [r_lo, r_hi) (R-26)."""
+        out = self._torch.empty(1, dtype=self._torch.int64, device=self.device)
+        self._chk("lcs_pair_count", self._L.lcs_pair_count(self._h, float(r_lo), float(r_hi), _ptr(out)))
         return out
 
     def staging_bytes(self, n):

@@ -458,6 +458,45 @@ int lcs_get_count_table(lcs_t* h, int64_t* d_table)
     return check_launch(h);
 }
 
+int lcs_pair_count(lcs_t* h, double r_lo, double r_hi, int64_t* d_count)
+{
+    if (!h || !d_count || (reinterpret_cast<uintptr_t>(d_count) & 7u)) return LCS_ERR_INVALID_ARG;
+    if (!(r_lo >= 0.0) || !(r_hi > r_lo) || !std::isfinite(r_hi)) return LCS_ERR_INVALID_ARG;
+    const Geom& G = h->G;
+    if (r_hi > G.L / 3.0) return LCS_ERR_INVALID_ARG;          // the cell list needs at least three cells per axis
+    if (!h->have_particles || h->pushed) return LCS_ERR_STATE;
+    if (h->sticky) return h->sticky;
+    // scratch in the send pool (free between steps): slot indices sorted by cell, then the cell arrays
+    const size_t slots = (size_t)G.P * (size_t)G.cap;
+    const size_t idx_bytes = align_up(slots * 4);
+    if (h->pool_bytes < idx_bytes + 1024) return LCS_ERR_INVALID_ARG;
+    const size_t avail = h->pool_bytes - idx_bytes;
+    long long M = std::min<long long>(256, (long long)std::floor(G.L / r_hi));
+    M = std::min<long long>(M, std::max<long long>(3, (long long)std::cbrt((double)slots)));   // about one particle per cell
+    while (M > 3 && (size_t)(8 * M * M * M + 4 + 4 * ((M * M * M + kScanChunk - 1) / kScanChunk) + 256) > avail) --M;
+    if (M < 3) return LCS_ERR_INVALID_ARG;
+    const size_t ncell = (size_t)(M * M * M);
+    const int nchunks = (int)((ncell + kScanChunk - 1) / kScanChunk);
+    char* base = static_cast<char*>(h->pool);
+    uint32_t* idx = reinterpret_cast<uint32_t*>(base);
+    uint32_t* cellstart = reinterpret_cast<uint32_t*>(base + idx_bytes);       // [ncell + 1]
+    uint32_t* cellfill = cellstart + ncell + 1;                                // [ncell]
+    uint32_t* sums = cellfill + ncell;                                         // [nchunks]
+    PairGeom Q;
+    Q.M = (int)M; Q.inv_cell = (double)M / G.L; Q.L = G.L; Q.half_L = 0.5 * G.L; Q.lo2 = r_lo * r_lo; Q.hi2 = r_hi * r_hi;
+    cudaMemsetAsync(cellstart, 0, (2 * ncell + 1) * 4, h->stream);
+    cudaMemsetAsync(d_count, 0, 8, h->stream);
+    const dim3 pgrid((unsigned)((G.cap + 255) / 256), G.P);
+    k_pc_count<<<pgrid, 256, 0, h->stream>>>(G, h->S, h->T, Q, cellstart);
+    k_scan_sums<<<nchunks, 256, 0, h->stream>>>(cellstart, ncell, sums);
+    k_scan_top<<<1, 1024, 0, h->stream>>>(sums, nchunks, cellstart + ncell);
+    k_scan_apply<<<nchunks, 256, 0, h->stream>>>(cellstart, ncell, sums);
+    k_pc_fill<<<pgrid, 256, 0, h->stream>>>(G, h->S, h->T, Q, cellstart, cellfill, idx);
+    k_pc_pairs<<<(unsigned)((slots + 255) / 256), 256, 0, h->stream>>>(h->S, Q, cellstart, idx, cellstart + ncell,
+                                                                        reinterpret_cast<unsigned long long*>(d_count));
+    return check_launch(h, 6);
+}
+
 int lcs_get_status(lcs_t* h, int* sticky_error, int64_t* n_total, int64_t* n_migrated_last)
 {
     if (!h) return LCS_ERR_INVALID_ARG;

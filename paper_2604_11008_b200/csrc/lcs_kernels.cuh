@@ -1508,4 +1508,138 @@ k_set_scatter(Geom G, Slabs S, int64_t n, InPtrs I, const int32_t* __restrict__ 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Statistics hook: the pair count behind g(r) (R-26).
+// A cell list over ALL particles of the box with M^3 cells of side L/M >= r_hi (M >= 3): count per cell, exclusive scan,
+// fill (slot indices sorted by cell; the order inside a cell is arbitrary, the COUNT does not depend on it), then one
+// thread per particle walks the 27 neighbouring cells and counts the partners that come later in the sorted order, so
+// every unordered pair is seen once.  Integer result: bit-exact against the oracle.
+// ---------------------------------------------------------------------------------------------
+struct PairGeom { int M; double inv_cell, half_L, L, lo2, hi2; };
+
+__device__ __forceinline__ int pc_cell1(double a, const PairGeom& Q)
+{
+    const int c = __double2int_rd(a * Q.inv_cell);
+    return max(0, min(c, Q.M - 1));
+}
+
+__global__ void __launch_bounds__(256)
+k_pc_count(Geom G, Slabs S, Tables T, PairGeom Q, uint32_t* __restrict__ cellcnt)
+{
+    const int s = blockIdx.y;
+    const uint32_t i = blockIdx.x * 256u + threadIdx.x;
+    if (i >= T.count[s]) return;
+    const size_t at = (size_t)s * (size_t)G.cap + i;
+    const int c = pc_cell1(S.f[0][at], Q) + Q.M * (pc_cell1(S.f[1][at], Q) + Q.M * pc_cell1(S.f[2][at], Q));
+    atomicAdd(&cellcnt[c], 1u);
+}
+
+// exclusive scan of a u32 array in three launches: chunk sums, scan of the sums (one CTA), apply
+constexpr int kScanChunk = 4096;
+__global__ void __launch_bounds__(256)
+k_scan_sums(const uint32_t* __restrict__ a, size_t n, uint32_t* __restrict__ sums)
+{
+    __shared__ uint32_t sh[8];
+    const size_t base = (size_t)blockIdx.x * kScanChunk;
+    uint32_t v = 0;
+    for (int k = threadIdx.x; k < kScanChunk; k += 256) if (base + k < n) v += a[base + k];
+    v = warp_sum(v);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) { uint32_t t = 0; for (int w = 0; w < 8; ++w) t += sh[w]; sums[blockIdx.x] = t; }
+}
+__global__ void __launch_bounds__(1024)
+k_scan_top(uint32_t* __restrict__ sums, int nchunks, uint32_t* __restrict__ total)
+{   // in place, exclusive; nchunks <= 1024 * 16
+    __shared__ uint32_t sh[1024];
+    const int per = (nchunks + 1023) / 1024;
+    const int c0 = min(nchunks, (int)threadIdx.x * per), c1 = min(nchunks, c0 + per);
+    uint32_t v = 0;
+    for (int c = c0; c < c1; ++c) v += sums[c];
+    sh[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+        const uint32_t add = threadIdx.x >= (unsigned)o ? sh[threadIdx.x - o] : 0u;
+        __syncthreads();
+        sh[threadIdx.x] += add;
+        __syncthreads();
+    }
+    uint32_t run = sh[threadIdx.x] - v;
+    for (int c = c0; c < c1; ++c) { const uint32_t t = sums[c]; sums[c] = run; run += t; }
+    if (threadIdx.x == 1023) *total = sh[1023];
+}
+__global__ void __launch_bounds__(256)
+k_scan_apply(uint32_t* __restrict__ a, size_t n, const uint32_t* __restrict__ sums)
+{   // a <- exclusive prefix of a; every thread owns 16 consecutive elements of the chunk
+    __shared__ uint32_t sh[256];
+    const size_t base = (size_t)blockIdx.x * kScanChunk + (size_t)threadIdx.x * 16;
+    uint32_t v[16], sum = 0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { v[k] = base + k < n ? a[base + k] : 0u; sum += v[k]; }
+    sh[threadIdx.x] = sum;
+    __syncthreads();
+    for (int o = 1; o < 256; o <<= 1) {
+        const uint32_t add = threadIdx.x >= (unsigned)o ? sh[threadIdx.x - o] : 0u;
+        __syncthreads();
+        sh[threadIdx.x] += add;
+        __syncthreads();
+    }
+    uint32_t run = sums[blockIdx.x] + sh[threadIdx.x] - sum;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { if (base + k < n) a[base + k] = run; run += v[k]; }
+}
+
+__global__ void __launch_bounds__(256)
+k_pc_fill(Geom G, Slabs S, Tables T, PairGeom Q, const uint32_t* __restrict__ cellstart, uint32_t* __restrict__ cellfill,
+          uint32_t* __restrict__ idx)
+{
+    const int s = blockIdx.y;
+    const uint32_t i = blockIdx.x * 256u + threadIdx.x;
+    if (i >= T.count[s]) return;
+    const size_t at = (size_t)s * (size_t)G.cap + i;
+    const int c = pc_cell1(S.f[0][at], Q) + Q.M * (pc_cell1(S.f[1][at], Q) + Q.M * pc_cell1(S.f[2][at], Q));
+    idx[cellstart[c] + atomicAdd(&cellfill[c], 1u)] = (uint32_t)at;            // P*cap < 2^31
+}
+
+__device__ __forceinline__ double pc_minimg(double d, const PairGeom& Q)
+{
+    if (d > Q.half_L) d = d - Q.L;
+    else if (d < -Q.half_L) d = d + Q.L;
+    return d;
+}
+
+__global__ void __launch_bounds__(256)
+k_pc_pairs(Slabs S, PairGeom Q, const uint32_t* __restrict__ cellstart, const uint32_t* __restrict__ idx,
+           const uint32_t* __restrict__ n_total, unsigned long long* __restrict__ out)
+{
+    const uint32_t p = blockIdx.x * 256u + threadIdx.x;
+    uint32_t cnt = 0;
+    if (p < *n_total) {
+        const uint32_t at = idx[p];
+        const double x = S.f[0][at], y = S.f[1][at], z = S.f[2][at];
+        const int cx = pc_cell1(x, Q), cy = pc_cell1(y, Q), cz = pc_cell1(z, Q);
+        const int M = Q.M;
+        for (int dz = -1; dz <= 1; ++dz) {
+            const int nz = cz + dz < 0 ? M - 1 : (cz + dz >= M ? 0 : cz + dz);
+            for (int dy = -1; dy <= 1; ++dy) {
+                const int ny = cy + dy < 0 ? M - 1 : (cy + dy >= M ? 0 : cy + dy);
+                for (int dx = -1; dx <= 1; ++dx) {
+                    const int nx = cx + dx < 0 ? M - 1 : (cx + dx >= M ? 0 : cx + dx);
+                    const int c = nx + M * (ny + M * nz);
+                    const uint32_t q1 = cellstart[c + 1];
+                    for (uint32_t q = max(cellstart[c], p + 1u); q < q1; ++q) {      // partners later in the sorted order
+                        const uint32_t bt = idx[q];
+                        const double ddx = pc_minimg(x - S.f[0][bt], Q), ddy = pc_minimg(y - S.f[1][bt], Q),
+                                     ddz = pc_minimg(z - S.f[2][bt], Q);
+                        const double r2 = fma(ddz, ddz, fma(ddy, ddy, ddx * ddx));
+                        cnt += (Q.lo2 <= r2 && r2 < Q.hi2) ? 1u : 0u;
+                    }
+                }
+            }
+        }
+    }
+    cnt = warp_sum(cnt);
+    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(out, (unsigned long long)cnt);
+}
+
 }  // namespace lcs

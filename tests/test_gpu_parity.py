@@ -317,6 +317,63 @@ def test_host_buffer_entry_point_matches_oracle(torch_cuda, oracle_lib):
     dev.close()
 
 
+def test_pair_count_matches_oracle(torch_cuda, oracle_lib):
+    """lcs_pair_count (the statistic behind g(r), R-26) against the oracle's O(n^2) definition:
+    integer, bit-exact.  Uniform and clumped particles, several decompositions, shells that hit the cell-list limits
+    (r_hi = L/3: three cells per axis; tiny shells: 256 cells per axis), before and after migration steps."""
+    from paper_2604_11008_b200 import LCS, LcsError, LCS_ERR_INVALID_ARG
+    rng = np.random.default_rng(21)
+    for P, N, n in (((2, 2, 2), 16, 6000), ((1, 1, 1), 8, 1), ((3, 2, 1), 12, 9001), ((4, 4, 4), 32, 20000)):
+        Ls = np.array([L / P[0], L / P[1], L / P[2]])
+        parts = random_parts(rng, n, 0.4 * Ls)
+        if n > 100:                                        # a clump with many close pairs, and a few pairs across the seams
+            k = n // 4
+            for a in "xyz":
+                parts[a][:k] = (parts[a][:k] - L / 2) * 0.03 + L / 2
+            parts["x"][k:k + 50] = np.where(np.arange(50) % 2 == 0, 1e-3 * rng.random(50), L - 1e-3 * rng.random(50))
+            parts["x"][k:k + 50] = np.minimum(parts["x"][k:k + 50], np.nextafter(L, 0.0))
+            parts["y"][k:k + 50] = 1.0 + 1e-3 * rng.random(50)
+            parts["z"][k:k + 50] = 2.0 + 1e-3 * rng.random(50)
+        z = np.zeros(N ** 3)
+        cap = 2 * (int(2.5 * n / (P[0] * P[1] * P[2])) // 2 + 400)
+        o, dev, rc = make_pair(torch_cuda, oracle_lib, N, P, cap, (z, z, z), parts)
+        assert rc == 0
+        shells = ((0.0, 0.01), (0.01, 0.05), (0.0, 2e-3), (0.3, L / 3), (0.0, L / 3), (0.05, 0.050001))
+        for step in range(2):
+            for r_lo, r_hi in shells:
+                assert int(dev.pair_count(r_lo, r_hi).item()) == o.pair_count(r_lo, r_hi), (P, n, step, r_lo, r_hi)
+            dev.step_fused(0.5)
+            assert o.step(0.5) == 0
+        for bad in ((0.1, 0.1), (-0.1, 0.2), (0.0, L / 3 * 1.01), (0.2, 0.1)):
+            with pytest.raises(LcsError) as ei:
+                dev.pair_count(*bad)
+            assert ei.value.code == LCS_ERR_INVALID_ARG
+        dev.close()
+
+
+def test_pair_count_uniform_gives_g_one_at_scale(torch_cuda):
+    """2^22 uniform random particles: g = count / (n(n-1)/2 V_shell / L^3) = 1 within 4 sigma of the Poisson error
+    (a property that holds at any size; the O(n^2) oracle cannot run here)."""
+    import math
+    from paper_2604_11008_b200 import LCS
+    torch = torch_cuda
+    n = 1 << 22
+    g = torch.Generator(device="cuda").manual_seed(5)
+    X = torch.rand((3, n), dtype=torch.float64, device="cuda", generator=g) * L
+    X = torch.clamp(X, max=float(np.nextafter(L, 0.0)))
+    zero = torch.zeros(n, dtype=torch.float64, device="cuda")
+    dev = LCS(16, 4, 4, 4, 2 * (n // 64))
+    dev.set_fluid(*(torch.zeros(16 ** 3, dtype=torch.float64, device="cuda") for _ in range(3)))
+    dev.set_particles(X[0].contiguous(), X[1].contiguous(), X[2].contiguous(), zero, zero, zero, zero + 1.0,
+                      torch.arange(n, dtype=torch.int64, device="cuda"))
+    assert dev.get_status()[:2] == (0, n)
+    for r_lo, r_hi in ((0.0, 0.02), (0.02, 0.03)):
+        expect = 0.5 * n * (n - 1) * (4.0 / 3.0) * math.pi * (r_hi ** 3 - r_lo ** 3) / L ** 3
+        got = int(dev.pair_count(r_lo, r_hi).item())
+        assert abs(got - expect) <= 4.0 * math.sqrt(expect), (got, expect)
+    dev.close()
+
+
 def test_all_27_codes_hand_placed(torch_cuda, oracle_lib):
     for P in [(3, 3, 3), (2, 2, 2), (1, 2, 3), (1, 1, 1)]:
         N = 24
