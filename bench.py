@@ -28,9 +28,33 @@ sys.path.insert(0, ROOT)
 
 METRIC = "particles/s (fused push + prefix-scan migrate step)"
 F8 = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
-# DRAM bytes of one k_tile_pass<fused> launch from the committed ncu --set full capture (profiles/r1c_tile_pass_full.md):
-# 9.079250 GB read + 4.307880 GB written.  --traffic-bytes overrides it after a new capture.
-NCU_TRAFFIC_BYTES = {"Large": 9.079250e9 + 4.307880e9}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "traffic.json")
+KERNEL_SOURCES = [os.path.join(ROOT, "paper_2604_11008_b200", "csrc", f) for f in ("lcs_kernels.cuh", "lcs_api.cu")]
+
+
+def kernel_source_hash():
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload, kernel):
+    """DRAM bytes per launch of `kernel` on `workload` from the committed ncu --set full capture listed in
+    profiles/traffic.json (dram__bytes_read.sum + dram__bytes_write.sum).  The entry names the capture file and the hash
+    of the kernel sources it was taken on; if the sources have changed since, the figure is stale and is NOT reported.
+    -> (bytes or None, source string or None, stale flag)"""
+    try:
+        with open(TRAFFIC_FILE) as f:
+            tab = json.load(f)
+        e = tab[workload][kernel]
+    except Exception:
+        return None, None, False
+    if e.get("kernel_source_sha256_16") != kernel_source_hash():
+        return None, e.get("capture"), True
+    return float(e["dram_bytes_read"]) + float(e["dram_bytes_write"]), e.get("capture"), False
 
 
 def measured_peak_hbm():
@@ -370,7 +394,17 @@ def run_cuda(args):
         ms_e2e = t0.elapsed_time(t1)
         ms_e2e = max_over_ranks(ms_e2e, dist, dev)
         assert int(h_counts.sum()) == n
+        # the link itself: one pinned array each way, alone (the floor of this path is 8 arrays in + 8 arrays out)
+        one = torch.empty(n, dtype=torch.float64, device=dev)
+        lk = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        lk[0].record(); one.copy_(h_in["x"], non_blocking=True); lk[1].record(); h_out["x"].copy_(one, non_blocking=True); lk[2].record()
+        torch.cuda.synchronize()
+        h2d_gbps = 8.0 * n / (lk[0].elapsed_time(lk[1]) * 1e-3) / 1e9
+        d2h_gbps = 8.0 * n / (lk[1].elapsed_time(lk[2]) * 1e-3) / 1e9
+        del one
         e2e = {"value": world * n * args.e2e_steps / (ms_e2e * 1e-3), "unit": "particles/s",
+               "h2d_GBps_alone": h2d_gbps, "d2h_GBps_alone": d2h_gbps,
+               "link_floor_ms_per_step": (64.0 * n / h2d_gbps + 64.0 * n / d2h_gbps) / 1e6,
                "h2d_bytes_per_step": 64 * n, "d2h_bytes_per_step": 64 * n + 8 * P,
                "steps": args.e2e_steps, "ms_per_step": ms_e2e / args.e2e_steps,
                "call": "lcs_step_fused_host (pinned host particle arrays in/out; fluid field resident)"}
@@ -387,13 +421,14 @@ def run_cuda(args):
     tile_ms = prof["tile_pass_ms"] / max(prof["steps"], 1)
     achieved = alg_bytes / (tile_ms * 1e-3) / 1e9
     step_bytes = n * (128.0 + 128.0 * m) + 24.0 * N ** 3
-    traffic = args.traffic_bytes
-    if traffic is None and args.workload in NCU_TRAFFIC_BYTES:
-        traffic = NCU_TRAFFIC_BYTES[args.workload]
+    traffic, traffic_src, traffic_stale = ncu_traffic(args.workload, "k_tile_pass<fused>")
+    if args.traffic_bytes is not None:
+        traffic, traffic_src, traffic_stale = args.traffic_bytes, "--traffic-bytes", False
     roofline = {"bound": "hbm", "kernel": "k_tile_pass<fused>", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic,
-                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch, profiles/r1c_tile_pass_full.md"
-                if traffic is not None else None,
+                "frac": achieved / peak, "traffic": traffic, "traffic_stale": traffic_stale,
+                "traffic_source": (f"ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch, {traffic_src}"
+                                   if traffic_src else None),
+                "traffic_over_algorithmic": (traffic / alg_bytes) if traffic else None,
                 "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": tile_ms,
                 "kernel_share_of_step": tile_ms / ms_step,
@@ -402,6 +437,25 @@ def run_cuda(args):
                 "step_algorithmic_GBps": step_bytes / (ms_step * 1e-3) / 1e9,
                 "step_frac_of_measured_peak": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
                 "step_frac_of_nominal_8TBps": step_bytes / (ms_step * 1e-3) / 1e9 / 8000.0}
+
+    # ---- what actually bounds the tile pass: the L2 -> SM traffic of the gather ----------------
+    # Every particle brings 64 B in by bulk copy and 8 x 32 B record sectors through L1 (random inside the brick of its
+    # subdomain, which L2 holds); lcs_probe_gather measures, on the same fluid records and alone on the GPU, what the
+    # memory system delivers for that pattern.
+    brick_mb = (N // cfg["P"][0] + 1) * (N // cfg["P"][1] + 1) * (N // cfg["P"][2] + 1) * 32 / 1048576.0
+    try:
+        ceil_l2 = lcs.probe_gather(brick_mb, 200)
+        ceil_dram = lcs.probe_gather(N ** 3 * 32 / 1048576.0, 50)
+    except Exception as exc:                        # pragma: no cover
+        print(f"bench.py: lcs_probe_gather failed: {exc!r}", file=sys.stderr)
+        ceil_l2 = ceil_dram = None
+    l2_bytes = 320.0 * n
+    roofline["l2_to_sm"] = {
+        "bytes_per_launch": l2_bytes, "GBps_in_tile_pass": l2_bytes / (tile_ms * 1e-3) / 1e9,
+        "gather_ceiling_GBps": ceil_l2, "frac_of_gather_ceiling": (l2_bytes / (tile_ms * 1e-3) / 1e9 / ceil_l2) if ceil_l2 else None,
+        "dram_random_sector_GBps": ceil_dram, "brick_MB": brick_mb,
+        "note": "64 B bulk copy + 8 record sectors of 32 B per particle; ceiling = lcs_probe_gather on one brick-sized window, "
+                "same load instruction, 12 warps per SM, nothing else running"}
 
     # ---- the oracle on the host cores, bounded sample ---------------------------------------------
     cpu = None

@@ -181,6 +181,15 @@ int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8
 int lcs_profile_begin(lcs_t* h, int max_steps);
 int lcs_profile_end(lcs_t* h, double* ms_tile_pass, double* ms_table, double* ms_unpack, int* n_steps);
 
+/* Measurement aid for the roofline of the gather (a1): runs, alone on the handle's stream, a kernel in which every
+ * lane issues eight independent 32-byte record loads per iteration (the gather's own load instruction, 12 warps per
+ * SM) at pseudo-random records inside the first window_mb megabytes of the repacked fluid field, `iters` times, and
+ * times it with CUDA events (synchronises).  *h_ms: duration in milliseconds, *h_bytes: sector bytes requested (host
+ * pointers).  With a window that fits L2 (like one subdomain's brick) h_bytes / h_ms is the L2 -> SM ceiling of the
+ * gather's access pattern on this GPU; with the whole field it is the DRAM random-sector rate.  Computes nothing that
+ * the path uses.  LCS_ERR_STATE before lcs_set_fluid. */
+int lcs_probe_gather(lcs_t* h, double window_mb, int iters, double* h_ms, double* h_bytes);
+
 /* Number of kernels this library has launched on the handle since create (for bench accounting). */
 int64_t lcs_kernel_launches(lcs_t* h);
 

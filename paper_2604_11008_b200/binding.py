@@ -11,7 +11,7 @@ LCS_ERR_CAPACITY, LCS_ERR_JUMP, LCS_ERR_RANGE, LCS_ERR_NOMEM = -4, -5, -6, -7
 EXPORTED_SYMBOLS = (
     "lcs_workspace_bytes", "lcs_create", "lcs_destroy", "lcs_set_fluid", "lcs_set_particles",
     "lcs_particle_step", "lcs_migrate", "lcs_migrate_sweeps", "lcs_step_rk2", "lcs_step_fused", "lcs_get_counts", "lcs_get_particles",
-    "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_staging_bytes", "lcs_step_fused_host", "lcs_pair_count",
+    "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_staging_bytes", "lcs_step_fused_host", "lcs_pair_count", "lcs_probe_gather",
     "lcs_profile_begin", "lcs_profile_end", "lcs_kernel_launches", "lcs_version")
 
 FIELDS = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
@@ -67,6 +67,7 @@ def load_library(build_if_missing: bool = True):
     L.lcs_get_count_table.argtypes = [vp, vp]
     L.lcs_get_status.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(i64), C.POINTER(i64)]
     L.lcs_pair_count.argtypes = [vp, dbl, dbl, vp]
+    L.lcs_probe_gather.argtypes = [vp, dbl, C.c_int, C.POINTER(dbl), C.POINTER(dbl)]
     L.lcs_staging_bytes.restype = C.c_size_t
     L.lcs_staging_bytes.argtypes = [i64, C.c_int]
     L.lcs_step_fused_host.argtypes = [vp, dbl, i64, C.POINTER(vp), C.POINTER(vp), vp, vp, C.c_size_t]
@@ -210,6 +211,12 @@ class LCS:
         out = self._torch.empty(1, dtype=self._torch.int64, device=self.device)
         self._chk("lcs_pair_count", self._L.lcs_pair_count(self._h, float(r_lo), float(r_hi), _ptr(out)))
         return out
+
+    def probe_gather(self, window_mb, iters=200):
+        """-> GB/s of 32-byte record loads at random records of the first window_mb MB of the fluid field (measurement aid)."""
+        ms, nb = C.c_double(), C.c_double()
+        self._chk("lcs_probe_gather", self._L.lcs_probe_gather(self._h, float(window_mb), int(iters), C.byref(ms), C.byref(nb)))
+        return nb.value / (ms.value * 1e-3) / 1e9
 
     def staging_bytes(self, n):
         """Bytes of device scratch lcs_step_fused_host needs for n particles (+ 256 so that the block can be aligned)."""

@@ -580,6 +580,32 @@ int lcs_profile_end(lcs_t* h, double* ms_tile_pass, double* ms_table, double* ms
     return rc;
 }
 
+int lcs_probe_gather(lcs_t* h, double window_mb, int iters, double* h_ms, double* h_bytes)
+{
+    if (!h || !h_ms || !h_bytes || !(window_mb > 0.0) || iters < 1) return LCS_ERR_INVALID_ARG;
+    if (!h->have_fluid) return LCS_ERR_STATE;
+    const size_t nrec = (size_t)h->G.N * h->G.N * h->G.N;
+    const uint32_t wrecs = (uint32_t)std::max<size_t>(1, std::min<size_t>(nrec, (size_t)(window_mb * 1048576.0 / 32.0)));
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return LCS_ERR_CUDA;
+    double* sink = reinterpret_cast<double*>(h->T.n_total) + 8;              // spare words of the misc block
+    k_probe_gather<<<sms, 384, 0, h->stream>>>(h->fluid4, wrecs, std::max(1, iters / 8), sink);      // warm-up: fills L2
+    cudaEventRecord(e0, h->stream);
+    k_probe_gather<<<sms, 384, 0, h->stream>>>(h->fluid4, wrecs, iters, sink);
+    cudaEventRecord(e1, h->stream);
+    int rc = cudaEventSynchronize(e1) == cudaSuccess ? LCS_OK : LCS_ERR_CUDA;
+    float ms = 0.f;
+    if (rc == LCS_OK && cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) rc = LCS_ERR_CUDA;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *h_ms = ms;
+    *h_bytes = (double)sms * 384.0 * (double)iters * 8.0 * 32.0;            // one 32-byte sector per load
+    h->launches += 2;
+    return rc;
+}
+
 int64_t lcs_kernel_launches(lcs_t* h) { return h ? h->launches : 0; }
 
 }  // extern "C"

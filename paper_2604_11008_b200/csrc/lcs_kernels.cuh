@@ -1642,4 +1642,29 @@ k_pc_pairs(Slabs S, PairGeom Q, const uint32_t* __restrict__ cellstart, const ui
     if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(out, (unsigned long long)cnt);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Measurement aid (lcs_probe_gather): the L2 -> SM ceiling of the gather's access pattern, measured on the handle's own
+// fluid records.  Every lane issues eight independent 32-byte record loads per iteration (the same instruction the
+// gather uses, the same number in flight per warp, 12 warps per SM) at pseudo-random records of a window of the field
+// that fits L2 (like the brick of one subdomain); nothing else runs.  The rate it reaches is what the memory system
+// delivers for this pattern when no other work competes -- the denominator for the gather part of the tile pass.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(384)
+k_probe_gather(const double* __restrict__ F4, uint32_t window_recs, int iters, double* __restrict__ sink)
+{
+    uint32_t x = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u;
+    double acc = 0.0;
+    for (int it = 0; it < iters; ++it) {
+        Cell c[8];
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            x = x * 1664525u + 1013904223u;
+            c[m] = ld_cell(F4, (x >> 8) % window_recs);
+        }
+#pragma unroll
+        for (int m = 0; m < 8; ++m) acc += c[m].u + c[m].v * c[m].w;
+    }
+    if (acc == 1.2345678e300) *sink = acc;                 // keeps the loads alive
+}
+
 }  // namespace lcs
