@@ -53,6 +53,11 @@ struct Layout {
     int64_t send_cap;
 };
 
+inline size_t brick_records(int N, int Px, int Py, int Pz)
+{
+    return (size_t)(N / Px + 2) * (size_t)(N / Py + 2) * (size_t)(N / Pz + 2);
+}
+
 bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* prm)
 {
     if (!prm) return false;
@@ -61,6 +66,7 @@ bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* pr
     if (N % Px || N % Py || N % Pz) return false;
     const int64_t P = (int64_t)Px * Py * Pz;
     if (P > 8192) return false;                          // grid.y and shared-histogram limits
+    if ((unsigned long long)P * brick_records(N, Px, Py, Pz) >= (1ull << 32)) return false;   // fluid record indices are 32-bit
     if (cap < 2 || (cap & 1)) return false;               // even: slab bases stay 16-byte aligned
     if (cap > 0x7fffffff) return false;
     if ((unsigned long long)P * (unsigned long long)cap >= (1ull << 31)) return false;   // slot indices are 32-bit, and the bulk
@@ -95,7 +101,8 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
     const size_t set_bytes = align_up(slots * 4) + align_up(set_tiles * P * 4);
     L.pool = off; L.pool_bytes = send_bytes > set_bytes ? send_bytes : set_bytes;
     off = align_up(off + L.pool_bytes);
-    L.fluid4 = off;    off = align_up(off + (size_t)N * N * N * 32);
+    // fluid bricks: every subdomain's cells plus a periodic halo of one cell, 32 B per record
+    L.fluid4 = off;    off = align_up(off + P * brick_records(N, Px, Py, Pz) * 32);
     L.count = off;     off = align_up(off + P * 4);
     L.cnt = off;       off = align_up(off + P * 32 * 4);
     L.recv_off = off;  off = align_up(off + P * 32 * 4);
@@ -217,6 +224,8 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     Geom& G = h->G;
     G.N = N; G.Px = Px; G.Py = Py; G.Pz = Pz; G.P = Px * Py * Pz;
     G.nx = N / Px; G.ny = N / Py; G.nz = N / Pz;
+    G.bj = G.nz + 2; G.bi = (G.ny + 2) * (G.nz + 2);
+    G.brick = (uint32_t)brick_records(N, Px, Py, Pz);
     G.tiles_per_sub = L.tiles_per_sub;
     G.chunks_per_sub = L.chunks_per_sub;
     G.lbgroups_per_sub = L.lbgroups_per_sub;
@@ -308,8 +317,9 @@ int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* 
 {
     if (!h || !d_u || !d_v || !d_w) return LCS_ERR_INVALID_ARG;
     if (!aligned16(d_u) || !aligned16(d_v) || !aligned16(d_w)) return LCS_ERR_INVALID_ARG;
-    const int N = h->G.N, tiles = (N + 31) / 32;
-    k_repack_fluid<<<dim3(tiles * tiles, N), 256, 0, h->stream>>>(N, d_u, d_v, d_w, h->fluid4);
+    const Geom& G = h->G;
+    const int tiles = ((G.nx + 2 + 31) / 32) * ((G.nz + 2 + 31) / 32);
+    k_repack_fluid<<<dim3(tiles, G.ny + 2, G.P), 256, 0, h->stream>>>(G, d_u, d_v, d_w, h->fluid4);
     h->have_fluid = true;
     return check_launch(h);
 }
@@ -584,8 +594,8 @@ int lcs_probe_gather(lcs_t* h, double window_mb, int iters, double* h_ms, double
 {
     if (!h || !h_ms || !h_bytes || !(window_mb > 0.0) || iters < 1) return LCS_ERR_INVALID_ARG;
     if (!h->have_fluid) return LCS_ERR_STATE;
-    const size_t nrec = (size_t)h->G.N * h->G.N * h->G.N;
-    const uint32_t wrecs = (uint32_t)std::max<size_t>(1, std::min<size_t>(nrec, (size_t)(window_mb * 1048576.0 / 32.0)));
+    const size_t nrec = (size_t)h->G.P * h->G.brick;
+    const uint32_t wrecs = (uint32_t)std::max<size_t>(2, std::min<size_t>(nrec, (size_t)(window_mb * 1048576.0 / 32.0)));
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
