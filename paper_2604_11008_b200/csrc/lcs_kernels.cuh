@@ -619,7 +619,8 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
     if (lane < kNC && cnt_c) atomicAdd(&T.cnt[s * 32 + lane], cnt_c);      // a4
 }
 
-struct TileRef { int s, t; uint32_t cnt; bool ok; };     // a ticketed tile: subdomain, tile index, count[s]
+struct TileRef { int s, t; uint32_t cnt; uint32_t codes; bool ok; };   // a ticketed tile: subdomain, tile index, count[s];
+                                                                        // unfused pass: this lane's code bytes, one per row
 
 template <bool kFused, bool kBig, int kDrag>
 __global__ void LCS_TP_BOUNDS
@@ -672,7 +673,7 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
     auto take_finish = [&](TileRef& R, unsigned int g) {
         g = __shfl_sync(0xffffffffu, g, 0);
         R.ok = g < n_active;
-        R.s = R.t = 0; R.cnt = 0;
+        R.s = R.t = 0; R.cnt = 0; R.codes = 0u;
         if (R.ok) {
             int s = s_hint;
             bool found = false;
@@ -687,6 +688,14 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             }
             s_hint = s;
             R.s = s; R.t = (int)(g - ts(s)); R.cnt = __ldg(T.count + s);
+            if (!kFused) {
+                // the code bytes of the tile (one per row and lane), requested here, two tiles before they are used
+                const uint32_t first = (uint32_t)R.t * kTile;
+                const uint32_t last = min((uint32_t)kTile, R.cnt - first) - 1u;
+#pragma unroll
+                for (int rr = 0; rr < kRows; ++rr)
+                    R.codes |= (uint32_t)S.code[(uint32_t)s * cap32 + first + min(32u * rr + (uint32_t)lane, last)] << (8 * rr);
+            }
         }
     };
     auto take = [&](TileRef& R) { take_finish(R, take_issue()); };
@@ -713,7 +722,11 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
     issue_load(cur, 0);
     take(nxt);
     if (nxt.ok) issue_load(nxt, 1);
-    nn.ok = false; nn.s = nn.t = 0; nn.cnt = 0;
+    nn.ok = false; nn.s = nn.t = 0; nn.cnt = 0; nn.codes = 0u;
+    // The ticket of the tile after next is requested one whole tile before it is resolved (the atomic's round trip is
+    // longer than a tile of the unfused pass): g_ahead is in flight across the loop's back edge.
+    bool have_g = nxt.ok;
+    unsigned int g_ahead = have_g ? take_issue() : 0u;
     Gath Q;
     if (kFused) {
         wait_buf(0);
@@ -732,7 +745,6 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
         if (!have && !have_pend) break;
         TileInfo ti = pend;
         nn.ok = false;
-        unsigned int g_early = 0u;
         Poll lb;                                           // first look-back poll of the pending tile (early, see the row loop)
         lb.a = lb.b = lb.c = 0ull;
         if (!have && have_pend) poll_issue(lb, G, T, pend.s, pend.t, lane, epoch);      // drain: no row loop ran, poll now
@@ -751,16 +763,12 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
             if (kFused) {
                 B = box_of(s);
             } else {
-                // the code bytes of the whole tile, requested before the wait for the tile's bulk copy (one byte per row and lane)
-#pragma unroll
-                for (int rr = 0; rr < kRows; ++rr)
-                    codes_u |= (uint32_t)S.code[(uint32_t)s * cap32 + first + min(32u * rr + (uint32_t)lane, nvalid - 1u)] << (8 * rr);
+                codes_u = cur.codes;       // requested when the tile's ticket was resolved
                 wait_buf(bc);
             }
             uint32_t n_mig = 0, n_stay = 0;
 #pragma unroll
             for (int rr = 0; rr < kRows; ++rr) ti.stay[rr] = 0u;
-            g_early = 0u;
             bool jump = false;
 #pragma unroll 1
             for (int r = 0; r < kRows; ++r) {
@@ -778,7 +786,6 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     // long-latency requests of the tile end, issued under the arithmetic of the last row: the ticket of the
                     // tile after next, and the first look-back poll of the pending tile
                     if (have_pend) poll_issue(lb, G, T, pend.s, pend.t, lane, epoch);
-                    if (nxt.ok) g_early = take_issue();
                 }
                 if (kFused) {
                     // gather of the next row: of this tile, or row 0 of the next tile (whose bulk copy must have landed)
@@ -833,8 +840,12 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 if (lane == 1) atomicAdd(T.gacc + (size_t)s * G.lbgroups_per_sub + (t >> 5), (1ull << 40) | agg);
             }
             ti.s = s; ti.t = t; ti.n_mig = n_mig;
-            // ticket of the tile after next: taken right after this tile's aggregate is out
-            if (nxt.ok) take_finish(nn, g_early);
+        }
+        // ticket of the tile after next: requested a tile ago, resolved now; the one after that is requested at once
+        if (have_g) {
+            take_finish(nn, g_ahead);
+            have_g = nn.ok;
+            if (have_g) g_ahead = take_issue();
         }
 
         // ================= resolve of the previous tile: look-back, then copy-out =================
