@@ -69,7 +69,9 @@ typedef struct {
 /* Bytes of device workspace lcs_create needs; 0 if the arguments are invalid. */
 size_t lcs_workspace_bytes(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params* prm);
 
-/* Create a handle.  N: fluid grid points per axis (2 <= N <= 1625, divisible by Px, Py and Pz);
+/* Create a handle.  N: fluid grid points per axis (2 <= N <= 1625, divisible by Px, Py and Pz, and
+ * Px*Py*Pz*(N/Px+2)*(N/Py+2)*(N/Pz+2) < 2^32: the fluid is kept as one brick of cells plus a one-cell periodic halo
+ * per subdomain and record indices are 32-bit; N = 1625 needs at least two subdomains along one axis);
  * Px, Py, Pz: 1..1024 each, Px*Py*Pz <= 8192; capacity: particle slots per subdomain slab (it must
  * be even, so that slab bases and tile runs stay 16-byte aligned, and P*capacity < 2^31: slots are
  * 32-bit indices); LCS_ERR_INVALID_ARG otherwise.  d_workspace: device block of at
@@ -79,9 +81,11 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
                void* d_workspace, size_t workspace_bytes, void* cuda_stream, lcs_t** out);
 int lcs_destroy(lcs_t* h);
 
-/* Fluid velocity on the N^3 cell centres.  The three arrays are read once, at call
- * time in stream order, and repacked into the workspace as one 32-byte (u,v,w,0) record per cell
- * (one L2 sector per stencil corner); the caller may reuse them once the call's work has run. */
+/* Fluid velocity on the N^3 cell centres, x fastest: u[i + N*(j + N*k)].  The three arrays are read
+ * once, at call time in stream order, and repacked into the workspace as one 32-byte (u,v,w,0) record per cell (one
+ * L2 sector per stencil corner), one contiguous brick of cells plus a periodic halo of one cell per subdomain -- what a
+ * rank of the paper's decomposition holds; the caller may reuse them once the call's work has run.
+ * LCS_ERR_INVALID_ARG for a null pointer or one that is not 16-byte aligned. */
 int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* d_w);
 
 /* Load n particles given in any order; they are binned stably (input order kept inside each

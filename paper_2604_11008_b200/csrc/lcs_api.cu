@@ -318,8 +318,11 @@ int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* 
     if (!h || !d_u || !d_v || !d_w) return LCS_ERR_INVALID_ARG;
     if (!aligned16(d_u) || !aligned16(d_v) || !aligned16(d_w)) return LCS_ERR_INVALID_ARG;
     const Geom& G = h->G;
-    const int tiles = ((G.nx + 2 + 31) / 32) * ((G.nz + 2 + 31) / 32);
-    k_repack_fluid<<<dim3(tiles, G.ny + 2, G.P), 256, 0, h->stream>>>(G, d_u, d_v, d_w, h->fluid4);
+    // chunks of the local (a, c) plane: as equal as possible, at most kRpA x kRpC
+    const int ea = G.nx + 2, ec = G.nz + 2;
+    const int na = (ea + kRpA - 1) / kRpA, nc = (ec + kRpC - 1) / kRpC;
+    const int ca = (ea + na - 1) / na, cc = (ec + nc - 1) / nc;
+    k_repack_fluid<<<dim3(na * nc, G.ny + 2, G.P), 256, 0, h->stream>>>(G, d_u, d_v, d_w, h->fluid4, ca, cc, na);
     h->have_fluid = true;
     return check_launch(h);
 }
@@ -476,9 +479,10 @@ int lcs_pair_count(lcs_t* h, double r_lo, double r_hi, int64_t* d_count)
     if (r_hi > G.L / 3.0) return LCS_ERR_INVALID_ARG;          // the cell list needs at least three cells per axis
     if (!h->have_particles || h->pushed) return LCS_ERR_STATE;
     if (h->sticky) return h->sticky;
-    // scratch in the send pool (free between steps): slot indices sorted by cell, then the cell arrays
+    // scratch in the send pool (free between steps): the positions sorted by cell (three arrays), then the cell arrays
     const size_t slots = (size_t)G.P * (size_t)G.cap;
-    const size_t idx_bytes = align_up(slots * 4);
+    const size_t arr_bytes = align_up(slots * 8);
+    const size_t idx_bytes = 3 * arr_bytes;
     if (h->pool_bytes < idx_bytes + 1024) return LCS_ERR_INVALID_ARG;
     const size_t avail = h->pool_bytes - idx_bytes;
     long long M = std::min<long long>(256, (long long)std::floor(G.L / r_hi));
@@ -488,7 +492,9 @@ int lcs_pair_count(lcs_t* h, double r_lo, double r_hi, int64_t* d_count)
     const size_t ncell = (size_t)(M * M * M);
     const int nchunks = (int)((ncell + kScanChunk - 1) / kScanChunk);
     char* base = static_cast<char*>(h->pool);
-    uint32_t* idx = reinterpret_cast<uint32_t*>(base);
+    double* sx = reinterpret_cast<double*>(base);
+    double* sy = reinterpret_cast<double*>(base + arr_bytes);
+    double* sz = reinterpret_cast<double*>(base + 2 * arr_bytes);
     uint32_t* cellstart = reinterpret_cast<uint32_t*>(base + idx_bytes);       // [ncell + 1]
     uint32_t* cellfill = cellstart + ncell + 1;                                // [ncell]
     uint32_t* sums = cellfill + ncell;                                         // [nchunks]
@@ -501,8 +507,8 @@ int lcs_pair_count(lcs_t* h, double r_lo, double r_hi, int64_t* d_count)
     k_scan_sums<<<nchunks, 256, 0, h->stream>>>(cellstart, ncell, sums);
     k_scan_top<<<1, 1024, 0, h->stream>>>(sums, nchunks, cellstart + ncell);
     k_scan_apply<<<nchunks, 256, 0, h->stream>>>(cellstart, ncell, sums);
-    k_pc_fill<<<pgrid, 256, 0, h->stream>>>(G, h->S, h->T, Q, cellstart, cellfill, idx);
-    k_pc_pairs<<<(unsigned)((slots + 255) / 256), 256, 0, h->stream>>>(h->S, Q, cellstart, idx, cellstart + ncell,
+    k_pc_fill<<<pgrid, 256, 0, h->stream>>>(G, h->S, h->T, Q, cellstart, cellfill, sx, sy, sz);
+    k_pc_pairs<<<(unsigned)((slots + 255) / 256), 256, 0, h->stream>>>(Q, cellstart, sx, sy, sz, cellstart + ncell,
                                                                         reinterpret_cast<unsigned long long*>(d_count));
     return check_launch(h, 6);
 }

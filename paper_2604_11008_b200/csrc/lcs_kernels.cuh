@@ -317,45 +317,41 @@ __device__ __forceinline__ uint32_t row_rank(int code, bool valid, int lane, uin
 // ---------------------------------------------------------------------------------------------
 // K0: lcs_set_fluid -- repack the three x-fastest arrays u,v,w[i + N*(j + N*k)] into the bricks: one (u,v,w,0)
 // record per cell of every subdomain plus its periodic halo, z fastest (see a1 above).  One CTA per (subdomain, local y
-// index b, 32x32 tile of the local (a, c) plane): 32x32 transposes through shared memory so that both the reads
-// (along i) and the writes (along k) are coalesced.  Halo cells are read from their periodic images.
+// index b, chunk of the local (a, c) plane): the chunk goes through shared memory with the threads flattened over it,
+// a fastest for the reads (runs along i in the input) and c fastest for the writes (runs of records along k in the
+// brick), so neither side wastes lanes on the ragged extents nx+2, nz+2.  Halo cells are read from their periodic images.
 // ---------------------------------------------------------------------------------------------
+constexpr int kRpA = 96, kRpC = 16;            // largest chunk: kRpA indices along a times kRpC along c
+
 __global__ void __launch_bounds__(256)
 k_repack_fluid(Geom G, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
-               double* __restrict__ F4)
+               double* __restrict__ F4, int ca, int cc, int na)
 {
-    __shared__ double t[3][32][33];
+    __shared__ double t[3][kRpC][kRpA + 1];
     const int s = blockIdx.z, b = blockIdx.y;
     const int ea = G.nx + 2, ec = G.nz + 2;                       // extents of the local (a, c) plane
-    const int tiles_a = (ea + 31) / 32;
-    const int ta = blockIdx.x % tiles_a, tc = blockIdx.x / tiles_a;
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;      // 32 x 8
+    const int a0 = (int)(blockIdx.x % na) * ca, c0 = (int)(blockIdx.x / na) * cc;
+    const int wa = min(ca, ea - a0), wc = min(cc, ec - c0);
+    if (wa <= 0 || wc <= 0) return;
     const SubBox B = sub_box(G, s);
     const size_t Ns = (size_t)G.N;
     int j = B.loy + b - 1;
     j = j < 0 ? j + G.N : (j >= G.N ? j - G.N : j);
-#pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const int c = tc * 32 + ty + 8 * r, a = ta * 32 + tx;
-        if (c < ec && a < ea) {
-            int i = B.lox + a - 1, k = B.loz + c - 1;
-            i = i < 0 ? i + G.N : (i >= G.N ? i - G.N : i);
-            k = k < 0 ? k + G.N : (k >= G.N ? k - G.N : k);
-            const size_t src = i + Ns * (j + Ns * k);
-            t[0][ty + 8 * r][tx] = __ldg(u + src);
-            t[1][ty + 8 * r][tx] = __ldg(v + src);
-            t[2][ty + 8 * r][tx] = __ldg(w + src);
-        }
+    for (int idx = threadIdx.x; idx < wa * wc; idx += 256) {
+        const int a = idx % wa, c = idx / wa;
+        int i = B.lox + a0 + a - 1, k = B.loz + c0 + c - 1;
+        i = i < 0 ? i + G.N : (i >= G.N ? i - G.N : i);
+        k = k < 0 ? k + G.N : (k >= G.N ? k - G.N : k);
+        const size_t src = i + Ns * (j + Ns * k);
+        t[0][c][a] = __ldg(u + src);
+        t[1][c][a] = __ldg(v + src);
+        t[2][c][a] = __ldg(w + src);
     }
     __syncthreads();
-#pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const int a = ta * 32 + ty + 8 * r, c = tc * 32 + tx;
-        if (c < ec && a < ea) {
-            const size_t dst = (size_t)B.base + (size_t)c + (size_t)G.bj * b + (size_t)G.bi * a;
-            const double4 rec = make_double4(t[0][tx][ty + 8 * r], t[1][tx][ty + 8 * r], t[2][tx][ty + 8 * r], 0.0);
-            *reinterpret_cast<double4*>(F4 + 4 * dst) = rec;
-        }
+    for (int idx = threadIdx.x; idx < wa * wc; idx += 256) {
+        const int c = idx % wc, a = idx / wc;
+        const size_t dst = (size_t)B.base + (size_t)(c0 + c) + (size_t)G.bj * b + (size_t)G.bi * (a0 + a);
+        *reinterpret_cast<double4*>(F4 + 4 * dst) = make_double4(t[0][c][a], t[1][c][a], t[2][c][a], 0.0);
     }
 }
 
@@ -1220,16 +1216,24 @@ k_rk2_stage(Geom G, Slabs S, Slabs SB, Tables T, const double* __restrict__ F4, 
         if (32u * r >= nvalid) break;
         const bool valid = 32u * r + (uint32_t)lane < nvalid;
         const uint32_t at = (uint32_t)s * (uint32_t)G.cap + first + min(32u * r + (uint32_t)lane, nvalid - 1u);
-        double x[3], v0[3], v[3], k1[3];
+        double x[3], v0[3], v[3], k1[3], x0[3];
+        // every streamed value of the row is requested before the first one is used (one exposed DRAM latency per row)
 #pragma unroll
-        for (int a = 0; a < 3; ++a) { x[a] = S.f[a][at]; v0[a] = S.f[3 + a][at]; v[a] = v0[a]; k1[a] = 0.0; }
-        const double d = S.f[6][at];
-        Gath Q;
-        gather_issue(Q, F4, G, Bx, x[0], x[1], x[2], lane);
+        for (int a = 0; a < 3; ++a) x[a] = __longlong_as_double(ld_stream(S.f[a] + at));
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { v0[a] = __longlong_as_double(ld_stream(S.f[3 + a] + at)); k1[a] = 0.0; x0[a] = 0.0; }
+        const double d = __longlong_as_double(ld_stream(S.f[6] + at));
         if (kStage == 2) {
 #pragma unroll
-            for (int a = 0; a < 3; ++a) { k1[a] = SB.f[3 + a][at]; v[a] = fma(dt, k1[a], v0[a]); }   // V1, recomputed (R-25)
+            for (int a = 0; a < 3; ++a) {
+                k1[a] = __longlong_as_double(ld_stream(SB.f[3 + a] + at));
+                x0[a] = __longlong_as_double(ld_stream(SB.f[a] + at));
+            }
         }
+        Gath Q;
+        gather_issue(Q, F4, G, Bx, x[0], x[1], x[2], lane);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) v[a] = (kStage == 2) ? fma(dt, k1[a], v0[a]) : v0[a];     // V1, recomputed (R-25)
         double tau = (G.K_tau * d) * d;
         const Vec3 Uv = gather_reduce(Q, lane);
         const double U[3] = {Uv.x, Uv.y, Uv.z};
@@ -1246,13 +1250,14 @@ k_rk2_stage(Geom G, Slabs S, Slabs SB, Tables T, const double* __restrict__ F4, 
             }
             if (valid) {
 #pragma unroll
-                for (int a = 0; a < 3; ++a) { SB.f[a][at] = x[a]; SB.f[3 + a][at] = k[a]; }
+                for (int a = 0; a < 3; ++a) {
+                    st_stream(SB.f[a] + at, __double_as_longlong(x[a])); st_stream(SB.f[3 + a] + at, __double_as_longlong(k[a]));
+                }
             }
         } else {
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                const double x0 = SB.f[a][at];
-                pos[a] = wrap_once(fma(hdt, v0[a] + v[a], x0), G);              // X = X0 + dt/2 (V0 + V1)
+                pos[a] = wrap_once(fma(hdt, v0[a] + v[a], x0[a]), G);           // X = X0 + dt/2 (V0 + V1)
                 vn[a] = fma(hdt, k1[a] + k[a], v0[a]);                          // V = V0 + dt/2 (K1 + K2)
             }
         }
@@ -1262,7 +1267,10 @@ k_rk2_stage(Geom G, Slabs S, Slabs SB, Tables T, const double* __restrict__ F4, 
         if (valid) {
             jump |= jmp;
 #pragma unroll
-            for (int a = 0; a < 3; ++a) { S.f[a][at] = pos[a]; if (kStage == 2) S.f[3 + a][at] = vn[a]; }
+            for (int a = 0; a < 3; ++a) {
+                st_stream(S.f[a] + at, __double_as_longlong(pos[a]));
+                if (kStage == 2) st_stream(S.f[3 + a] + at, __double_as_longlong(vn[a]));
+            }
             S.code[at] = (uint8_t)code;
         }
     }
@@ -1540,9 +1548,10 @@ k_set_scatter(Geom G, Slabs S, int64_t n, InPtrs I, const int32_t* __restrict__ 
 // ---------------------------------------------------------------------------------------------
 // Statistics hook: the pair count behind g(r) (R-26).
 // A cell list over ALL particles of the box with M^3 cells of side L/M >= r_hi (M >= 3): count per cell, exclusive scan,
-// fill (slot indices sorted by cell; the order inside a cell is arbitrary, the COUNT does not depend on it), then one
-// thread per particle walks the 27 neighbouring cells and counts the partners that come later in the sorted order, so
-// every unordered pair is seen once.  Integer result: bit-exact against the oracle.
+// fill (the POSITIONS sorted by cell, x fastest in the cell index, so the particles of three x-adjacent cells are one
+// contiguous run; the order inside a cell is arbitrary, the COUNT does not depend on it), then one thread per particle
+// walks the 27 neighbouring cells (nine runs of x-adjacent cells in memory) and counts the partners that come later in
+// the sorted order, so every unordered pair is seen once.  Integer result: bit-exact against the oracle.
 // ---------------------------------------------------------------------------------------------
 struct PairGeom { int M; double inv_cell, half_L, L, lo2, hi2; };
 
@@ -1620,14 +1629,16 @@ k_scan_apply(uint32_t* __restrict__ a, size_t n, const uint32_t* __restrict__ su
 
 __global__ void __launch_bounds__(256)
 k_pc_fill(Geom G, Slabs S, Tables T, PairGeom Q, const uint32_t* __restrict__ cellstart, uint32_t* __restrict__ cellfill,
-          uint32_t* __restrict__ idx)
+          double* __restrict__ sx, double* __restrict__ sy, double* __restrict__ sz)
 {
     const int s = blockIdx.y;
     const uint32_t i = blockIdx.x * 256u + threadIdx.x;
     if (i >= T.count[s]) return;
     const size_t at = (size_t)s * (size_t)G.cap + i;
-    const int c = pc_cell1(S.f[0][at], Q) + Q.M * (pc_cell1(S.f[1][at], Q) + Q.M * pc_cell1(S.f[2][at], Q));
-    idx[cellstart[c] + atomicAdd(&cellfill[c], 1u)] = (uint32_t)at;            // P*cap < 2^31
+    const double x = S.f[0][at], y = S.f[1][at], z = S.f[2][at];
+    const int c = pc_cell1(x, Q) + Q.M * (pc_cell1(y, Q) + Q.M * pc_cell1(z, Q));
+    const uint32_t q = cellstart[c] + atomicAdd(&cellfill[c], 1u);
+    sx[q] = x; sy[q] = y; sz[q] = z;
 }
 
 __device__ __forceinline__ double pc_minimg(double d, const PairGeom& Q)
@@ -1638,28 +1649,26 @@ __device__ __forceinline__ double pc_minimg(double d, const PairGeom& Q)
 }
 
 __global__ void __launch_bounds__(256)
-k_pc_pairs(Slabs S, PairGeom Q, const uint32_t* __restrict__ cellstart, const uint32_t* __restrict__ idx,
-           const uint32_t* __restrict__ n_total, unsigned long long* __restrict__ out)
+k_pc_pairs(PairGeom Q, const uint32_t* __restrict__ cellstart, const double* __restrict__ sx, const double* __restrict__ sy,
+           const double* __restrict__ sz, const uint32_t* __restrict__ n_total, unsigned long long* __restrict__ out)
 {
     const uint32_t p = blockIdx.x * 256u + threadIdx.x;
     uint32_t cnt = 0;
     if (p < *n_total) {
-        const uint32_t at = idx[p];
-        const double x = S.f[0][at], y = S.f[1][at], z = S.f[2][at];
+        const double x = sx[p], y = sy[p], z = sz[p];
         const int cx = pc_cell1(x, Q), cy = pc_cell1(y, Q), cz = pc_cell1(z, Q);
         const int M = Q.M;
         for (int dz = -1; dz <= 1; ++dz) {
             const int nz = cz + dz < 0 ? M - 1 : (cz + dz >= M ? 0 : cz + dz);
             for (int dy = -1; dy <= 1; ++dy) {
                 const int ny = cy + dy < 0 ? M - 1 : (cy + dy >= M ? 0 : cy + dy);
+                const int row = M * (ny + M * nz);
                 for (int dx = -1; dx <= 1; ++dx) {
                     const int nx = cx + dx < 0 ? M - 1 : (cx + dx >= M ? 0 : cx + dx);
-                    const int c = nx + M * (ny + M * nz);
+                    const int c = nx + row;
                     const uint32_t q1 = cellstart[c + 1];
                     for (uint32_t q = max(cellstart[c], p + 1u); q < q1; ++q) {      // partners later in the sorted order
-                        const uint32_t bt = idx[q];
-                        const double ddx = pc_minimg(x - S.f[0][bt], Q), ddy = pc_minimg(y - S.f[1][bt], Q),
-                                     ddz = pc_minimg(z - S.f[2][bt], Q);
+                        const double ddx = pc_minimg(x - sx[q], Q), ddy = pc_minimg(y - sy[q], Q), ddz = pc_minimg(z - sz[q], Q);
                         const double r2 = fma(ddz, ddz, fma(ddy, ddy, ddx * ddx));
                         cnt += (Q.lo2 <= r2 && r2 < Q.hi2) ? 1u : 0u;
                     }
