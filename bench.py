@@ -345,15 +345,24 @@ def run_cuda(args):
         peak_p, _ = measured_peak_hbm()
         push_bytes = 105.0 * n + 24.0 * N ** 3            # R 56 + W 48 + 1 code byte per particle + the grid once
         mig_bytes = n * (129.0 + 128.0 * m_u)             # code byte + stayers R/W 64 + migrants' second hop
+        # DRAM bytes per launch from the committed ncu captures (profiles/traffic.json, hash-checked like roofline.traffic)
+        tr_push, src_push, stale_push = ncu_traffic(args.workload, "k_push")
+        tr_tp, src_tp, stale_tp = ncu_traffic(args.workload, "k_tile_pass<unfused>")
+        tr_un, _, _ = ncu_traffic(args.workload, "k_unpack")
+        tr_mig = (tr_tp + tr_un) if (tr_tp and tr_un) else None
         phases = {
             "steps": args.phase_steps, "timing": "median of per-call CUDA-event times",
             "push": {"call": "lcs_particle_step", "ms": push_ms, "particles_per_s": n / (push_ms * 1e-3),
                      "algorithmic_GBps": push_bytes / (push_ms * 1e-3) / 1e9,
-                     "frac_of_measured_peak": push_bytes / (push_ms * 1e-3) / 1e9 / peak_p},
+                     "frac_of_measured_peak": push_bytes / (push_ms * 1e-3) / 1e9 / peak_p,
+                     "traffic": tr_push, "traffic_stale": stale_push, "traffic_source": src_push,
+                     "traffic_over_algorithmic": (tr_push / push_bytes) if tr_push else None},
             "migrate": {"call": "lcs_migrate", "ms": mig_ms, "particles_per_s": n / (mig_ms * 1e-3),
                         "algorithmic_GBps": mig_bytes / (mig_ms * 1e-3) / 1e9,
                         "frac_of_measured_peak": mig_bytes / (mig_ms * 1e-3) / 1e9 / peak_p,
-                        "migrant_fraction": m_u},
+                        "migrant_fraction": m_u,
+                        "traffic": tr_mig, "traffic_stale": stale_tp, "traffic_source": src_tp,
+                        "traffic_over_algorithmic": (tr_mig / mig_bytes) if tr_mig else None},
             "migrate_sweeps": {"call": "lcs_migrate_sweeps", "ms": sweeps_ms, "particles_per_s": n / (sweeps_ms * 1e-3),
                                "note": "x, y, z sweeps: three classify + unfused tile pass + scan + table + unpack rounds"},
             "rk2": None if rk2_ms is None else {
