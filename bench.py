@@ -368,7 +368,7 @@ def run_cuda(args):
             "rk2": None if rk2_ms is None else {
                 "call": "lcs_step_rk2", "ms": rk2_ms, "particles_per_s": n / (rk2_ms * 1e-3), "dt": dt_rk2,
                 "migrant_fraction_second_migration": n_mig_r / n,
-                "note": "two stages; 16 arrays migrate after stage 1 (two rounds of the 8-array tile pass), 8 after stage 2"},
+                "note": "both stages run inside the tile pass; after stage 1 the slabs (8 arrays) and group B (X0, K1: 6 arrays) migrate in two rounds with the same codes, after stage 2 the slabs"},
             "set_fluid": {"call": "lcs_set_fluid", "ms": fluid_ms,
                           "GBps": (24.0 + 32.0) * N ** 3 / (fluid_ms * 1e-3) / 1e9,
                           "note": "reads 24 B and writes 32 B per cell; off the timed step (the fluid is frozen)"},

@@ -120,7 +120,7 @@ Layout make_layout(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params*
 
 // Tensor map of one group of 8 arrays for the bulk tile loads: 2-D [8 fields][slots] of 8-byte words, rows `stride` bytes
 // apart, box 8 x kTile.  The encoder is fetched from the driver through the runtime (no link against libcuda).
-bool make_slab_map(CUtensorMap* out, void* base, size_t slots, size_t stride)
+bool make_slab_map(CUtensorMap* out, void* base, size_t slots, size_t stride, int rows = 8)
 {
     typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -130,7 +130,7 @@ bool make_slab_map(CUtensorMap* out, void* base, size_t slots, size_t stride)
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
     const cuuint64_t gdim[2] = {(cuuint64_t)slots, 8};
     const cuuint64_t gstride[1] = {(cuuint64_t)stride};
-    const cuuint32_t box[2] = {(cuuint32_t)kTile, 8};
+    const cuuint32_t box[2] = {(cuuint32_t)kTile, (cuuint32_t)rows};
     const cuuint32_t estr[2] = {1, 1};
     return reinterpret_cast<encode_fn>(fn)(out, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, base, gdim, gstride, box, estr,
                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -153,8 +153,8 @@ inline int check_launch(lcs_t* h, int n = 1)
 // One round of the migration machinery on one group of 8 arrays (the slabs, or an RK2 group that travels with the same
 // codes): tile pass, per-code scan, table, unpack; `commit` also installs the new counts and the next tile index.  The
 // rounds of one migration see the same codes and the same counts, so they apply the same permutation.
-int enqueue_tile_pass(lcs_t* h, bool fused, double dt, const Slabs* grp = nullptr, const CUtensorMap* map = nullptr,
-                      bool commit = true)
+int enqueue_tile_pass(lcs_t* h, int mode, double dt, const Slabs* grp = nullptr, const CUtensorMap* map = nullptr,
+                      bool commit = true, int nf = 8)
 {
     const Geom& G = h->G;
     const Slabs& S = grp ? *grp : h->S;
@@ -170,15 +170,20 @@ int enqueue_tile_pass(lcs_t* h, bool fused, double dt, const Slabs* grp = nullpt
     const size_t smem = tile_pass_smem(G.P);
     cudaMemsetAsync(h->T.gacc, 0, h->gacc_bytes, h->stream);
     const bool big = G.P > kTableSmemMax;
+    const bool fused = mode != 0;
     const bool sn = fused && G.drag_model == 1;            // the unfused pass carries no push: one instantiation
 #define LCS_LAUNCH_TP(F, B, D, GRID) \
-    k_tile_pass<F, B, D><<<GRID, kBlock, smem, h->stream>>>(G, S, h->Snd, h->T, h->fluid4, dt, h->epoch, M)
-    if (fused) {
-        if (big) { if (sn) LCS_LAUNCH_TP(true, true, 1, h->grid_fused); else LCS_LAUNCH_TP(true, true, 0, h->grid_fused); }
-        else     { if (sn) LCS_LAUNCH_TP(true, false, 1, h->grid_fused); else LCS_LAUNCH_TP(true, false, 0, h->grid_fused); }
-    } else {
-        if (big) LCS_LAUNCH_TP(false, true, 0, h->grid_pack); else LCS_LAUNCH_TP(false, false, 0, h->grid_pack);
+    k_tile_pass<F, B, D><<<GRID, kBlock, smem, h->stream>>>(G, S, h->Snd, h->T, h->fluid4, dt, h->epoch, M, h->SB, nf)
+#define LCS_LAUNCH_MODE(F) \
+    do { if (big) { if (sn) LCS_LAUNCH_TP(F, true, 1, h->grid_fused); else LCS_LAUNCH_TP(F, true, 0, h->grid_fused); } \
+         else     { if (sn) LCS_LAUNCH_TP(F, false, 1, h->grid_fused); else LCS_LAUNCH_TP(F, false, 0, h->grid_fused); } } while (0)
+    if (mode == 1) LCS_LAUNCH_MODE(1);
+    else if (mode == 2) LCS_LAUNCH_MODE(2);
+    else if (mode == 3) LCS_LAUNCH_MODE(3);
+    else {
+        if (big) LCS_LAUNCH_TP(0, true, 0, h->grid_pack); else LCS_LAUNCH_TP(0, false, 0, h->grid_pack);
     }
+#undef LCS_LAUNCH_MODE
 #undef LCS_LAUNCH_TP
     if (rec) cudaEventRecord(ev[1], h->stream);
     k_send_scan<<<G.P, 256, 0, h->stream>>>(G, h->Snd, h->T);
@@ -272,7 +277,7 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
         for (int a = 0; a < 7; ++a) h->SB.f[a] = reinterpret_cast<double*>(w + L.rk2_b + a * st);
         h->SB.id = reinterpret_cast<int64_t*>(w + L.rk2_b + 7 * st);
         h->SB.code = h->S.code;
-        if (!make_slab_map(&h->mapB, w + L.rk2_b, (size_t)P * (size_t)capacity, st)) { delete h; return LCS_ERR_CUDA; }
+        if (!make_slab_map(&h->mapB, w + L.rk2_b, (size_t)P * (size_t)capacity, st, 6)) { delete h; return LCS_ERR_CUDA; }
         if (cudaMemsetAsync(w + L.rk2_b, 0, 8 * st, h->stream) != cudaSuccess) { delete h; return LCS_ERR_CUDA; }
     }
     {   // persistent grids: one wave of resident CTAs
@@ -287,11 +292,15 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
             occ = occ == 0 ? o : std::min(occ, o);
         };
         if (G.P > kTableSmemMax) {
-            setup(k_tile_pass<true, true, 0>, occ_f); setup(k_tile_pass<true, true, 1>, occ_f);
-            setup(k_tile_pass<false, true, 0>, occ_p);
+            setup(k_tile_pass<1, true, 0>, occ_f); setup(k_tile_pass<1, true, 1>, occ_f);
+            setup(k_tile_pass<2, true, 0>, occ_f); setup(k_tile_pass<2, true, 1>, occ_f);
+            setup(k_tile_pass<3, true, 0>, occ_f); setup(k_tile_pass<3, true, 1>, occ_f);
+            setup(k_tile_pass<0, true, 0>, occ_p);
         } else {
-            setup(k_tile_pass<true, false, 0>, occ_f); setup(k_tile_pass<true, false, 1>, occ_f);
-            setup(k_tile_pass<false, false, 0>, occ_p);
+            setup(k_tile_pass<1, false, 0>, occ_f); setup(k_tile_pass<1, false, 1>, occ_f);
+            setup(k_tile_pass<2, false, 0>, occ_f); setup(k_tile_pass<2, false, 1>, occ_f);
+            setup(k_tile_pass<3, false, 0>, occ_f); setup(k_tile_pass<3, false, 1>, occ_f);
+            setup(k_tile_pass<0, false, 0>, occ_p);
         }
         if (sms < 1) sms = 148;
         const long long max_tiles = ((long long)G.P * G.tiles_per_sub + kWarps - 1) / kWarps;
@@ -380,7 +389,7 @@ int lcs_migrate(lcs_t* h)
     if (!h) return LCS_ERR_INVALID_ARG;
     if (!h->pushed) return LCS_ERR_STATE;
     if (h->sticky) return h->sticky;
-    return enqueue_tile_pass(h, false, 0.0);
+    return enqueue_tile_pass(h, 0, 0.0);
 }
 
 int lcs_migrate_sweeps(lcs_t* h)
@@ -392,7 +401,7 @@ int lcs_migrate_sweeps(lcs_t* h)
     for (int axis = 0; axis < 3; ++axis) {
         k_classify_axis<<<dim3((unsigned)((G.cap + 255) / 256), G.P), 256, 0, h->stream>>>(G, h->S, h->T, axis);
         int rc = check_launch(h);
-        if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0);
+        if (rc == LCS_OK) rc = enqueue_tile_pass(h, 0, 0.0);
         if (rc != LCS_OK) return rc;
     }
     return LCS_OK;
@@ -403,20 +412,14 @@ int lcs_step_rk2(lcs_t* h, double dt)
     if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
     if (!h->rk2 || !h->have_fluid || !h->have_particles || h->pushed) return LCS_ERR_STATE;
     if (h->sticky) return h->sticky;
-    const Geom& G = h->G;
-    const dim3 grid((G.tiles_per_sub + kPushWarps - 1) / kPushWarps, G.P);
-    // stage 1, then everything that is live between the stages migrates: two rounds of 8 arrays with the same codes
-    // (slabs: X1, V0, d, id; group B: X0, K1), the counts committed by the second one
-    k_rk2_stage<1><<<grid, 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->SB, h->T, h->fluid4, dt);
-    int rc = check_launch(h);
-    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0, &h->S, &h->slab_map, false);
-    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0, &h->SB, &h->mapB, true);
+    // Stage 1 runs inside the tile pass of the slabs (X1, V0, d, id migrate; X0, K1 and the code byte are written at the
+    // particle's slot), then group B (X0, K1) travels in an unfused round with the same codes, which commits the counts.
+    int rc = enqueue_tile_pass(h, 2, dt, &h->S, &h->slab_map, false);
+    if (rc == LCS_OK) rc = enqueue_tile_pass(h, 0, 0.0, &h->SB, &h->mapB, true, 6);     // X0, K1: six live arrays
     if (rc != LCS_OK) return rc;
-    // stage 2 consumes X0, K1; only X, V, d, id are live afterwards: one round
-    k_rk2_stage<2><<<grid, 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->SB, h->T, h->fluid4, dt);
-    rc = check_launch(h);
-    if (rc == LCS_OK) rc = enqueue_tile_pass(h, false, 0.0);
-    return rc;
+    // Stage 2 runs inside the tile pass too: it reads X0, K1 of group B at the particle's slot; only X, V, d, id are live
+    // afterwards, so this one round ends the step.
+    return enqueue_tile_pass(h, 3, dt);
 }
 
 int lcs_step_fused(lcs_t* h, double dt)
@@ -424,7 +427,7 @@ int lcs_step_fused(lcs_t* h, double dt)
     if (!h || !(dt > 0.0) || !std::isfinite(dt)) return LCS_ERR_INVALID_ARG;
     if (!h->have_fluid || !h->have_particles || h->pushed) return LCS_ERR_STATE;   // a pending push must be migrated first
     if (h->sticky) return h->sticky;
-    return enqueue_tile_pass(h, true, dt);
+    return enqueue_tile_pass(h, 1, dt);
 }
 
 int lcs_get_counts(lcs_t* h, int64_t* d_counts)

@@ -515,6 +515,28 @@ __device__ __forceinline__ int advance_particle(Particle& p, const Vec3& U, cons
     return code;
 }
 
+// Helpers of the minimum-image classification (R-24) and of the RK2 stages (R-25).
+__device__ __forceinline__ int min_image_dir(double a, const Geom& G, int Pa, int n_a, int p_a, bool& jump)
+{
+    if (!(a >= 0.0 && a < G.L)) { jump = true; return 0; }
+    int ic = __double2int_rd(a * G.inv_dx);
+    ic = max(0, min(ic, G.N - 1));
+    int dd = ic / n_a - p_a;
+    if (Pa >= 3) {
+        if (dd > 1) dd -= Pa;
+        else if (dd < -1) dd += Pa;
+    }
+    if (dd < -1 || dd > 1) { jump = true; dd = dd < -1 ? -1 : 1; }
+    return dd;
+}
+
+__device__ __forceinline__ double wrap_once(double xu, const Geom& G)
+{
+    if (xu < 0.0) { xu = xu + G.L; if (xu >= G.L) xu = G.L_below; }
+    else if (xu >= G.L) xu = xu - G.L;
+    return xu;                                     // still outside [0, L): min_image_dir raises the jump
+}
+
 // What a pushed tile carries from its push to its resolve one iteration later.
 struct TileInfo {
     int s, t;
@@ -618,11 +640,25 @@ k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
 struct TileRef { int s, t; uint32_t cnt; uint32_t codes; bool ok; };   // a ticketed tile: subdomain, tile index, count[s];
                                                                         // unfused pass: this lane's code bytes, one per row
 
-template <bool kFused, bool kBig, int kDrag>
+// kMode: 0 = migration only (codes from S.code); 1 = single-stage push fused in front (a1-a4, DESIGN R-1);
+//        2 / 3 = stage 1 / stage 2 of the paper's two-stage RK2 (Heun) fused in front, one migration per stage
+//        (R-25):
+//          stage 1: K1 = (U(X0) - V0)/tau + g ; X1 = X0 + dt V0 ; X1 replaces X0 in the tile, X0, K1 and the code byte
+//                   are written at the particle's slot (group SB then travels in a second, unfused round with the same
+//                   codes), V0 stays in the slabs
+//          stage 2: V1 = V0 + dt K1 (recomputed: the same fma the oracle stored) ; K2 = (U(X1) - V1)/tau + g ;
+//                   X = X0 + dt/2 (V0 + V1) ; V = V0 + dt/2 (K1 + K2) ; X0, K1 are read from group SB at the particle's
+//                   slot, requested together with the row's gather
+//        tau = tau_p / f, f at the start of the stage.  Destination: per axis the minimum-image direction from the slab
+//        the particle sits in to the owner of its new position (R-24's rule).  Of the paper's 17 arrays 14 travel between
+//        the stages (X1, V0, d, id in the slabs; X0, K1 in group SB, whose two spare arrays travel too): V1 never exists
+//        in memory.
+template <int kMode, bool kBig, int kDrag>
 __global__ void LCS_TP_BOUNDS
 k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4, double dt, uint32_t epoch,
-            const __grid_constant__ CUtensorMap slab_map)
-{
+            const __grid_constant__ CUtensorMap slab_map, Slabs SB, int nf)
+{   // nf: arrays of the group that are live (8, or 6 for the RK2 group SB: the box of its tensor map has nf rows)
+    constexpr bool kFused = kMode != 0;
     extern __shared__ __align__(128) unsigned char s_raw[];
     TileBuf* bufs = reinterpret_cast<TileBuf*>(s_raw);                                      // [kWarps][kNBuf]
     uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_raw + kWarps * kNBuf * sizeof(TileBuf)); // [kWarps][kNBuf]
@@ -703,7 +739,7 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
         __syncwarp();
         if (lane == 0) {
             const uint32_t bar = bar0 + 8u * b;
-            mbar_expect_tx(bar, 8u * kTile * 8u);
+            mbar_expect_tx(bar, (uint32_t)nf * kTile * 8u);
             bulk_tensor2d_g2s(smem_u32(&my[b].f[0][0]), &slab_map, (uint32_t)R.s * cap32 + (uint32_t)R.t * kTile, 0u, bar);
         }
     };
@@ -724,11 +760,22 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
     bool have_g = nxt.ok;
     unsigned int g_ahead = have_g ? take_issue() : 0u;
     Gath Q;
+    double ex0[3] = {0.0, 0.0, 0.0}, ek1[3] = {0.0, 0.0, 0.0};   // RK2 stage 2: X0 and K1 of the NEXT row (requested with its gather)
+    const uint32_t last_slot = (uint32_t)G.P * cap32 - 1u;
+    auto extra_issue = [&](uint32_t slot) {
+        slot = min(slot, last_slot);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            ex0[a] = __longlong_as_double(ld_stream(SB.f[a] + slot));
+            ek1[a] = __longlong_as_double(ld_stream(SB.f[3 + a] + slot));
+        }
+    };
     if (kFused) {
         wait_buf(0);
         const unsigned long long* px = &my[0].f[0][0];
         gather_issue(Q, F4, G, box_of(cur.s), __longlong_as_double(px[lane]), __longlong_as_double(px[kTile + lane]),
                      __longlong_as_double(px[2 * kTile + lane]), lane);
+        if (kMode == 3) extra_issue((uint32_t)cur.s * cap32 + (uint32_t)cur.t * kTile + (uint32_t)lane);
     }
     TileInfo pend;
     pend.s = pend.t = 0; pend.n_mig = 0;
@@ -774,8 +821,11 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                 U.x = U.y = U.z = 0.0;
                 Drag D;
                 D.tau = D.alpha = D.b = 0.0;
+                double x0c[3], k1c[3];                                  // RK2 stage 2: this row's X0, K1 (landed with its gather)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) { x0c[a] = ex0[a]; k1c[a] = ek1[a]; }
                 if (kFused) {
-                    if (kDrag == 0) D = drag_coeffs(__longlong_as_double(W.f[6][p]), dt, G);   // serial chain, issued under the lerps
+                    if (kMode == 1 && kDrag == 0) D = drag_coeffs(__longlong_as_double(W.f[6][p]), dt, G);   // serial chain, issued under the lerps
                     U = gather_reduce(Q, lane);
                 }
                 if (r + 1 == nrows) {
@@ -793,10 +843,52 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     else if (nxt.ok) { wait_buf(bn); px = &my[bn].f[0][0]; Bg = box_of(nxt.s); }
                     gather_issue(Q, F4, G, Bg, __longlong_as_double(px[lane]),
                                  __longlong_as_double(px[kTile + lane]), __longlong_as_double(px[2 * kTile + lane]), lane);
+                    if (kMode == 3)
+                        extra_issue(r + 1 < nrows ? (uint32_t)s * cap32 + first + 32u * (uint32_t)(r + 1) + (uint32_t)lane
+                                                  : (uint32_t)nxt.s * cap32 + (uint32_t)nxt.t * kTile + (uint32_t)lane);
                 }
                 const bool valid = p < nvalid;
                 int code;
-                if (kFused) {
+                if (kMode == 2 || kMode == 3) {
+                    // one stage of the paper's RK2, operation for operation as the oracle does it (R-25)
+                    double x[3], v0[3], v[3], k[3], pos[3], vn[3];
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) {
+                        x[a] = __longlong_as_double(W.f[a][p]); v0[a] = __longlong_as_double(W.f[3 + a][p]);
+                        v[a] = (kMode == 3) ? fma(dt, k1c[a], v0[a]) : v0[a];              // V1, recomputed in stage 2
+                    }
+                    const double dd = __longlong_as_double(W.f[6][p]);
+                    double tau = (G.K_tau * dd) * dd;
+                    const double Ua[3] = {U.x, U.y, U.z};
+                    if (kDrag == 1) tau = tau / drag_factor(dd, v[0] - Ua[0], v[1] - Ua[1], v[2] - Ua[2], G.inv_nu);
+                    const double g[3] = {G.gx, G.gy, G.gz};
+                    const double hdt = 0.5 * dt;
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) {
+                        k[a] = (Ua[a] - v[a]) / tau + g[a];                                // Eq. 6 + g (R-4)
+                        if (kMode == 2) { pos[a] = wrap_once(fma(dt, v0[a], x[a]), G); vn[a] = v0[a]; }
+                        else { pos[a] = wrap_once(fma(hdt, v0[a] + v[a], x0c[a]), G); vn[a] = fma(hdt, k1c[a] + k[a], v0[a]); }
+                    }
+                    const uint32_t c3 = xyz(s);
+                    bool jmp = false;
+                    code = kStay + min_image_dir(pos[0], G, G.Px, G.nx, (int)(c3 & 1023u), jmp)
+                         + 3 * min_image_dir(pos[1], G, G.Py, G.ny, (int)((c3 >> 10) & 1023u), jmp)
+                         + 9 * min_image_dir(pos[2], G, G.Pz, G.nz, (int)(c3 >> 20), jmp);
+                    jump |= jmp && valid;
+                    const uint32_t slot = (uint32_t)s * cap32 + first + p;
+                    if (kMode == 2 && valid) {                                             // kept for stage 2, at the particle's slot
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) {
+                            st_stream(SB.f[a] + slot, __double_as_longlong(x[a])); st_stream(SB.f[3 + a] + slot, __double_as_longlong(k[a]));
+                        }
+                        S.code[slot] = (uint8_t)code;                                      // the second round (group SB) reads it
+                    }
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) {
+                        W.f[a][p] = __double_as_longlong(pos[a]);
+                        if (kMode == 3) W.f[3 + a][p] = __double_as_longlong(vn[a]);
+                    }
+                } else if (kFused) {
                     Particle q;
                     q.x = __longlong_as_double(W.f[0][p]); q.y = __longlong_as_double(W.f[1][p]);
                     q.z = __longlong_as_double(W.f[2][p]); q.vx = __longlong_as_double(W.f[3][p]);
@@ -881,8 +973,8 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                     const uint32_t dst = base + __popc(m & lt);
                     const uint32_t src = 32u * (uint32_t)rr + (uint32_t)lane;
 #pragma unroll
-                    for (int a = 0; a < 7; ++a) st_stream(S.f[a] + dst, W.f[a][src]);
-                    st_stream(S.id + dst, W.f[7][src]);
+                    for (int a = 0; a < 7; ++a) if (a < nf) st_stream(S.f[a] + dst, W.f[a][src]);
+                    if (nf == 8) st_stream(S.id + dst, W.f[7][src]);
                 }
                 base += __popc(m);
             }
@@ -898,8 +990,8 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
                         const uint32_t dst = sendbase + a;
                         const uint32_t src = e & 0xffu;
 #pragma unroll
-                        for (int q = 0; q < 7; ++q) st_stream(Snd.f[q] + dst, W.f[q][src]);
-                        st_stream(Snd.id + dst, W.f[7][src]);
+                        for (int q = 0; q < 7; ++q) if (q < nf) st_stream(Snd.f[q] + dst, W.f[q][src]);
+                        if (nf == 8) st_stream(Snd.id + dst, W.f[7][src]);
                         Snd.code[dst] = (uint8_t)(e >> 8);
                     }
                 }
@@ -1164,117 +1256,6 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
                 S.id[dst[u]] = (int64_t)v[u][7];
             }
     }
-}
-
-// ---------------------------------------------------------------------------------------------
-// The paper's two-stage RK2 (Heun) with one migration per stage (R-25).
-//   stage 1: K1 = (U(X0) - V0)/tau + g ; X1 = X0 + dt V0 ; X0 and K1 kept in group B, V0 stays in the slabs
-//   stage 2: V1 = V0 + dt K1 (recomputed: the same fma the oracle stored) ; K2 = (U(X1) - V1)/tau + g ;
-//            X = X0 + dt/2 (V0 + V1) ; V = V0 + dt/2 (K1 + K2)
-// tau = tau_p / f, f at the start of the stage.  Destination: per axis the minimum-image direction from the slab the
-// particle sits in to the owner of its new position (R-24's rule).  One warp per tile, unpipelined like k_push.
-// Of the paper's 17 arrays 14 travel between the stages (X1, V0, d, id in the slabs; X0, K1 in group B, whose two
-// spare arrays travel too): V1 never exists in memory.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ int min_image_dir(double a, const Geom& G, int Pa, int n_a, int p_a, bool& jump)
-{
-    if (!(a >= 0.0 && a < G.L)) { jump = true; return 0; }
-    int ic = __double2int_rd(a * G.inv_dx);
-    ic = max(0, min(ic, G.N - 1));
-    int dd = ic / n_a - p_a;
-    if (Pa >= 3) {
-        if (dd > 1) dd -= Pa;
-        else if (dd < -1) dd += Pa;
-    }
-    if (dd < -1 || dd > 1) { jump = true; dd = dd < -1 ? -1 : 1; }
-    return dd;
-}
-
-__device__ __forceinline__ double wrap_once(double xu, const Geom& G)
-{
-    if (xu < 0.0) { xu = xu + G.L; if (xu >= G.L) xu = G.L_below; }
-    else if (xu >= G.L) xu = xu - G.L;
-    return xu;                                     // still outside [0, L): min_image_dir raises the jump
-}
-
-template <int kStage>
-__global__ void __launch_bounds__(32 * kPushWarps, 3)
-k_rk2_stage(Geom G, Slabs S, Slabs SB, Tables T, const double* __restrict__ F4, double dt)
-{
-    const int s = blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint32_t first = (uint32_t)(blockIdx.x * kPushWarps + warp) * kTile;
-    const uint32_t cnt_s = T.count[s];
-    if (first >= cnt_s) return;
-    const int px = s % G.Px, py = (s / G.Px) % G.Py, pz = s / (G.Px * G.Py);
-    const SubBox Bx = sub_box(G, s);
-    const uint32_t nvalid = min((uint32_t)kTile, cnt_s - first);
-    const double hdt = 0.5 * dt;
-    bool jump = false;
-#pragma unroll 1
-    for (int r = 0; r < kRows; ++r) {
-        if (32u * r >= nvalid) break;
-        const bool valid = 32u * r + (uint32_t)lane < nvalid;
-        const uint32_t at = (uint32_t)s * (uint32_t)G.cap + first + min(32u * r + (uint32_t)lane, nvalid - 1u);
-        double x[3], v0[3], v[3], k1[3], x0[3];
-        // every streamed value of the row is requested before the first one is used (one exposed DRAM latency per row)
-#pragma unroll
-        for (int a = 0; a < 3; ++a) x[a] = __longlong_as_double(ld_stream(S.f[a] + at));
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { v0[a] = __longlong_as_double(ld_stream(S.f[3 + a] + at)); k1[a] = 0.0; x0[a] = 0.0; }
-        const double d = __longlong_as_double(ld_stream(S.f[6] + at));
-        if (kStage == 2) {
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                k1[a] = __longlong_as_double(ld_stream(SB.f[3 + a] + at));
-                x0[a] = __longlong_as_double(ld_stream(SB.f[a] + at));
-            }
-        }
-        Gath Q;
-        gather_issue(Q, F4, G, Bx, x[0], x[1], x[2], lane);
-#pragma unroll
-        for (int a = 0; a < 3; ++a) v[a] = (kStage == 2) ? fma(dt, k1[a], v0[a]) : v0[a];     // V1, recomputed (R-25)
-        double tau = (G.K_tau * d) * d;
-        const Vec3 Uv = gather_reduce(Q, lane);
-        const double U[3] = {Uv.x, Uv.y, Uv.z};
-        if (G.drag_model == 1) tau = tau / drag_factor(d, v[0] - U[0], v[1] - U[1], v[2] - U[2], G.inv_nu);
-        const double g[3] = {G.gx, G.gy, G.gz};
-        double k[3], pos[3], vn[3];
-#pragma unroll
-        for (int a = 0; a < 3; ++a) k[a] = (U[a] - v[a]) / tau + g[a];          // Eq. 6 + g (R-4)
-        if (kStage == 1) {
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                pos[a] = wrap_once(fma(dt, v0[a], x[a]), G);                    // X1 = X0 + dt V0
-                vn[a] = v0[a];                                                  // V0 stays; V1 = V0 + dt K1 is recomputed
-            }
-            if (valid) {
-#pragma unroll
-                for (int a = 0; a < 3; ++a) {
-                    st_stream(SB.f[a] + at, __double_as_longlong(x[a])); st_stream(SB.f[3 + a] + at, __double_as_longlong(k[a]));
-                }
-            }
-        } else {
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                pos[a] = wrap_once(fma(hdt, v0[a] + v[a], x0[a]), G);           // X = X0 + dt/2 (V0 + V1)
-                vn[a] = fma(hdt, k1[a] + k[a], v0[a]);                          // V = V0 + dt/2 (K1 + K2)
-            }
-        }
-        bool jmp = false;
-        const int code = kStay + min_image_dir(pos[0], G, G.Px, G.nx, px, jmp) + 3 * min_image_dir(pos[1], G, G.Py, G.ny, py, jmp)
-                       + 9 * min_image_dir(pos[2], G, G.Pz, G.nz, pz, jmp);
-        if (valid) {
-            jump |= jmp;
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                st_stream(S.f[a] + at, __double_as_longlong(pos[a]));
-                if (kStage == 2) st_stream(S.f[3 + a] + at, __double_as_longlong(vn[a]));
-            }
-            S.code[at] = (uint8_t)code;
-        }
-    }
-    if (jump) raise(T.status, -5);
 }
 
 // ---------------------------------------------------------------------------------------------
