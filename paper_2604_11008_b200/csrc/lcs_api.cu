@@ -36,6 +36,9 @@ struct lcs_handle {
     Slabs SB;                          // RK2: x0 y0 z0 k1x k1y k1z + 2 spare arrays (a group of 8 for the tile pass)
     CUtensorMap mapB;
     size_t gacc_bytes;
+    cudaStream_t copy_stream;          // lcs_step_fused_host: the host copies run here, beside the kernels (created on first use)
+    cudaEvent_t ev[12];                // start, x/y/z in, all in, one per array out, copies done
+    bool have_copy_stream;
 };
 
 namespace {
@@ -318,6 +321,11 @@ int lcs_destroy(lcs_t* h)
     if (!h) return LCS_ERR_INVALID_ARG;
     cudaStreamSynchronize(h->stream);
     if (h->prof) lcs_profile_end(h, nullptr, nullptr, nullptr, nullptr);
+    if (h->have_copy_stream) {
+        cudaStreamSynchronize(h->copy_stream);
+        for (auto& e : h->ev) cudaEventDestroy(e);
+        cudaStreamDestroy(h->copy_stream);
+    }
     delete h;
     return LCS_OK;
 }
@@ -336,10 +344,10 @@ int lcs_set_fluid(lcs_t* h, const double* d_u, const double* d_v, const double* 
     return check_launch(h);
 }
 
-int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y, const double* d_z,
-                      const double* d_vx, const double* d_vy, const double* d_vz, const double* d_diam,
-                      const int64_t* d_id)
-{
+static int set_particles_impl(lcs_t* h, int64_t n, const double* d_x, const double* d_y, const double* d_z,
+                              const double* d_vx, const double* d_vy, const double* d_vz, const double* d_diam,
+                              const int64_t* d_id, cudaEvent_t rest_ready)
+{   // rest_ready (may be null): an event after which d_vx .. d_id are valid; owner, scan and tile index need x, y, z only
     if (!h || n < 0) return LCS_ERR_INVALID_ARG;
     const Geom& G = h->G;
     if (n > (int64_t)G.P * G.cap) return LCS_ERR_INVALID_ARG;
@@ -359,6 +367,7 @@ int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y,
         k_set_owner<<<ntiles, 256, (size_t)G.P * 4, h->stream>>>(G, h->T, n, d_x, d_y, d_z, owner, tilehist);
     k_set_scan<<<(G.P + 31) / 32, 1024, 0, h->stream>>>(G, h->T, ntiles, tilehist, n);
     k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, 0);
+    if (rest_ready) cudaStreamWaitEvent(h->stream, rest_ready, 0);
     if (ntiles > 0) {
         int W = 8;                                                           // warps per tile, a power of two: W * P 16-bit
         while (W > 1 && W * G.P > 16384) W >>= 1;                             // counters in shared memory
@@ -370,6 +379,13 @@ int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y,
         k_set_scatter<<<ntiles, 32 * W, smem, h->stream>>>(G, h->S, n, I, owner, tilehist, W);
     }
     return check_launch(h, ntiles > 0 ? 4 : 2);
+}
+
+int lcs_set_particles(lcs_t* h, int64_t n, const double* d_x, const double* d_y, const double* d_z,
+                      const double* d_vx, const double* d_vy, const double* d_vz, const double* d_diam,
+                      const int64_t* d_id)
+{
+    return set_particles_impl(h, n, d_x, d_y, d_z, d_vx, d_vy, d_vz, d_diam, d_id, nullptr);
 }
 
 int lcs_particle_step(lcs_t* h, double dt)
@@ -545,24 +561,52 @@ int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8
     for (int a = 0; a < 8; ++a) {
         if (!h_in[a] || !h_out[a]) return LCS_ERR_INVALID_ARG;
         if ((reinterpret_cast<uintptr_t>(h_in[a]) | reinterpret_cast<uintptr_t>(h_out[a])) & 7u) return LCS_ERR_INVALID_ARG;
-        if (cudaMemcpyAsync(st + a * arr, h_in[a], (size_t)n * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
-            return LCS_ERR_CUDA;
     }
+    // The host copies run on a stream of their own, ordered against the kernels by events, one array at a time: the
+    // owner / scan kernels (x, y, z only) run under the copy-in of the other five arrays, and the copy-out of array a
+    // runs under the packing of array a+1.  The two directions cannot overlap: the step needs every particle.
+    if (!h->have_copy_stream) {
+        if (cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return LCS_ERR_CUDA;
+        for (auto& e : h->ev)
+            if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return LCS_ERR_CUDA;
+        h->have_copy_stream = true;
+    }
+    cudaStream_t cs = h->copy_stream;
+    cudaEvent_t ev_start = h->ev[0], ev_xyz = h->ev[1], ev_all = h->ev[2], ev_done = h->ev[11];
+    cudaEventRecord(ev_start, h->stream);                       // earlier work on the handle's stream (staging reuse) comes first
+    cudaStreamWaitEvent(cs, ev_start, 0);
+    for (int a = 0; a < 8; ++a) {
+        if (cudaMemcpyAsync(st + a * arr, h_in[a], (size_t)n * 8, cudaMemcpyHostToDevice, cs) != cudaSuccess) return LCS_ERR_CUDA;
+        if (a == 2) cudaEventRecord(ev_xyz, cs);
+    }
+    cudaEventRecord(ev_all, cs);
     double* f[7];
     for (int a = 0; a < 7; ++a) f[a] = reinterpret_cast<double*>(st + a * arr);
     int64_t* ids = reinterpret_cast<int64_t*>(st + 7 * arr);
     int64_t* d_counts = reinterpret_cast<int64_t*>(st + 8 * arr);
-    int rc = lcs_set_particles(h, n, f[0], f[1], f[2], f[3], f[4], f[5], f[6], ids);
+    cudaStreamWaitEvent(h->stream, ev_xyz, 0);
+    int rc = set_particles_impl(h, n, f[0], f[1], f[2], f[3], f[4], f[5], f[6], ids, ev_all);
     if (rc) return rc;
     rc = lcs_step_fused(h, dt);
     if (rc) return rc;
-    rc = lcs_get_particles(h, d_counts, f[0], f[1], f[2], f[3], f[4], f[5], f[6], ids);
+    // packed copy-out, one array per launch, each followed by its device-to-host copy on the copy stream
+    const Geom& G = h->G;
+    k_counts_out<<<1, 256, 0, h->stream>>>(G, h->T, d_counts, h->prefix);
+    const dim3 cgrid((unsigned)((G.cap + kCopyTile - 1) / kCopyTile), G.P);
+    for (int a = 0; a < 8; ++a) {
+        OutPtrs O;
+        for (int q = 0; q < 7; ++q) O.f[q] = (q == a) ? f[q] : nullptr;
+        O.id = (a == 7) ? ids : nullptr; O.code = nullptr;
+        k_copy_out<<<cgrid, 256, 0, h->stream>>>(G, h->S, h->T, h->prefix, O, 0);
+        cudaEventRecord(h->ev[3 + a], h->stream);
+        cudaStreamWaitEvent(cs, h->ev[3 + a], 0);
+        if (cudaMemcpyAsync(h_out[a], st + a * arr, (size_t)n * 8, cudaMemcpyDeviceToHost, cs) != cudaSuccess) return LCS_ERR_CUDA;
+        if (a == 0 && cudaMemcpyAsync(h_counts, d_counts, (size_t)G.P * 8, cudaMemcpyDeviceToHost, cs) != cudaSuccess) return LCS_ERR_CUDA;
+    }
+    cudaEventRecord(ev_done, cs);
+    cudaStreamWaitEvent(h->stream, ev_done, 0);
+    rc = check_launch(h, 9);
     if (rc) return rc;
-    for (int a = 0; a < 8; ++a)
-        if (cudaMemcpyAsync(h_out[a], st + a * arr, (size_t)n * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
-            return LCS_ERR_CUDA;
-    if (cudaMemcpyAsync(h_counts, d_counts, (size_t)h->G.P * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
-        return LCS_ERR_CUDA;
     return lcs_get_status(h, nullptr, nullptr, nullptr);
 }
 
