@@ -171,7 +171,10 @@ int lcs_get_status(lcs_t* h, int* sticky_error, int64_t* n_total, int64_t* n_mig
  * h_out arrays need room for n; 8-byte aligned).  d_staging: device scratch, 256-byte aligned, of at
  * least lcs_staging_bytes(n, P) bytes (eight arrays of n words, each rounded up to 256 bytes, plus
  * the P counts; 0 for n < 0 or P < 1).  LCS_ERR_INVALID_ARG for a null or misaligned pointer or a
- * staging block that is too small. */
+ * staging block that is too small.  The host copies run on a copy stream the handle creates on first use (the only CUDA
+ * object the library creates besides profiling events; destroyed by lcs_destroy), ordered against the handle's stream by
+ * events, one array at a time; host buffers should be pinned, or the copies serialise with the kernels.  On return the
+ * handle's stream is synchronised and h_out / h_counts are complete. */
 size_t lcs_staging_bytes(int64_t n, int P);
 int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8], void* const h_out[8],
                         int64_t* h_counts, void* d_staging, size_t staging_bytes);
