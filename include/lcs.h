@@ -69,9 +69,9 @@ typedef struct {
 /* Bytes of device workspace lcs_create needs; 0 if the arguments are invalid. */
 size_t lcs_workspace_bytes(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params* prm);
 
-/* Create a handle.  N: fluid grid points per axis (2 <= N <= 1625, divisible by Px, Py and Pz, and
+/* Create a handle.  N: fluid grid points per axis (N >= 2, divisible by Px, Py and Pz, and
  * Px*Py*Pz*(N/Px+2)*(N/Py+2)*(N/Pz+2) < 2^32: the fluid is kept as one brick of cells plus a one-cell periodic halo
- * per subdomain and record indices are 32-bit; N = 1625 needs at least two subdomains along one axis);
+ * per subdomain and record indices are 32-bit, which allows N <= 1623 with one subdomain and less with many);
  * Px, Py, Pz: 1..1024 each, Px*Py*Pz <= 8192; capacity: particle slots per subdomain slab (it must
  * be even, so that slab bases and tile runs stay 16-byte aligned, and P*capacity < 2^31: slots are
  * 32-bit indices); LCS_ERR_INVALID_ARG otherwise.  d_workspace: device block of at

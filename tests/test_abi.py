@@ -38,12 +38,15 @@ def test_version_and_workspace_size_checks(lib):
     assert ok > 8 * 8 * 4096 * 8                                 # at least the eight slabs
     prm_rk2 = LcsParams(1.5e-5, 1000.0, (C.c_double * 3)(0, 0, 0), 0, 0, 1)
     assert lib.lcs_workspace_bytes(32, 2, 2, 2, 4096, C.byref(prm_rk2)) >= ok + 8 * 8 * 4096 * 8   # + the RK2 group
+    assert lib.lcs_workspace_bytes(1623, 1, 1, 1, 4096, C.byref(prm)) > 1625 ** 3 * 32          # 1625^3 records < 2^32
     bad = [
         (33, 2, 2, 2, 4096, prm),                                # N not divisible by Px
         (1, 1, 1, 1, 4096, prm),                                 # N < 2
         (32, 2, 2, 2, 4095, prm),                                # odd capacity
         (32, 2, 2, 2, 0, prm),                                   # no capacity
         (2048, 2, 2, 2, 4096, prm),                              # N > 1625 (32-bit record indices)
+        (1624, 1, 1, 1, 4096, prm),                              # one brick of 1626^3 records >= 2^32 (1623 is the limit)
+        (1600, 8, 8, 8, 4096, prm),                              # 512 bricks of 202^3 records >= 2^32
         (32, 2, 2, 2, 1 << 31, prm),                             # capacity beyond 2^31 - 1
         (32, 2, 2, 2, 1 << 28, prm),                             # P * capacity = 2^31: slot indices and copy coordinates
         (32, 2, 2, 2, 4096, LcsParams(0.0, 1000.0, (C.c_double * 3)(0, 0, 0), 0, 0, 0)),        # nu <= 0
