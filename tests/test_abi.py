@@ -46,7 +46,7 @@ def test_version_and_workspace_size_checks(lib):
         (32, 2, 2, 2, 0, prm),                                   # no capacity
         (2048, 2, 2, 2, 4096, prm),                              # N > 1625 (32-bit record indices)
         (1624, 1, 1, 1, 4096, prm),                              # one brick of 1626^3 records >= 2^32 (1623 is the limit)
-        (1600, 8, 8, 8, 4096, prm),                              # 512 bricks of 202^3 records >= 2^32
+        (1616, 8, 8, 8, 4096, prm),                              # 512 bricks of 204^3 records >= 2^32
         (32, 2, 2, 2, 1 << 31, prm),                             # capacity beyond 2^31 - 1
         (32, 2, 2, 2, 1 << 28, prm),                             # P * capacity = 2^31: slot indices and copy coordinates
         (32, 2, 2, 2, 4096, LcsParams(0.0, 1000.0, (C.c_double * 3)(0, 0, 0), 0, 0, 0)),        # nu <= 0
