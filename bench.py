@@ -379,6 +379,30 @@ def run_cuda(args):
                       "particles_per_s": n / (ms_total / args.steps * 1e-3)},
         }
 
+    # ---- the state the timed steps left, checked on the device with properties that hold at any size (the element-wise
+    # comparison with the oracle is the job of tests/, which runs the same launch configuration): every id exactly once,
+    # and every particle inside the subdomain of the slab it sits in
+    post = None
+    if args.post_check:
+        st = lcs.get_particles(n)
+        ids = st["id"]
+        ref = torch.arange(n, dtype=torch.int64, device=dev)
+        ids_ok = bool(ids.sum() == ref.sum()) and bool((ids * ids).sum() == (ref * ref).sum()) and int(ids.min()) == 0 and int(ids.max()) == n - 1
+        del ref
+        inv_dx = N / (2.0 * np.pi)
+        own = None
+        for k, Pk, mul in (("x", cfg["P"][0], 1), ("y", cfg["P"][1], cfg["P"][0]), ("z", cfg["P"][2], cfg["P"][0] * cfg["P"][1])):
+            c = torch.clamp(torch.floor(st[k] * inv_dx).to(torch.int64), 0, N - 1) // (N // Pk) * mul
+            own = c if own is None else own + c
+        slab = torch.repeat_interleave(torch.arange(P, dtype=torch.int64, device=dev), st["counts"])
+        misplaced = int((own != slab).sum()) if slab.numel() == n else -1
+        post = {"ids_each_once": ids_ok, "particles_outside_their_slab": misplaced, "count_sum": int(st["counts"].sum()),
+                "note": "after the timed fused steps and the phase calls; property checks on the device, not an oracle comparison"}
+        del st, ids, own, slab
+        if not ids_ok or misplaced != 0:
+            print(f"bench.py: post-check failed: {post}", file=sys.stderr)
+            return 3
+
     # ---- end to end through the host-buffer entry point (rank-local, then max over ranks) ----------
     e2e = None
     if args.e2e_steps > 0:
@@ -483,7 +507,7 @@ def run_cuda(args):
                    "dt": dt, "migrant_fraction_last_step": m, "drag_model": args.drag_model,
                    "l2": "inputs larger than L2 (no flush)",
                    "parallelism": "independent box per GPU" if world > 1 else "single GPU"},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "phases": phases,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "phases": phases, "post_check": post,
         "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
@@ -507,6 +531,7 @@ def main():
                     help="0: Stokes drag (BASELINE.json's configs); 1: f = 1 + 0.15 Re^0.687 (SURVEY 8(f) NEXT #2)")
     ap.add_argument("--rk2", action="store_true",
                     help="also time lcs_step_rk2 (SURVEY 8(f) NEXT #1); reserves 8 more arrays of P*capacity doubles")
+    ap.add_argument("--post-check", type=int, default=1, help="1: check the id multiset and the containment of the final state on the device")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), reported as roofline.traffic")
     args = ap.parse_args()
