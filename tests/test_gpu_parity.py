@@ -247,7 +247,8 @@ def test_axis_sweeps_match_oracle(torch_cuda, oracle_lib, P, N):
     dev.close(); dev_direct.close()
 
 
-@pytest.mark.parametrize("P,drag_model", [((2, 2, 2), 0), ((3, 2, 1), 0), ((1, 1, 1), 0), ((4, 4, 2), 1), ((2, 2, 2), 1)])
+@pytest.mark.parametrize("P,drag_model", [((2, 2, 2), 0), ((3, 2, 1), 0), ((1, 1, 1), 0), ((4, 4, 2), 1), ((2, 2, 2), 1),
+                                          ((12, 12, 8), 1)])     # P = 1152 > 1024: the stages with the tables in global memory
 def test_two_stage_rk2_matches_oracle(torch_cuda, oracle_lib, P, drag_model):
     """lcs_step_rk2 (the paper's two-stage RK2 with a migration of all 17 arrays after stage 1 and one after stage 2;
     SURVEY 8(f) NEXT #1, DESIGN R-25) against the oracle: ids, order, counts exact, state 0 ulp, in the paper's regime
