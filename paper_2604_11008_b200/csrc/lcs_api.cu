@@ -35,6 +35,7 @@ struct lcs_handle {
     bool rk2;                          // the 9 extra arrays of the two-stage RK2 exist (lcs_params.enable_rk2)
     Slabs SB;                          // RK2: x0 y0 z0 k1x k1y k1z + 2 spare arrays (a group of 8 for the tile pass)
     CUtensorMap mapB;
+    CUtensorMap map_push_ld, map_push_st;   // the slabs again with a box of 7 rows (x .. d, loads) and of 6 rows (x .. vz, stores)
     size_t gacc_bytes;
     cudaStream_t copy_stream;          // lcs_step_fused_host: the host copies run here, beside the kernels (created on first use)
     cudaEvent_t ev[12];                // start, x/y/z in, all in, one per array out, copies done
@@ -274,6 +275,8 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
     h->prefix = reinterpret_cast<int64_t*>(w + L.prefix);
     h->stream = static_cast<cudaStream_t>(cuda_stream);
     if (!make_slab_map(&h->slab_map, w + L.slab_f[0], (size_t)P * (size_t)capacity, L.slab_f[1] - L.slab_f[0])) { delete h; return LCS_ERR_CUDA; }
+    if (!make_slab_map(&h->map_push_ld, w + L.slab_f[0], (size_t)P * (size_t)capacity, L.slab_f[1] - L.slab_f[0], 7) ||
+        !make_slab_map(&h->map_push_st, w + L.slab_f[0], (size_t)P * (size_t)capacity, L.slab_f[1] - L.slab_f[0], 6)) { delete h; return LCS_ERR_CUDA; }
     h->rk2 = prm->enable_rk2 == 1;
     if (h->rk2) {   // the RK2 group: same stride and shape as the slabs, so the same tile pass moves it
         const size_t st = L.slab_f[1] - L.slab_f[0];
@@ -299,11 +302,13 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
             setup(k_tile_pass<2, true, 0>, occ_f); setup(k_tile_pass<2, true, 1>, occ_f);
             setup(k_tile_pass<3, true, 0>, occ_f); setup(k_tile_pass<3, true, 1>, occ_f);
             setup(k_tile_pass<0, true, 0>, occ_p);
+            setup(k_push_tiles<true, 0>, occ_f); setup(k_push_tiles<true, 1>, occ_f);
         } else {
             setup(k_tile_pass<1, false, 0>, occ_f); setup(k_tile_pass<1, false, 1>, occ_f);
             setup(k_tile_pass<2, false, 0>, occ_f); setup(k_tile_pass<2, false, 1>, occ_f);
             setup(k_tile_pass<3, false, 0>, occ_f); setup(k_tile_pass<3, false, 1>, occ_f);
             setup(k_tile_pass<0, false, 0>, occ_p);
+            setup(k_push_tiles<false, 0>, occ_f); setup(k_push_tiles<false, 1>, occ_f);
         }
         if (sms < 1) sms = 148;
         const long long max_tiles = ((long long)G.P * G.tiles_per_sub + kWarps - 1) / kWarps;
@@ -395,7 +400,15 @@ int lcs_particle_step(lcs_t* h, double dt)
     if (h->sticky) return h->sticky;
     const Geom& G = h->G;
     cudaMemsetAsync(h->T.cnt, 0, (size_t)G.P * 32 * 4, h->stream);
-    k_push<<<dim3((G.tiles_per_sub + kPushWarps - 1) / kPushWarps, G.P), 32 * kPushWarps, 0, h->stream>>>(G, h->S, h->T, h->fluid4, dt);
+    {
+        const size_t smem = tile_pass_smem(G.P);
+        const bool big = G.P > kTableSmemMax, sn = G.drag_model == 1;
+#define LCS_LAUNCH_PUSH(B, D) \
+    k_push_tiles<B, D><<<h->grid_fused, kBlock, smem, h->stream>>>(G, h->S, h->T, h->fluid4, dt, h->map_push_ld, h->map_push_st)
+        if (big) { if (sn) LCS_LAUNCH_PUSH(true, 1); else LCS_LAUNCH_PUSH(true, 0); }
+        else     { if (sn) LCS_LAUNCH_PUSH(false, 1); else LCS_LAUNCH_PUSH(false, 0); }
+#undef LCS_LAUNCH_PUSH
+    }
     h->pushed = true;
     return check_launch(h);
 }

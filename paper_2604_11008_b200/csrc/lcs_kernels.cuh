@@ -575,68 +575,6 @@ __device__ __forceinline__ uint32_t pack_xyz(const Geom& G, int s)
     return (uint32_t)px | ((uint32_t)py << 10) | ((uint32_t)pz << 20);
 }
 
-// a1-a3 for this lane's particle (all 32 lanes must call), unpipelined: the unfused push hides latency with
-// resident warps.  Same arithmetic, same order as the row pipeline of the tile pass.  Returns the destination code.
-__device__ __forceinline__ int push_particle(Particle& p, const double* __restrict__ F4, const Geom& G,
-                                             const SubBox& B, double dt, int lane, bool& jump)
-{
-    Gath Q;
-    gather_issue(Q, F4, G, B, p.x, p.y, p.z, lane);
-    Drag D;
-    if (G.drag_model == 0) D = drag_coeffs(p.d, dt, G);       // independent of the gather: issued under its latency
-    const Vec3 U = gather_reduce(Q, lane);
-    if (G.drag_model == 1)                                    // f needs the slip V - U(X) (DESIGN R-23)
-        D = drag_coeffs(p.d, dt, G, drag_factor(p.d, p.vx - U.x, p.vy - U.y, p.vz - U.z, G.inv_nu), true);
-    return advance_particle(p, U, D, G, B, dt, jump);
-}
-
-// ---------------------------------------------------------------------------------------------
-// K1: unfused push (a1-a4), lcs_particle_step.  One warp per tile; in place; codes + count table.
-// ---------------------------------------------------------------------------------------------
-constexpr int kPushWarps = 4;                      // 128-thread CTAs, four per SM (<= 128 registers)
-#ifndef LCS_PUSH_BLOCKS
-#define LCS_PUSH_BLOCKS 4
-#endif
-__global__ void __launch_bounds__(32 * kPushWarps, LCS_PUSH_BLOCKS)
-k_push(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt)
-{
-    const int s = blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int t = blockIdx.x * kPushWarps + warp;
-    const uint32_t cnt_s = T.count[s];
-    const int64_t first = (int64_t)t * kTile;
-    if (first >= (int64_t)cnt_s) return;
-    const SubBox B = sub_box(G, s);
-    uint32_t cnt_c = 0;
-    bool jump = false;
-#pragma unroll 1
-    for (int r = 0; r < kRows; ++r) {
-        const int64_t slot = first + 32 * r + lane;
-        if (first + 32 * r >= (int64_t)cnt_s) break;
-        const bool valid = slot < (int64_t)cnt_s;
-        const size_t at = (size_t)s * (size_t)G.cap + (size_t)slot;
-        Particle p{0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 1.0};
-        if (valid) {
-            p.x = __longlong_as_double(ld_stream(S.f[0] + at)); p.y = __longlong_as_double(ld_stream(S.f[1] + at));
-            p.z = __longlong_as_double(ld_stream(S.f[2] + at)); p.vx = __longlong_as_double(ld_stream(S.f[3] + at));
-            p.vy = __longlong_as_double(ld_stream(S.f[4] + at)); p.vz = __longlong_as_double(ld_stream(S.f[5] + at));
-            p.d = __longlong_as_double(ld_stream(S.f[6] + at));
-        }
-        bool jmp = false;
-        int code = push_particle(p, F4, G, B, dt, lane, jmp);
-        if (valid) {
-            jump |= jmp;
-            st_stream(S.f[0] + at, __double_as_longlong(p.x)); st_stream(S.f[1] + at, __double_as_longlong(p.y));
-            st_stream(S.f[2] + at, __double_as_longlong(p.z)); st_stream(S.f[3] + at, __double_as_longlong(p.vx));
-            st_stream(S.f[4] + at, __double_as_longlong(p.vy)); st_stream(S.f[5] + at, __double_as_longlong(p.vz));
-            S.code[at] = (uint8_t)code;
-        } else code = kInvalid;
-        (void)row_rank(code, valid, lane, cnt_c);
-    }
-    if (jump) raise(T.status, -5);
-    if (lane < kNC && cnt_c) atomicAdd(&T.cnt[s * 32 + lane], cnt_c);      // a4
-}
-
 struct TileRef { int s, t; uint32_t cnt; uint32_t codes; bool ok; };   // a ticketed tile: subdomain, tile index, count[s];
                                                                         // unfused pass: this lane's code bytes, one per row
 
@@ -1006,6 +944,170 @@ k_tile_pass(Geom G, Slabs S, Slabs Snd, Tables T, const double* __restrict__ F4,
         cur = nxt;
         nxt = nn;
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K1: unfused push (a1-a4), lcs_particle_step, as a persistent pipeline like the tile pass but without any
+// cross-warp protocol: every warp takes the tiles g = warp, warp + W, ... of the compact tile index (no tickets: a push
+// has no ordering to respect), brings them in by bulk tensor copies two tiles ahead, runs the same row pipeline (gather
+// of the next row in flight under the advance of the current one), writes x, v back with ONE bulk tensor store per
+// tile (six rows of the buffer; ragged last tiles of a slab use plain stores, a bulk store would run into the next
+// slab), the code byte per slot and the count table by one atomic per (tile, code present).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void bulk_tensor2d_s2g(const CUtensorMap* tmap, uint32_t c0, uint32_t c1, uint32_t src)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"(tmap), "r"(c0), "r"(c1), "r"(src) : "memory");
+}
+
+template <bool kBig, int kDrag>
+__global__ void LCS_TP_BOUNDS
+k_push_tiles(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt,
+             const __grid_constant__ CUtensorMap map_ld, const __grid_constant__ CUtensorMap map_st)
+{
+    extern __shared__ __align__(128) unsigned char s_raw[];
+    TileBuf* bufs = reinterpret_cast<TileBuf*>(s_raw);
+    uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_raw + kWarps * kNBuf * sizeof(TileBuf));
+    uint32_t* s_ts = reinterpret_cast<uint32_t*>(s_bar + kWarps * kNBuf);
+    uint32_t* s_xyz = s_ts + (G.P + 1);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (!kBig) {
+        for (int i = threadIdx.x; i <= G.P; i += kBlock) {
+            s_ts[i] = T.tile_start[i];
+            if (i < G.P) s_xyz[i] = pack_xyz(G, i);
+        }
+    }
+    TileBuf* const my = bufs + warp * kNBuf;
+    const uint32_t bar0 = smem_u32(s_bar + warp * kNBuf);
+    if (lane == 0) {
+#pragma unroll
+        for (int b = 0; b < kNBuf; ++b) mbar_init(bar0 + 8u * b, 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    auto ts = [&](int i) -> uint32_t { return kBig ? __ldg(T.tile_start + i) : s_ts[i]; };
+    auto box_of = [&](int s) -> SubBox {
+        const uint32_t c3 = kBig ? pack_xyz(G, s) : s_xyz[s];
+        SubBox B;
+        B.lox = (int)(c3 & 1023u) * G.nx; B.loy = (int)((c3 >> 10) & 1023u) * G.ny; B.loz = (int)(c3 >> 20) * G.nz;
+        B.base = (uint32_t)s * G.brick;
+        return B;
+    };
+    const unsigned int n_active = ts(G.P);
+    const uint32_t cap32 = (uint32_t)G.cap;
+    const unsigned int stride = gridDim.x * kWarps;
+    int s_hint = 0;
+    uint32_t phase = 0;
+    auto resolve = [&](TileRef& R, unsigned int g) {           // tile index -> (subdomain, tile); g increases per warp
+        R.ok = g < n_active; R.s = R.t = 0; R.cnt = 0; R.codes = 0u;
+        if (R.ok) {
+            int s = s_hint;
+            while (g >= ts(s + 1)) ++s;
+            s_hint = s;
+            R.s = s; R.t = (int)(g - ts(s)); R.cnt = __ldg(T.count + s);
+        }
+    };
+    auto issue_load = [&](const TileRef& R, int b) {
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+            const uint32_t bar = bar0 + 8u * b;
+            mbar_expect_tx(bar, 7u * kTile * 8u);              // x y z vx vy vz d
+            bulk_tensor2d_g2s(smem_u32(&my[b].f[0][0]), &map_ld, (uint32_t)R.s * cap32 + (uint32_t)R.t * kTile, 0u, bar);
+        }
+    };
+    auto wait_buf = [&](int b) { mbar_wait(bar0 + 8u * b, (phase >> b) & 1u); phase ^= 1u << b; };
+
+    TileRef cur, nxt, nn;
+    unsigned int g = blockIdx.x * kWarps + warp;
+    resolve(cur, g);
+    if (!cur.ok) return;
+    issue_load(cur, 0);
+    resolve(nxt, g + stride);
+    if (nxt.ok) issue_load(nxt, 1);
+    Gath Q;
+    wait_buf(0);
+    {
+        const unsigned long long* px = &my[0].f[0][0];
+        gather_issue(Q, F4, G, box_of(cur.s), __longlong_as_double(px[lane]), __longlong_as_double(px[kTile + lane]),
+                     __longlong_as_double(px[2 * kTile + lane]), lane);
+    }
+    int bc = 0;
+    bool jump = false;
+    while (cur.ok) {
+        g += stride;
+        resolve(nn, g + stride);
+        TileBuf& W = my[bc];
+        const int bn = bc + 1 == kNBuf ? 0 : bc + 1;
+        const int s = cur.s;
+        const uint32_t first = (uint32_t)cur.t * kTile;
+        const uint32_t nvalid = min((uint32_t)kTile, cur.cnt - first);
+        const int nrows = (int)((nvalid + 31u) >> 5);
+        const SubBox B = box_of(s);
+        const uint32_t slot0 = (uint32_t)s * cap32 + first;
+        uint32_t cnt_c = 0;                                    // lane c: particles of this tile with code c
+#pragma unroll 1
+        for (int r = 0; r < kRows; ++r) {
+            if (r >= nrows) break;
+            const uint32_t p = 32u * (uint32_t)r + (uint32_t)lane;
+            Drag D;
+            D.tau = D.alpha = D.b = 0.0;
+            if (kDrag == 0) D = drag_coeffs(__longlong_as_double(W.f[6][p]), dt, G);
+            const Vec3 U = gather_reduce(Q, lane);
+            {   // gather of the next row: of this tile, or row 0 of the next tile (whose bulk copy must have landed)
+                const unsigned long long* px = &W.f[0][32 * r];
+                SubBox Bg = B;
+                if (r + 1 < nrows) px += 32;
+                else if (nxt.ok) { wait_buf(bn); px = &my[bn].f[0][0]; Bg = box_of(nxt.s); }
+                gather_issue(Q, F4, G, Bg, __longlong_as_double(px[lane]), __longlong_as_double(px[kTile + lane]),
+                             __longlong_as_double(px[2 * kTile + lane]), lane);
+            }
+            const bool valid = p < nvalid;
+            Particle q;
+            q.x = __longlong_as_double(W.f[0][p]); q.y = __longlong_as_double(W.f[1][p]);
+            q.z = __longlong_as_double(W.f[2][p]); q.vx = __longlong_as_double(W.f[3][p]);
+            q.vy = __longlong_as_double(W.f[4][p]); q.vz = __longlong_as_double(W.f[5][p]);
+            q.d = 0.0;
+            if (kDrag == 1) {
+                const double dd = __longlong_as_double(W.f[6][p]);
+                D = drag_coeffs(dd, dt, G, drag_factor(dd, q.vx - U.x, q.vy - U.y, q.vz - U.z, G.inv_nu), true);
+            }
+            bool jmp = false;
+            int code = advance_particle(q, U, D, G, B, dt, jmp);
+            jump |= jmp && valid;
+            W.f[0][p] = __double_as_longlong(q.x); W.f[1][p] = __double_as_longlong(q.y);
+            W.f[2][p] = __double_as_longlong(q.z); W.f[3][p] = __double_as_longlong(q.vx);
+            W.f[4][p] = __double_as_longlong(q.vy); W.f[5][p] = __double_as_longlong(q.vz);
+            if (valid) S.code[slot0 + p] = (uint8_t)code; else code = kInvalid;
+            (void)row_rank(code, valid, lane, cnt_c);
+        }
+        if (lane < kNC && cnt_c) atomicAdd(&T.cnt[s * 32 + lane], cnt_c);      // a4
+        // write-back of x, v
+        if (nvalid == (uint32_t)kTile) {
+            fence_proxy_async();                               // the tile's generic-proxy stores come before the bulk store
+            __syncwarp();
+            if (lane == 0) {
+                bulk_tensor2d_s2g(&map_st, slot0, 0u, smem_u32(&W.f[0][0]));
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
+        } else {
+            __syncwarp();
+            for (uint32_t p = lane; p < nvalid; p += 32) {
+#pragma unroll
+                for (int a = 0; a < 6; ++a) st_stream(S.f[a] + slot0 + p, W.f[a][p]);
+            }
+            if (lane == 0) asm volatile("cp.async.bulk.commit_group;" ::: "memory");      // an empty group keeps the count in step
+        }
+        // the buffer of the tile before this one receives the tile after next: its bulk store must have read it
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+        __syncwarp();
+        if (nn.ok) issue_load(nn, bc + 2 >= kNBuf ? bc + 2 - kNBuf : bc + 2);
+        bc = bn;
+        cur = nxt;
+        nxt = nn;
+    }
+    if (jump) raise(T.status, -5);
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // ---------------------------------------------------------------------------------------------
