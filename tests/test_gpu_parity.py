@@ -175,6 +175,12 @@ def test_many_subdomains_and_long_slabs(torch_cuda, oracle_lib, P, N, per_sub):
         dev.step_fused(0.6)
         assert dev.get_status() == (0, n, o.n_migrated_last)
         compare_packed(dev, o, f"P={P} step {step}")
+    # the unfused pair on the same tables: the push pipeline (k_push_tiles) and the migration-only tile pass
+    assert o.step(0.6) == 0
+    dev.particle_step(0.6)
+    dev.migrate()
+    assert dev.get_status() == (0, n, o.n_migrated_last)
+    compare_packed(dev, o, f"P={P} unfused step")
     dev.close()
 
 
