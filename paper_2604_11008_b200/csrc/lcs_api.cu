@@ -190,7 +190,7 @@ int enqueue_tile_pass(lcs_t* h, int mode, double dt, const Slabs* grp = nullptr,
 #undef LCS_LAUNCH_MODE
 #undef LCS_LAUNCH_TP
     if (rec) cudaEventRecord(ev[1], h->stream);
-    k_send_scan<<<G.P, 256, 0, h->stream>>>(G, h->Snd, h->T);
+    k_send_scan<<<G.P, 32 * kScanWarps, 0, h->stream>>>(G, h->Snd, h->T);
     k_table<<<(G.P + 7) / 8, 256, 0, h->stream>>>(G, h->T);
     if (rec) cudaEventRecord(ev[2], h->stream);
     k_unpack<<<dim3((G.chunks_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, S, h->Snd, h->T);

@@ -1114,7 +1114,7 @@ k_push_tiles(Geom G, Slabs S, Tables T, const double* __restrict__ F4, double dt
 // K2b (a4/a5 for the migrants): the send region of a subdomain holds its migrants in slot order, each with its code.
 // Per chunk of kChunk migrants: the per-code counts, then their exclusive prefix over the chunks of the region (what
 // the unpack needs to turn "k-th migrant with code c of the region" into a slot of the receiver), and the totals
-// cnt[s][c] of the count table; cnt[s][13] = stayers.  One CTA of 8 warps per subdomain, lane c owns code c; each warp
+// cnt[s][c] of the count table; cnt[s][13] = stayers.  One CTA of 32 warps per subdomain, lane c owns code c; each warp
 // takes a contiguous range of chunks.  The totals of the region come from the look-back accumulators of the tile pass.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t chunk_hist(const uint8_t* __restrict__ codes, uint32_t n, int lane, uint32_t* s_cnt)
@@ -1134,11 +1134,12 @@ __device__ __forceinline__ uint32_t chunk_hist(const uint8_t* __restrict__ codes
     return c;
 }
 
-__global__ void __launch_bounds__(256)
+constexpr int kScanWarps = 32;                     // warps of a k_send_scan CTA: each takes a contiguous range of chunks
+__global__ void __launch_bounds__(32 * kScanWarps)
 k_send_scan(Geom G, Slabs Snd, Tables T)
 {
-    __shared__ uint32_t s_part[8][32];
-    __shared__ uint32_t s_hist[8][32];
+    __shared__ uint32_t s_part[kScanWarps][32];
+    __shared__ uint32_t s_hist[kScanWarps][32];
     __shared__ uint32_t s_tot[2];
     const int s = blockIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -1150,7 +1151,7 @@ k_send_scan(Geom G, Slabs Snd, Tables T)
         const int nt = (int)((cnt_s + kTile - 1) / kTile);
         const int ngrp = (nt + 31) / 32;
         uint32_t st = 0, mg = 0;
-        for (int g = threadIdx.x; g < ngrp; g += 256) {
+        for (int g = threadIdx.x; g < ngrp; g += 32 * kScanWarps) {
             const unsigned long long w = T.gacc[(size_t)s * G.lbgroups_per_sub + g];
             st += (uint32_t)(w & kField20); mg += (uint32_t)((w >> 20) & kField20);
         }
@@ -1161,7 +1162,7 @@ k_send_scan(Geom G, Slabs Snd, Tables T)
     const uint32_t n_stay = s_tot[0];
     const uint32_t n_mig = (uint32_t)min((unsigned long long)s_tot[1], (unsigned long long)G.send_cap);   // overflow: already raised
     const int nch = (int)((n_mig + kChunk - 1) / kChunk);
-    const int per = (nch + 7) / 8;
+    const int per = (nch + kScanWarps - 1) / kScanWarps;
     const int q0 = min(nch, warp * per), q1 = min(nch, q0 + per);
     const uint8_t* codes = Snd.code + (size_t)s * (size_t)G.send_cap;
     uint32_t* ce = T.chunk_excl + (size_t)s * G.chunks_per_sub * 32;
@@ -1174,7 +1175,7 @@ k_send_scan(Geom G, Slabs Snd, Tables T)
     s_part[warp][lane] = sum;
     __syncthreads();
     uint32_t run = 0, total = 0;
-    for (int w = 0; w < 8; ++w) { const uint32_t v = s_part[w][lane]; if (w < warp) run += v; total += v; }
+    for (int w = 0; w < kScanWarps; ++w) { const uint32_t v = s_part[w][lane]; if (w < warp) run += v; total += v; }
     for (int q = q0; q < q1; ++q) {                       // counts -> exclusive prefix, in place (this warp wrote them)
         const uint32_t c = ce[(size_t)q * 32 + lane];
         ce[(size_t)q * 32 + lane] = run;
