@@ -428,7 +428,8 @@ int lcs_migrate_sweeps(lcs_t* h)
     if (h->sticky) return h->sticky;
     const Geom& G = h->G;
     for (int axis = 0; axis < 3; ++axis) {
-        k_classify_axis<<<dim3((unsigned)((G.cap + 255) / 256), G.P), 256, 0, h->stream>>>(G, h->S, h->T, axis);
+        k_classify_axis<<<dim3((unsigned)((G.cap + 1023) / 1024), G.P), 256, 0, h->stream>>>(G, h->S.f[axis], h->S.code, h->T.count,
+                                                                                                h->T.status, axis);
         int rc = check_launch(h);
         if (rc == LCS_OK) rc = enqueue_tile_pass(h, 0, 0.0);
         if (rc != LCS_OK) return rc;

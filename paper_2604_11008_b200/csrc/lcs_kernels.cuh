@@ -1364,34 +1364,44 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
 // ---------------------------------------------------------------------------------------------
 // Axis-by-axis exchange (R-24): destination code along ONE axis from the particle's current
 // position relative to the slab it sits in (minimum-image difference of subdomain indices), written
-// as the code byte the unfused tile pass consumes.  One thread per slot.
+// as the code byte the unfused tile pass consumes.  Four slots per thread.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_classify_axis(Geom G, Slabs S, Tables T, int axis)
-{
+k_classify_axis(Geom G, const double* __restrict__ pos, uint8_t* __restrict__ code, const uint32_t* __restrict__ count,
+                int* status, int axis)
+{   // pos: the slab array of this axis (passed as a pointer: indexing the parameter struct with a run-time axis would
+    // move it to local memory); four slots per thread, 1024 per CTA
     const int s = blockIdx.y;
-    const uint32_t cnt_s = T.count[s];
-    const uint32_t i = blockIdx.x * 256u + threadIdx.x;
-    if (i >= cnt_s) return;
+    const uint32_t cnt_s = count[s];
+    const uint32_t i0 = blockIdx.x * 1024u + threadIdx.x;
+    if (i0 >= cnt_s) return;
     const int Pa = axis == 0 ? G.Px : (axis == 1 ? G.Py : G.Pz);
     const int n_a = axis == 0 ? G.nx : (axis == 1 ? G.ny : G.nz);
     const int p_a = axis == 0 ? s % G.Px : (axis == 1 ? (s / G.Px) % G.Py : s / (G.Px * G.Py));
     const int w = axis == 0 ? 1 : (axis == 1 ? 3 : 9);
-    const uint32_t at = (uint32_t)s * (uint32_t)G.cap + i;
-    const double a = S.f[axis][at];
-    int dd = 0;
-    if (!(a >= 0.0 && a < G.L)) raise(T.status, -5);
-    else {
-        int ic = __double2int_rd(a * G.inv_dx);
-        ic = max(0, min(ic, G.N - 1));
-        dd = ic / n_a - p_a;
-        if (Pa >= 3) {
-            if (dd > 1) dd -= Pa;
-            else if (dd < -1) dd += Pa;
+    const uint32_t base = (uint32_t)s * (uint32_t)G.cap;
+    double a[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) a[k] = (i0 + 256u * k < cnt_s) ? pos[base + i0 + 256u * k] : 0.0;
+    bool bad = false;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (i0 + 256u * k >= cnt_s) break;
+        int dd = 0;
+        if (!(a[k] >= 0.0 && a[k] < G.L)) bad = true;
+        else {
+            int ic = __double2int_rd(a[k] * G.inv_dx);
+            ic = max(0, min(ic, G.N - 1));
+            dd = ic / n_a - p_a;
+            if (Pa >= 3) {
+                if (dd > 1) dd -= Pa;
+                else if (dd < -1) dd += Pa;
+            }
+            if (dd < -1 || dd > 1) { bad = true; dd = dd < -1 ? -1 : 1; }
         }
-        if (dd < -1 || dd > 1) { raise(T.status, -5); dd = dd < -1 ? -1 : 1; }
+        code[base + i0 + 256u * k] = (uint8_t)(kStay + dd * w);
     }
-    S.code[at] = (uint8_t)(kStay + dd * w);
+    if (bad) raise(status, -5);
 }
 
 // ---------------------------------------------------------------------------------------------
