@@ -518,7 +518,7 @@ int lcs_pair_count(lcs_t* h, double r_lo, double r_hi, int64_t* d_count)
     const size_t idx_bytes = 3 * arr_bytes;
     if (h->pool_bytes < idx_bytes + 1024) return LCS_ERR_INVALID_ARG;
     const size_t avail = h->pool_bytes - idx_bytes;
-    long long M = std::min<long long>(256, (long long)std::floor(G.L / r_hi));
+    long long M = std::min<long long>(400, (long long)std::floor(G.L / r_hi));   // 400^3 cells = 15,625 scan chunks (k_scan_top takes 16,384)
     M = std::min<long long>(M, std::max<long long>(3, (long long)std::cbrt((double)slots)));   // about one particle per cell
     while (M > 3 && (size_t)(8 * M * M * M + 4 + 4 * ((M * M * M + kScanChunk - 1) / kScanChunk) + 256) > avail) --M;
     if (M < 3) return LCS_ERR_INVALID_ARG;

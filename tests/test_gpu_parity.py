@@ -327,7 +327,7 @@ def test_host_buffer_entry_point_matches_oracle(torch_cuda, oracle_lib):
 def test_pair_count_matches_oracle(torch_cuda, oracle_lib):
     """lcs_pair_count (the statistic behind g(r), R-26) against the oracle's O(n^2) definition:
     integer, bit-exact.  Uniform and clumped particles, several decompositions, shells that hit the cell-list limits
-    (r_hi = L/3: three cells per axis; tiny shells: 256 cells per axis), before and after migration steps."""
+    (r_hi = L/3: three cells per axis; tiny shells: as many cells per axis as the particle count allows), before and after migration steps."""
     from paper_2604_11008_b200 import LCS, LcsError, LCS_ERR_INVALID_ARG
     rng = np.random.default_rng(21)
     for P, N, n in (((2, 2, 2), 16, 6000), ((1, 1, 1), 8, 1), ((3, 2, 1), 12, 9001), ((4, 4, 4), 32, 20000)):
