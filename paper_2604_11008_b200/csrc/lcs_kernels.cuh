@@ -321,7 +321,7 @@ __device__ __forceinline__ uint32_t row_rank(int code, bool valid, int lane, uin
 // a fastest for the reads (runs along i in the input) and c fastest for the writes (runs of records along k in the
 // brick), so neither side wastes lanes on the ragged extents nx+2, nz+2.  Halo cells are read from their periodic images.
 // ---------------------------------------------------------------------------------------------
-constexpr int kRpA = 96, kRpC = 16;            // largest chunk: kRpA indices along a times kRpC along c
+constexpr int kRpA = 66, kRpC = 12;            // largest chunk: kRpA indices along a times kRpC along c (19 KB: eight CTAs per SM)
 
 __global__ void __launch_bounds__(256)
 k_repack_fluid(Geom G, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
