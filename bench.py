@@ -244,6 +244,17 @@ def run_cuda(args):
     lcs = LCS(N, *cfg["P"], cfg["capacity"], g=cfg["g"], drag_model=args.drag_model, rk2=args.rk2, device=dev)
     lcs.set_fluid(wl["u"], wl["v"], wl["w"])
     parts = wl["particles"]
+    if args.order == "morton":
+        # labelled variant (never the headline): the same particles, handed over sorted by the Morton key of their cell, so
+        # that the particles of a tile gather from neighbouring cells ("may be reported as a labelled variant")
+        key = torch.zeros(n, dtype=torch.int64, device=dev)
+        cells = [torch.clamp((parts[k] * (N / (2.0 * np.pi))).to(torch.int64), 0, N - 1) for k in "xyz"]
+        for b in range(int(N - 1).bit_length()):
+            for a in range(3):
+                key |= ((cells[a] >> b) & 1) << (3 * b + a)
+        perm = torch.argsort(key)
+        parts = {k: parts[k][perm].contiguous() for k in F8}
+        del key, cells, perm
     lcs.set_particles(*(parts[k] for k in F8))
     err, n_tot, _ = lcs.get_status()
     if (err or n_tot != n):
@@ -504,7 +515,7 @@ def run_cuda(args):
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg["name"], "N": N, "P": cfg["P"], "particles_per_gpu": n, "capacity": cfg["capacity"],
-                   "dt": dt, "migrant_fraction_last_step": m, "drag_model": args.drag_model,
+                   "dt": dt, "migrant_fraction_last_step": m, "drag_model": args.drag_model, "particle_order": args.order,
                    "l2": "inputs larger than L2 (no flush)",
                    "parallelism": "independent box per GPU" if world > 1 else "single GPU"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "phases": phases, "post_check": post,
@@ -531,6 +542,9 @@ def main():
                     help="0: Stokes drag (BASELINE.json's configs); 1: f = 1 + 0.15 Re^0.687 (SURVEY 8(f) NEXT #2)")
     ap.add_argument("--rk2", action="store_true",
                     help="also time lcs_step_rk2 (SURVEY 8(f) NEXT #1); reserves 8 more arrays of P*capacity doubles")
+    ap.add_argument("--order", default="generation", choices=["generation", "morton"],
+                    help="order in which the particles are handed to lcs_set_particles: generation order (spatially random, the "
+                         "headline) or sorted by the Morton key of their cell (a labelled variant)")
     ap.add_argument("--post-check", type=int, default=1, help="1: check the id multiset and the containment of the final state on the device")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), reported as roofline.traffic")
