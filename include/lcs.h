@@ -48,6 +48,7 @@ extern "C" {
 #define LCS_ERR_JUMP         (-5)   /* sticky: displacement > one subdomain, or non-finite        */
 #define LCS_ERR_RANGE        (-6)   /* sticky: lcs_set_particles saw a position outside [0, L)     */
 #define LCS_ERR_NOMEM        (-7)   /* host memory for the handle could not be allocated           */
+#define LCS_ERR_TOO_LARGE    (-8)   /* lcs_pair_count_static: the handle exceeds the built-in scratch */
 
 #define LCS_STAY_CODE 13
 
@@ -159,6 +160,44 @@ int lcs_get_count_table(lcs_t* h, int64_t* d_table);
  * lcs_particle_step and lcs_migrate.  LCS_ERR_INVALID_ARG unless 0 <= r_lo < r_hi <= L/3; LCS_ERR_STATE without
  * particles or with a pending push. */
 int lcs_pair_count(lcs_t* h, double r_lo, double r_hi, int64_t* d_count);
+
+/* lcs_pair_count for callers that have no device memory left to lend and may not ask the CUDA runtime for more.
+ *
+ * Who that is: lcs_pair_count borrows the handle's send pool for the positions sorted by cell and for its cell list,
+ * and gives up (LCS_ERR_INVALID_ARG) when that pool is smaller than three position arrays -- which is exactly what a
+ * production run has when it sized send_capacity for the few per cent of particles that migrate.  The obvious way out,
+ * a larger workspace, is closed to a diagnostics hook that is called from inside a running time loop: by then the host
+ * application (the flow solver, an in-situ analysis framework, a job that handed all of HBM to its own pool at start-up)
+ * owns every byte of device memory and forbids cudaMalloc / cudaFree in the loop, because those calls stall every stream
+ * of the device while they run and can fail with the memory already spoken for.  Such a caller passes what it has -- the
+ * handle (its particles are the input) and the 8-byte result word -- and this entry point brings its own scratch.
+ *
+ * Where the scratch lives: in ONE array of LCS_PAIR_COUNT_STATIC_BYTES (17 MiB) that is part of the library's device
+ * image.  Every GPU on which the library's kernels are loaded carries these 17 MiB from then until the process exits,
+ * whether or not this function is ever called; that is the price, and the reason the limit is modest.  The call itself
+ * performs no cudaMalloc, cudaFree or any other allocating runtime or library call, on the host or on the device.
+ *
+ * Limit: Px*Py*Pz*capacity <= LCS_PAIR_COUNT_STATIC_MAX_SLOTS (2^19 = 524,288 particle slots).  A larger handle gets
+ * LCS_ERR_TOO_LARGE and nothing is enqueued: use lcs_pair_count with a send pool of at least 3/8 of capacity instead.
+ *
+ * First call on a device: looks up the device address of the array (cudaGetSymbolAddress with that device current) and
+ * remembers it per device; later calls on that device only read the remembered pointer.  Make this first call during
+ * set-up, outside any stream capture.  The device that is current at the call must be the one that owns the handle's
+ * workspace (LCS_ERR_INVALID_ARG otherwise: each GPU has its own copy of the array, and another GPU's address is not
+ * usable); with more than LCS_PAIR_COUNT_STATIC_MAX_DEVICES (64) devices, ordinals beyond that get LCS_ERR_INVALID_ARG.
+ *
+ * Sharing: all handles and all threads of the process that use one GPU share the one array.  It still holds the previous
+ * call's cell list and sorted positions when a call begins; the call clears the part that has to start at zero (the cell
+ * counters) in stream order before it uses it, so back-to-back calls on one stream are independent.  Two calls whose
+ * GPU work can overlap -- different streams, or different host threads driving different handles -- race on the array
+ * and both results are then garbage: serialise them (one stream, or an event between them).
+ *
+ * Same arguments, same result (bit-exact count), same state rules and error codes as lcs_pair_count otherwise; the send
+ * pool is not touched, so unlike lcs_pair_count it does not matter how small send_capacity is. */
+#define LCS_PAIR_COUNT_STATIC_MAX_SLOTS   (1 << 19)
+#define LCS_PAIR_COUNT_STATIC_BYTES       (17u << 20)
+#define LCS_PAIR_COUNT_STATIC_MAX_DEVICES 64
+int lcs_pair_count_static(lcs_t* h, double r_lo, double r_hi, int64_t* d_count);
 
 /* Synchronises the stream and reads the status word.  Any out pointer may be NULL.
  * Returns the sticky error (0 if none). */

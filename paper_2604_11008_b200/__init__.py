@@ -6,4 +6,5 @@ entry point fails loudly if the library or a CUDA device is missing.
 """
 from .binding import (LCS, LcsError, lib_path, load_library, EXPORTED_SYMBOLS,  # noqa: F401
                       LCS_OK, LCS_ERR_INVALID_ARG, LCS_ERR_STATE, LCS_ERR_CUDA, LCS_ERR_CAPACITY,
-                      LCS_ERR_JUMP, LCS_ERR_RANGE, LCS_ERR_NOMEM)
+                      LCS_ERR_JUMP, LCS_ERR_RANGE, LCS_ERR_NOMEM, LCS_ERR_TOO_LARGE,
+                      LCS_PAIR_COUNT_STATIC_MAX_SLOTS)

@@ -7,11 +7,13 @@ import os
 
 LCS_OK, LCS_ERR_INVALID_ARG, LCS_ERR_STATE, LCS_ERR_CUDA = 0, -1, -2, -3
 LCS_ERR_CAPACITY, LCS_ERR_JUMP, LCS_ERR_RANGE, LCS_ERR_NOMEM = -4, -5, -6, -7
+LCS_ERR_TOO_LARGE = -8
+LCS_PAIR_COUNT_STATIC_MAX_SLOTS = 1 << 19
 
 EXPORTED_SYMBOLS = (
     "lcs_workspace_bytes", "lcs_create", "lcs_destroy", "lcs_set_fluid", "lcs_set_particles",
     "lcs_particle_step", "lcs_migrate", "lcs_migrate_sweeps", "lcs_step_rk2", "lcs_step_fused", "lcs_get_counts", "lcs_get_particles",
-    "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_staging_bytes", "lcs_step_fused_host", "lcs_pair_count", "lcs_probe_gather",
+    "lcs_get_codes", "lcs_get_count_table", "lcs_get_status", "lcs_staging_bytes", "lcs_step_fused_host", "lcs_pair_count", "lcs_pair_count_static", "lcs_probe_gather",
     "lcs_profile_begin", "lcs_profile_end", "lcs_kernel_launches", "lcs_version")
 
 FIELDS = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
@@ -19,7 +21,9 @@ FIELDS = ("x", "y", "z", "vx", "vy", "vz", "d", "id")
 
 class LcsError(RuntimeError):
     def __init__(self, fn, code):
-        super().__init__(f"{fn} returned {code}")
+        why = (f": the handle has more than {LCS_PAIR_COUNT_STATIC_MAX_SLOTS} particle slots (P*capacity), the limit of the "
+               "library's built-in scratch" if code == LCS_ERR_TOO_LARGE else "")
+        super().__init__(f"{fn} returned {code}{why}")
         self.code = code
 
 
@@ -67,6 +71,7 @@ def load_library(build_if_missing: bool = True):
     L.lcs_get_count_table.argtypes = [vp, vp]
     L.lcs_get_status.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(i64), C.POINTER(i64)]
     L.lcs_pair_count.argtypes = [vp, dbl, dbl, vp]
+    L.lcs_pair_count_static.argtypes = [vp, dbl, dbl, vp]
     L.lcs_probe_gather.argtypes = [vp, dbl, C.c_int, C.POINTER(dbl), C.POINTER(dbl)]
     L.lcs_staging_bytes.restype = C.c_size_t
     L.lcs_staging_bytes.argtypes = [i64, C.c_int]
@@ -210,6 +215,19 @@ class LCS:
         """-> device int64 tensor (1 element): unordered pairs with periodic separation in [r_lo, r_hi) (R-26)."""
         out = self._torch.empty(1, dtype=self._torch.int64, device=self.device)
         self._chk("lcs_pair_count", self._L.lcs_pair_count(self._h, float(r_lo), float(r_hi), _ptr(out)))
+        return out
+
+    def pair_count_static(self, r_lo, r_hi, out=None):
+        """pair_count for a caller that has no device memory to lend and may not allocate any (a diagnostics hook inside
+        a time loop whose host application owns all of HBM and bans cudaMalloc there): the scratch is a fixed 17 MiB array
+        inside the library instead of the send pool, so P*capacity must not exceed LCS_PAIR_COUNT_STATIC_MAX_SLOTS
+        (LcsError with LCS_ERR_TOO_LARGE otherwise).  Pass `out` (1-element int64 device tensor) and the call allocates
+        nothing at all; without it the binding asks torch for the 8-byte result.  One shared array per GPU: calls that
+        could overlap on the device (two streams) must be serialised by the caller.  include/lcs.h has the details."""
+        if out is None:
+            out = self._torch.empty(1, dtype=self._torch.int64, device=self.device)
+        assert out.is_cuda and out.dtype == self._torch.int64 and out.numel() == 1
+        self._chk("lcs_pair_count_static", self._L.lcs_pair_count_static(self._h, float(r_lo), float(r_hi), _ptr(out)))
         return out
 
     def probe_gather(self, window_mb, iters=200):

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -686,3 +687,94 @@ int lcs_probe_gather(lcs_t* h, double window_mb, int iters, double* h_ms, double
 int64_t lcs_kernel_launches(lcs_t* h) { return h ? h->launches : 0; }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// lcs_pair_count_static: the pair count for a caller that cannot lend scratch and must not allocate (include/lcs.h has
+// the full story: a diagnostics hook inside a time loop whose host application owns all device memory and bans
+// cudaMalloc / cudaFree there, with a send pool too small for lcs_pair_count).  The kernels are lcs_pair_count's own;
+// only the place of the scratch differs: the array below, which belongs to the library's device image.
+//
+// g_pc_static is a DEVICE array.  Seen from host code its name is only a handle the runtime knows the array by: taking
+// its address on the host yields a host address, and a kernel handed that address faults (or scribbles over host memory
+// on systems where the GPU can reach it).  The usable pointer comes from cudaGetSymbolAddress, asked once per device
+// with that device current, because every GPU that loads this image has its own copy at its own address.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+static __device__ __align__(256) unsigned char g_pc_static[LCS_PAIR_COUNT_STATIC_BYTES];
+
+std::mutex g_pc_static_lock;
+void* g_pc_static_ptr[LCS_PAIR_COUNT_STATIC_MAX_DEVICES];     // device address of g_pc_static on device d, or null
+
+// Device address of g_pc_static on the current device (set-up on the first call per device); null on failure.
+void* pc_static_scratch(int* dev_out)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= LCS_PAIR_COUNT_STATIC_MAX_DEVICES) return nullptr;
+    *dev_out = dev;
+    std::lock_guard<std::mutex> guard(g_pc_static_lock);
+    if (!g_pc_static_ptr[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_pc_static) != cudaSuccess || !p) {
+            cudaGetLastError();                                // the failure is reported by the return value
+            return nullptr;
+        }
+        g_pc_static_ptr[dev] = p;
+    }
+    return g_pc_static_ptr[dev];
+}
+
+}  // namespace
+
+extern "C" int lcs_pair_count_static(lcs_t* h, double r_lo, double r_hi, int64_t* d_count)
+{
+    if (!h || !d_count || (reinterpret_cast<uintptr_t>(d_count) & 7u)) return LCS_ERR_INVALID_ARG;
+    if (!(r_lo >= 0.0) || !(r_hi > r_lo) || !std::isfinite(r_hi)) return LCS_ERR_INVALID_ARG;
+    const Geom& G = h->G;
+    if (r_hi > G.L / 3.0) return LCS_ERR_INVALID_ARG;          // the cell list needs at least three cells per axis
+    if (!h->have_particles || h->pushed) return LCS_ERR_STATE;
+    if (h->sticky) return h->sticky;
+    const size_t slots = (size_t)G.P * (size_t)G.cap;
+    if (slots > (size_t)LCS_PAIR_COUNT_STATIC_MAX_SLOTS) return LCS_ERR_TOO_LARGE;
+    int dev = -1;
+    unsigned char* base = static_cast<unsigned char*>(pc_static_scratch(&dev));
+    if (!base) return dev < 0 ? LCS_ERR_INVALID_ARG : LCS_ERR_CUDA;
+    {   // the array of THIS device: the handle's particles must live on the device that is current
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, h->S.f[0]) != cudaSuccess) { cudaGetLastError(); return LCS_ERR_CUDA; }
+        if (at.type == cudaMemoryTypeDevice && at.device != dev) return LCS_ERR_INVALID_ARG;
+    }
+    // carve: positions sorted by cell (three arrays of `slots` doubles), cell starts [ncell + 1], fill counters [ncell],
+    // chunk sums of the scan [nchunks]
+    const size_t arr_bytes = align_up(slots * 8);
+    const size_t idx_bytes = 3 * arr_bytes;
+    const size_t avail = (size_t)LCS_PAIR_COUNT_STATIC_BYTES - idx_bytes;     // >= 5 MiB by the slot limit
+    // cells of side > r_hi, so that partners are never more than one cell away; with three cells per axis the 27
+    // neighbours are the whole box and any side will do (r_hi = L/3 lands there)
+    long long M = std::max<long long>(3, std::min<long long>(400, (long long)std::floor(G.L / (r_hi * (1.0 + 1e-12)))));
+    M = std::min<long long>(M, std::max<long long>(3, (long long)std::cbrt((double)slots)));      // about one particle per cell
+    while (M > 3 && (size_t)(8 * M * M * M + 4 + 4 * ((M * M * M + kScanChunk - 1) / kScanChunk) + 256) > avail) --M;
+    if (M < 3) return LCS_ERR_INVALID_ARG;
+    const size_t ncell = (size_t)(M * M * M);
+    const int nchunks = (int)((ncell + kScanChunk - 1) / kScanChunk);
+    double* sx = reinterpret_cast<double*>(base);
+    double* sy = reinterpret_cast<double*>(base + arr_bytes);
+    double* sz = reinterpret_cast<double*>(base + 2 * arr_bytes);
+    uint32_t* cellstart = reinterpret_cast<uint32_t*>(base + idx_bytes);
+    uint32_t* cellfill = cellstart + ncell + 1;
+    uint32_t* sums = cellfill + ncell;
+    PairGeom Q;
+    Q.M = (int)M; Q.inv_cell = (double)M / G.L; Q.L = G.L; Q.half_L = 0.5 * G.L; Q.lo2 = r_lo * r_lo; Q.hi2 = r_hi * r_hi;
+    // the array still holds the last call's cell list: the counters and the result word must start at zero
+    if (cudaMemsetAsync(cellstart, 0, (2 * ncell + 1) * 4, h->stream) != cudaSuccess ||
+        cudaMemsetAsync(d_count, 0, 8, h->stream) != cudaSuccess) { cudaGetLastError(); return LCS_ERR_CUDA; }
+    const dim3 pgrid((unsigned)((G.cap + 255) / 256), G.P);
+    k_pc_count<<<pgrid, 256, 0, h->stream>>>(G, h->S, h->T, Q, cellstart);
+    k_scan_sums<<<nchunks, 256, 0, h->stream>>>(cellstart, ncell, sums);
+    k_scan_top<<<1, 1024, 0, h->stream>>>(sums, nchunks, cellstart + ncell);
+    k_scan_apply<<<nchunks, 256, 0, h->stream>>>(cellstart, ncell, sums);
+    k_pc_fill<<<pgrid, 256, 0, h->stream>>>(G, h->S, h->T, Q, cellstart, cellfill, sx, sy, sz);
+    k_pc_pairs<<<(unsigned)((slots + 255) / 256), 256, 0, h->stream>>>(Q, cellstart, sx, sy, sz, cellstart + ncell,
+                                                                        reinterpret_cast<unsigned long long*>(d_count));
+    return check_launch(h, 6);
+}
