@@ -202,6 +202,15 @@ def oracle_sample_rate(cfg, wl, stride, steps, torch):
     return n_s * steps / dt, dt / steps, n_s
 
 
+def bench_config(cfg, args, world):
+    """The `config` object of the JSON line: the workload as named, the same keys and values in both arms (the
+    reference arm times a bounded sample of it and says which in `sample` / `cpu_baseline.sample`)."""
+    return {"workload": cfg["name"], "N": cfg["N"], "P": cfg["P"], "particles_per_gpu": cfg["n"], "capacity": cfg["capacity"],
+            "dt": cfg["dt"], "drag_model": args.drag_model, "particle_order": args.order,
+            "l2": "inputs larger than L2 (no flush)",
+            "parallelism": "independent box per GPU" if world > 1 else "single GPU"}
+
+
 def run_reference(args):
     torch, rank, world, local = pick_device()
     if rank != 0:
@@ -216,7 +225,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": rate, "unit": "particles/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["name"], "N": cfg["N"], "P": cfg["P"], "particles": cfg["n"], "dt": cfg["dt"]},
+        "config": bench_config(cfg, args, world),
+        "sample": {"particles_timed_per_step": n_s, "stride": stride},
         "cpu_baseline": {"value": rate, "unit": "particles/s", "cores": 1, "kind": "oracle",
                          "sample": f"every {stride}th particle of {cfg['name']} ({n_s} particles, full {cfg['N']}^3 field), "
                                    f"{args.steps} steps, single thread"},
@@ -486,7 +496,8 @@ def run_cuda(args):
     # Every particle brings 64 B in by bulk copy and 8 x 32 B record sectors through L1 (random inside the brick of its
     # subdomain, which L2 holds); lcs_probe_gather measures, on the same fluid records and alone on the GPU, what the
     # memory system delivers for that pattern.
-    brick_mb = (N // cfg["P"][0] + 1) * (N // cfg["P"][1] + 1) * (N // cfg["P"][2] + 1) * 32 / 1048576.0
+    # one brick = the subdomain's cells plus a one-cell halo on both sides: (n + 2) records per axis
+    brick_mb = (N // cfg["P"][0] + 2) * (N // cfg["P"][1] + 2) * (N // cfg["P"][2] + 2) * 32 / 1048576.0
     try:
         ceil_l2 = lcs.probe_gather(brick_mb, 200)
         ceil_dram = lcs.probe_gather(N ** 3 * 32 / 1048576.0, 50)
@@ -514,10 +525,7 @@ def run_cuda(args):
         "metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["name"], "N": N, "P": cfg["P"], "particles_per_gpu": n, "capacity": cfg["capacity"],
-                   "dt": dt, "migrant_fraction_last_step": m, "drag_model": args.drag_model, "particle_order": args.order,
-                   "l2": "inputs larger than L2 (no flush)",
-                   "parallelism": "independent box per GPU" if world > 1 else "single GPU"},
+        "config": bench_config(cfg, args, world), "migrant_fraction_last_step": m,
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "phases": phases, "post_check": post,
         "cpu_baseline": cpu,
     }
