@@ -157,8 +157,10 @@ int lcs_get_count_table(lcs_t* h, int64_t* d_table);
  * r_lo <= r < r_hi; g over the shell = count / (n (n-1) / 2 * 4/3 pi (r_hi^3 - r_lo^3) / L^3).  Arithmetic per pair as
  * DESIGN.md R-26 fixes it, so the count is bit-exact against the O(n^2) definition.  Uses the send pool as scratch
  * (slot indices sorted by cell + a cell list of up to 256^3 cells): call it between steps, not between
- * lcs_particle_step and lcs_migrate.  LCS_ERR_INVALID_ARG unless 0 <= r_lo < r_hi <= L/3; LCS_ERR_STATE without
- * particles or with a pending push. */
+ * lcs_particle_step and lcs_migrate.  LCS_ERR_INVALID_ARG unless 0 <= r_lo < r_hi <= L/3, and also when the send pool
+ * cannot hold the scratch: it needs three arrays of P*capacity doubles plus at least 1 KB of cell list, i.e.
+ * lcs_params.send_capacity of roughly 3/8 of capacity or more (0 = capacity always suffices); a handle with a smaller
+ * pool can use lcs_pair_count_static below.  LCS_ERR_STATE without particles or with a pending push. */
 int lcs_pair_count(lcs_t* h, double r_lo, double r_hi, int64_t* d_count);
 
 /* lcs_pair_count for callers that have no device memory left to lend and may not ask the CUDA runtime for more.
@@ -221,7 +223,8 @@ int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8
 /* Optional per-kernel timing for benchmarks.  lcs_profile_begin creates CUDA events (no device
  * memory) and makes every following lcs_step_fused / lcs_migrate record four of them on the
  * handle's stream: before the tile pass, after it, after the table scan, after unpack + commit.
- * At most max_steps steps are recorded; later steps run untimed.  lcs_profile_end synchronises the
+ * At most max_steps steps are recorded; later steps run untimed.  A "step" here is one migration round: lcs_step_rk2
+ * records three (stage 1, the X0/K1 group, stage 2) and lcs_migrate_sweeps three (x, y, z), and n_steps counts them so.  lcs_profile_end synchronises the
  * stream, returns the summed durations in milliseconds and the number of recorded steps, and
  * destroys the events.  Any out pointer may be NULL. */
 int lcs_profile_begin(lcs_t* h, int max_steps);

@@ -66,7 +66,7 @@ inline size_t brick_records(int N, int Px, int Py, int Pz)
 bool valid_args(int N, int Px, int Py, int Pz, int64_t cap, const lcs_params* prm)
 {
     if (!prm) return false;
-    if (N < 2 || N > 1625 || Px < 1 || Py < 1 || Pz < 1) return false;
+    if (N < 2 || N > 1623 || Px < 1 || Py < 1 || Pz < 1) return false;   // (N + 2)^3 < 2^32 with one subdomain; the brick test below is the rule
     if (Px > 1024 || Py > 1024 || Pz > 1024) return false;   // packed subdomain coordinates (10 bits each)
     if (N % Px || N % Py || N % Pz) return false;
     const int64_t P = (int64_t)Px * Py * Pz;
@@ -147,12 +147,35 @@ inline size_t tile_pass_smem(int P)
     return kWarps * kNBuf * (sizeof(TileBuf) + sizeof(uint64_t)) + (P <= kTableSmemMax ? (size_t)(2 * P + 1) * sizeof(uint32_t) : 0);
 }
 
+// dynamic shared memory of k_set_scatter with W warps per tile
+inline size_t set_scatter_smem(int W, int P)
+{
+    return ((size_t)(W + 1) * P + 2 * kSetTile + 1) * 2 + (size_t)kSetTile * 4 + 16;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel (per device), not to a handle: it is set to the
+// largest size any handle can ask for -- the same value on every lcs_create -- so that live handles with different P
+// cannot lower it under one another.  Largest tile pass: P = kTableSmemMax (tables mirrored in shared memory); largest
+// k_set_scatter: P = 8192 with two warps per tile.
+inline void set_kernel_smem_limits()
+{
+    const int tp = (int)tile_pass_smem(kTableSmemMax);
+    auto lim = [tp](auto kernel) { cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, tp); };
+    lim(k_tile_pass<0, true, 0>); lim(k_tile_pass<0, false, 0>);
+    lim(k_tile_pass<1, true, 0>); lim(k_tile_pass<1, true, 1>); lim(k_tile_pass<1, false, 0>); lim(k_tile_pass<1, false, 1>);
+    lim(k_tile_pass<2, true, 0>); lim(k_tile_pass<2, true, 1>); lim(k_tile_pass<2, false, 0>); lim(k_tile_pass<2, false, 1>);
+    lim(k_tile_pass<3, true, 0>); lim(k_tile_pass<3, true, 1>); lim(k_tile_pass<3, false, 0>); lim(k_tile_pass<3, false, 1>);
+    lim(k_push_tiles<true, 0>); lim(k_push_tiles<true, 1>); lim(k_push_tiles<false, 0>); lim(k_push_tiles<false, 1>);
+    cudaFuncSetAttribute(k_set_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)set_scatter_smem(2, 8192));
+}
+
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 inline int check_launch(lcs_t* h, int n = 1)
 {
     h->launches += n;
-    return cudaPeekAtLastError() == cudaSuccess ? LCS_OK : LCS_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? LCS_OK : LCS_ERR_CUDA;   // consumed: a failed launch on one handle does not
+                                                                          // make every later call on every handle fail
 }
 
 // One round of the migration machinery on one group of 8 arrays (the slabs, or an RK2 group that travels with the same
@@ -194,11 +217,26 @@ int enqueue_tile_pass(lcs_t* h, int mode, double dt, const Slabs* grp = nullptr,
     k_send_scan<<<G.P, 32 * kScanWarps, 0, h->stream>>>(G, h->Snd, h->T);
     k_table<<<(G.P + 7) / 8, 256, 0, h->stream>>>(G, h->T);
     if (rec) cudaEventRecord(ev[2], h->stream);
-    k_unpack<<<dim3((G.chunks_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, S, h->Snd, h->T);
+    k_unpack<<<dim3((G.chunks_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, S, h->Snd, h->T, nf);
     k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, commit ? 1 : 0);     // (also resets the tile ticket for the next round)
     if (rec) { cudaEventRecord(ev[3], h->stream); ++h->prof_steps; }
     if (commit) h->pushed = false;
     return check_launch(h, 5);
+}
+
+// Cells per axis of the pair count's cell list (lcs_pair_count, lcs_pair_count_static).  The walk over the 27 neighbouring
+// cells finds every partner closer than r_hi only if the cell side L/M is LARGER than r_hi by more than the rounding of
+// the cell index (a * M/L, floored): with L/M == r_hi up to rounding (lattice data, r_hi = L/M) two particles that count
+// can sit two cells apart.  So M = floor(L / (r_hi (1 + 1e-12))), except that with three cells per axis the 27
+// neighbours are the whole box and any side will do (r_hi = L/3 lands there).  Then: about one particle per cell, at
+// most 400 per axis (15,625 scan chunks; k_scan_top takes 16,384), and whatever fits `avail` bytes of scratch.
+long long pair_cells_per_axis(double L, double r_hi, size_t slots, size_t avail)
+{
+    long long M = std::max<long long>(3, std::min<long long>(400, (long long)std::floor(L / (r_hi * (1.0 + 1e-12)))));
+    M = std::min<long long>(M, std::max<long long>(3, (long long)std::cbrt((double)slots)));
+    while (M > 3 && (size_t)(8 * M * M * M + 4 + 4 * ((M * M * M + kScanChunk - 1) / kScanChunk) + 256) > avail) --M;
+    if ((size_t)(8 * M * M * M + 4 + 4 * ((M * M * M + kScanChunk - 1) / kScanChunk) + 256) > avail) return 0;
+    return M;
 }
 
 }  // namespace
@@ -292,8 +330,8 @@ int lcs_create(int N, int Px, int Py, int Pz, int64_t capacity, const lcs_params
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         const size_t smem = tile_pass_smem(G.P);
+        set_kernel_smem_limits();
         auto setup = [&](auto kernel, int& occ) {
-            cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             int o = 0;
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kernel, kBlock, smem);
             occ = occ == 0 ? o : std::min(occ, o);
@@ -377,8 +415,7 @@ static int set_particles_impl(lcs_t* h, int64_t n, const double* d_x, const doub
     if (ntiles > 0) {
         int W = 8;                                                           // warps per tile, a power of two: W * P 16-bit
         while (W > 1 && W * G.P > 16384) W >>= 1;                             // counters in shared memory
-        const size_t smem = ((size_t)(W + 1) * G.P + 2 * kSetTile + 1) * 2 + (size_t)kSetTile * 4 + 16;
-        cudaFuncSetAttribute(k_set_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const size_t smem = set_scatter_smem(W, G.P);        // within the limit lcs_create set (set_kernel_smem_limits)
         InPtrs I;
         I.f[0] = d_x; I.f[1] = d_y; I.f[2] = d_z; I.f[3] = d_vx; I.f[4] = d_vy; I.f[5] = d_vz; I.f[6] = d_diam;
         I.id = d_id;
@@ -519,9 +556,7 @@ int lcs_pair_count(lcs_t* h, double r_lo, double r_hi, int64_t* d_count)
     const size_t idx_bytes = 3 * arr_bytes;
     if (h->pool_bytes < idx_bytes + 1024) return LCS_ERR_INVALID_ARG;
     const size_t avail = h->pool_bytes - idx_bytes;
-    long long M = std::min<long long>(400, (long long)std::floor(G.L / r_hi));   // 400^3 cells = 15,625 scan chunks (k_scan_top takes 16,384)
-    M = std::min<long long>(M, std::max<long long>(3, (long long)std::cbrt((double)slots)));   // about one particle per cell
-    while (M > 3 && (size_t)(8 * M * M * M + 4 + 4 * ((M * M * M + kScanChunk - 1) / kScanChunk) + 256) > avail) --M;
+    const long long M = pair_cells_per_axis(G.L, r_hi, slots, avail);
     if (M < 3) return LCS_ERR_INVALID_ARG;
     const size_t ncell = (size_t)(M * M * M);
     const int nchunks = (int)((ncell + kScanChunk - 1) / kScanChunk);
@@ -581,9 +616,15 @@ int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8
     // owner / scan kernels (x, y, z only) run under the copy-in of the other five arrays, and the copy-out of array a
     // runs under the packing of array a+1.  The two directions cannot overlap: the step needs every particle.
     if (!h->have_copy_stream) {
-        if (cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return LCS_ERR_CUDA;
-        for (auto& e : h->ev)
-            if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return LCS_ERR_CUDA;
+        if (cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return LCS_ERR_CUDA; }
+        int made = 0;
+        while (made < 12 && cudaEventCreateWithFlags(&h->ev[made], cudaEventDisableTiming) == cudaSuccess) ++made;
+        if (made < 12) {                                        // nothing half-made is left behind
+            cudaGetLastError();
+            while (made > 0) cudaEventDestroy(h->ev[--made]);
+            cudaStreamDestroy(h->copy_stream);
+            return LCS_ERR_CUDA;
+        }
         h->have_copy_stream = true;
     }
     cudaStream_t cs = h->copy_stream;
@@ -749,11 +790,7 @@ extern "C" int lcs_pair_count_static(lcs_t* h, double r_lo, double r_hi, int64_t
     const size_t arr_bytes = align_up(slots * 8);
     const size_t idx_bytes = 3 * arr_bytes;
     const size_t avail = (size_t)LCS_PAIR_COUNT_STATIC_BYTES - idx_bytes;     // >= 5 MiB by the slot limit
-    // cells of side > r_hi, so that partners are never more than one cell away; with three cells per axis the 27
-    // neighbours are the whole box and any side will do (r_hi = L/3 lands there)
-    long long M = std::max<long long>(3, std::min<long long>(400, (long long)std::floor(G.L / (r_hi * (1.0 + 1e-12)))));
-    M = std::min<long long>(M, std::max<long long>(3, (long long)std::cbrt((double)slots)));      // about one particle per cell
-    while (M > 3 && (size_t)(8 * M * M * M + 4 + 4 * ((M * M * M + kScanChunk - 1) / kScanChunk) + 256) > avail) --M;
+    const long long M = pair_cells_per_axis(G.L, r_hi, slots, avail);
     if (M < 3) return LCS_ERR_INVALID_ARG;
     const size_t ncell = (size_t)(M * M * M);
     const int nchunks = (int)((ncell + kScanChunk - 1) / kScanChunk);

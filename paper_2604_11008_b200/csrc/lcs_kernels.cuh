@@ -451,7 +451,8 @@ __device__ __forceinline__ void gather_issue(Gath& Q, const double* __restrict__
     const int a0 = axis_stencil(x, G.inv_dx, B.lox, G.nx, fx);
     const int b0 = axis_stencil(y, G.inv_dx, B.loy, G.ny, fy);
     const int c0 = axis_stencil(z, G.inv_dx, B.loz, G.nz, Q.fz);
-    const uint32_t rec = B.base + (uint32_t)(c0 + G.bj * b0 + G.bi * a0);     // corner (i0, j0, k0); < 2^32 (lcs_create)
+    const uint32_t rec = B.base + (uint32_t)c0 + (uint32_t)G.bj * (uint32_t)b0 + (uint32_t)G.bi * (uint32_t)a0;   // corner (i0, j0, k0);
+                                                       // < 2^32 (lcs_create), above 2^31 for large bricks: unsigned arithmetic
     const int le = lane & ~1, lo = lane | 1;
     const uint32_t zs = (uint32_t)(lane & 1);                                 // this lane always fetches z-side (lane & 1)
     const double* pA = F4 + 4 * (size_t)(__shfl_sync(0xffffffffu, rec, le) + zs);
@@ -1275,8 +1276,8 @@ k_table(Geom G, Tables T)
 constexpr int kUnpackWarps = LCS_UNPACK_WARPS;
 
 __global__ void __launch_bounds__(32 * kUnpackWarps)
-k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
-{
+k_unpack(Geom G, Slabs S, Slabs Snd, Tables T, int nf)
+{   // nf: live arrays of the group (8 = seven fields + id; the RK2 group of X0, K1 has 6 and its send rows 6, 7 were never written)
     __shared__ uint32_t s_dst[kUnpackWarps][kChunk];      // sorted by code: destination slot (global index)
     __shared__ uint8_t s_src[kUnpackWarps][kChunk];       // sorted by code: position in the chunk
     __shared__ uint32_t s_next[kUnpackWarps][32], s_at[kUnpackWarps][32];
@@ -1348,15 +1349,15 @@ k_unpack(Geom G, Slabs S, Slabs Snd, Tables T)
         for (int u = 0; u < 2; ++u)
             if (dst[u] != 0xffffffffu) {
 #pragma unroll
-                for (int a = 0; a < 7; ++a) v[u][a] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.f[a] + src[u]));
-                v[u][7] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.id + src[u]));
+                for (int a = 0; a < 7; ++a) if (a < nf) v[u][a] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.f[a] + src[u]));
+                if (nf == 8) v[u][7] = __ldg(reinterpret_cast<const unsigned long long*>(Snd.id + src[u]));
             }
 #pragma unroll
         for (int u = 0; u < 2; ++u)
             if (dst[u] != 0xffffffffu) {
 #pragma unroll
-                for (int a = 0; a < 7; ++a) S.f[a][dst[u]] = __longlong_as_double(v[u][a]);
-                S.id[dst[u]] = (int64_t)v[u][7];
+                for (int a = 0; a < 7; ++a) if (a < nf) S.f[a][dst[u]] = __longlong_as_double(v[u][a]);
+                if (nf == 8) S.id[dst[u]] = (int64_t)v[u][7];
             }
     }
 }
