@@ -192,14 +192,47 @@ def oracle_sample_rate(cfg, wl, stride, steps, torch):
     rc = o.set_particles(*(parts[k] for k in F8))
     if rc:
         raise RuntimeError(f"oracle set_particles -> {rc}")
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        rc = o.step(cfg["dt"])
-        if rc:
-            raise RuntimeError(f"oracle step -> {rc}")
-    dt = time.perf_counter() - t0
+    # one pinned core; push and migrate timed apart: a step is exactly these two calls
+    old_aff = None
+    try:
+        old_aff = os.sched_getaffinity(0)
+        os.sched_setaffinity(0, {max(old_aff)})
+    except (AttributeError, OSError):
+        old_aff = None
+    t_push = t_mig = 0.0
+    try:
+        for _ in range(steps):
+            t0 = time.perf_counter()
+            rc = o.push(cfg["dt"])
+            t1 = time.perf_counter()
+            rc = rc or o.migrate()
+            t2 = time.perf_counter()
+            if rc:
+                raise RuntimeError(f"oracle step -> {rc}")
+            t_push += t1 - t0
+            t_mig += t2 - t1
+    finally:
+        if old_aff is not None:
+            os.sched_setaffinity(0, old_aff)
+    dt = t_push + t_mig
     o.close()
+    ORACLE_PHASES.update({"push": n_s * steps / t_push, "migrate": n_s * steps / t_mig, "step": n_s * steps / dt,
+                          "pinned": old_aff is not None, "core_model": cpu_model(), "nproc": os.cpu_count()})
     return n_s * steps / dt, dt / steps, n_s
+
+
+ORACLE_PHASES = {}      # filled by the last oracle_sample_rate call: particles/s per phase on the pinned core
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def bench_config(cfg, args, world):
@@ -229,7 +262,8 @@ def run_reference(args):
         "sample": {"particles_timed_per_step": n_s, "stride": stride},
         "cpu_baseline": {"value": rate, "unit": "particles/s", "cores": 1, "kind": "oracle",
                          "sample": f"every {stride}th particle of {cfg['name']} ({n_s} particles, full {cfg['N']}^3 field), "
-                                   f"{args.steps} steps, single thread"},
+                                   f"{args.steps} steps, single thread",
+                         "phases": dict(ORACLE_PHASES)},
         "e2e": {"value": rate, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line), flush=True)
@@ -251,6 +285,8 @@ def run_cuda(args):
     cfg, wl = build_workload(args.workload, dev)
     n, N = cfg["n"], cfg["N"]
     P = cfg["P"][0] * cfg["P"][1] * cfg["P"][2]
+    # the RK2 group is 8 more arrays of P*capacity doubles: 34 GB at Stress, which the box cannot spare beside the inputs
+    args.rk2 = bool(args.rk2) and args.phase_steps > 0 and cfg["name"] != "Stress"
     lcs = LCS(N, *cfg["P"], cfg["capacity"], g=cfg["g"], drag_model=args.drag_model, rk2=args.rk2, device=dev)
     lcs.set_fluid(wl["u"], wl["v"], wl["w"])
     parts = wl["particles"]
@@ -351,6 +387,22 @@ def run_cuda(args):
             evf[k][0].record(); lcs.set_fluid(wl["u"], wl["v"], wl["w"]); evf[k][1].record()
         torch.cuda.synchronize()
         fluid_ms = float(np.median([e[0].elapsed_time(e[1]) for e in evf]))
+        # ... and the refresh INSIDE the step, as the paper's coupled run has it (the fluid advances every time step,
+        # PAPER.md:41; the particles see the current field, :64): lcs_set_fluid with a field that differs from the one
+        # before (negated in place outside the timed region: the reversed flow, still divergence-free, so the slabs keep
+        # their occupancy -- a permutation of the components is compressible and overflows them within six steps)
+        # + lcs_step_fused, timed together
+        evs2 = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(6)]
+        for k in range(6):                                                    # an even count: the field ends as it began
+            for c in "uvw":
+                wl[c].neg_()
+            evs2[k][0].record(); lcs.set_fluid(wl["u"], wl["v"], wl["w"]); lcs.step_fused(dt); evs2[k][1].record()
+        torch.cuda.synchronize()
+        err_f, n_tot_f, n_mig_f = lcs.get_status()
+        if (err_f or n_tot_f != n):
+            print(f"bench.py: step with fluid refresh failed: sticky status {err_f}, total {n_tot_f}", file=sys.stderr)
+            return 3
+        refresh_step_ms = float(np.median([e[0].elapsed_time(e[1]) for e in evs2]))
         # statistics hook (second half): the pair count behind g(r), on a thin shell
         r_hi_pc = 2.0 * np.pi / N * 0.25
         evp = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
@@ -392,7 +444,15 @@ def run_cuda(args):
                 "note": "both stages run inside the tile pass; after stage 1 the slabs (8 arrays) and group B (X0, K1: 6 arrays) migrate in two rounds with the same codes, after stage 2 the slabs"},
             "set_fluid": {"call": "lcs_set_fluid", "ms": fluid_ms,
                           "GBps": (24.0 + 32.0) * N ** 3 / (fluid_ms * 1e-3) / 1e9,
-                          "note": "reads 24 B and writes 32 B per cell; off the timed step (the fluid is frozen)"},
+                          "note": "reads 24 B and writes 32 B per cell; timed alone here, inside the step in step_with_refresh"},
+            "step_with_refresh": {"call": "lcs_set_fluid + lcs_step_fused", "ms": refresh_step_ms,
+                                  "particles_per_s": n / (refresh_step_ms * 1e-3),
+                                  "algorithmic_bytes": n * (128.0 + 128.0 * m) + 24.0 * N ** 3 + 24.0 * N ** 3,
+                                  "algorithmic_GBps": (n * (128.0 + 128.0 * m) + 48.0 * N ** 3) / (refresh_step_ms * 1e-3) / 1e9,
+                                  "migrant_fraction": n_mig_f / n,
+                                  "note": "the field changes before every step (PAPER.md:41, :64): repack of a different "
+                                          "field + the fused step inside one timed region; bytes = the step's + 24 B per cell "
+                                          "read by the repack"},
             "pair_count": {"call": "lcs_pair_count", "ms": pair_ms, "r_lo": 0.0, "r_hi": r_hi_pc, "pairs": pairs, "g": g_of_r,
                            "particles_per_s": n / (pair_ms * 1e-3),
                            "note": "cell list of all particles + 27-cell neighbourhood; g = 1 for a uniform distribution"},
@@ -407,9 +467,13 @@ def run_cuda(args):
     if args.post_check:
         st = lcs.get_particles(n)
         ids = st["id"]
-        ref = torch.arange(n, dtype=torch.int64, device=dev)
-        ids_ok = bool(ids.sum() == ref.sum()) and bool((ids * ids).sum() == (ref * ref).sum()) and int(ids.min()) == 0 and int(ids.max()) == n - 1
-        del ref
+        # every id exactly once: n ids, all in [0, n), and every value of [0, n) hit (a scatter to a bool array)
+        ids_ok = ids.numel() == n and int(ids.min()) >= 0 and int(ids.max()) < n
+        if ids_ok:
+            hit = torch.zeros(n, dtype=torch.bool, device=dev)
+            hit[ids] = True
+            ids_ok = bool(hit.all())
+            del hit
         inv_dx = N / (2.0 * np.pi)
         own = None
         for k, Pk, mul in (("x", cfg["P"][0], 1), ("y", cfg["P"][1], cfg["P"][0]), ("z", cfg["P"][2], cfg["P"][0] * cfg["P"][1])):
@@ -519,7 +583,8 @@ def run_cuda(args):
         rate, sec, n_s = oracle_sample_rate(cfg, wl, stride, 2, torch)
         cpu = {"value": rate, "unit": "particles/s", "cores": 1, "kind": "oracle",
                "sample": f"every {stride}th particle of {cfg['name']} ({n_s} particles, full {N}^3 field), 2 steps, "
-                         f"single thread of {os.cpu_count()} host cores"}
+                         f"single thread of {os.cpu_count()} host cores",
+               "phases": dict(ORACLE_PHASES)}
 
     line = {
         "metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": world, "steps": args.steps,
@@ -548,8 +613,8 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1 << 21, help="--impl reference: particles per timed step")
     ap.add_argument("--drag-model", type=int, default=0, choices=[0, 1],
                     help="0: Stokes drag (BASELINE.json's configs); 1: f = 1 + 0.15 Re^0.687 (SURVEY 8(f) NEXT #2)")
-    ap.add_argument("--rk2", action="store_true",
-                    help="also time lcs_step_rk2 (SURVEY 8(f) NEXT #1); reserves 8 more arrays of P*capacity doubles")
+    ap.add_argument("--rk2", type=int, default=1, choices=[0, 1],
+                    help="1: also time lcs_step_rk2 (SURVEY 8(f) NEXT #1); reserves 8 more arrays of P*capacity doubles")
     ap.add_argument("--order", default="generation", choices=["generation", "morton"],
                     help="order in which the particles are handed to lcs_set_particles: generation order (spatially random, the "
                          "headline) or sorted by the Morton key of their cell (a labelled variant)")

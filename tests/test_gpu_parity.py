@@ -324,6 +324,41 @@ def test_host_buffer_entry_point_matches_oracle(torch_cuda, oracle_lib):
     dev.close()
 
 
+def test_live_handles_with_different_P_do_not_disturb_each_other(torch_cuda, oracle_lib):
+    """The dynamic shared memory limit of a kernel belongs to the kernel, not to a handle: a handle created later with a
+    smaller P (smaller tables in shared memory) must not lower the limit under a live handle with a larger P, and a failed
+    launch must not poison later calls.  Create (4,4,4), then (1,1,1) and (2,2,2), then step all of them, the first one
+    first, fused and unfused, and reload particles on each (k_set_scatter's limit is shared the same way)."""
+    rng = np.random.default_rng(77)
+    N = 16
+    z = np.zeros(N ** 3)
+    fluid = (z + 0.3, z - 0.2, z + 0.1)
+    pairs = []
+    for P, n in (((4, 4, 4), 20000), ((1, 1, 1), 3000), ((2, 2, 2), 9000)):
+        Ls = np.array([L / P[0], L / P[1], L / P[2]])
+        parts = random_parts(rng, n, 0.3 * Ls, d=2e-5)
+        cap = 2 * (int(2.5 * n / (P[0] * P[1] * P[2])) // 2 + 400)
+        o, dev, rc = make_pair(torch_cuda, oracle_lib, N, P, cap, fluid, parts)
+        assert rc == 0
+        pairs.append((o, dev, parts, P))
+    for rnd in range(2):
+        for o, dev, parts, P in pairs:                         # the (4,4,4) handle steps after the smaller ones exist
+            dev.step_fused(0.4)
+            assert o.step(0.4) == 0
+            dev.particle_step(0.4)
+            dev.migrate()
+            assert o.step(0.4) == 0
+            assert dev.get_status()[0] == 0
+            compare_packed(dev, o, f"P={P} round {rnd}")
+        for o, dev, parts, P in reversed(pairs):               # and a reload on every handle, largest P last
+            dp = to_dev(torch_cuda, parts)
+            dev.set_particles(*(dp[k] for k in F8))
+            assert o.set_particles(*(parts[k] for k in F8)) == 0
+            compare_packed(dev, o, f"reload P={P} round {rnd}")
+    for o, dev, parts, P in pairs:
+        dev.close()
+
+
 def test_pair_count_matches_oracle(torch_cuda, oracle_lib):
     """lcs_pair_count (the statistic behind g(r), R-26) against the oracle's O(n^2) definition:
     integer, bit-exact.  Uniform and clumped particles, several decompositions, shells that hit the cell-list limits
@@ -355,6 +390,39 @@ def test_pair_count_matches_oracle(torch_cuda, oracle_lib):
             with pytest.raises(LcsError) as ei:
                 dev.pair_count(*bad)
             assert ei.value.code == LCS_ERR_INVALID_ARG
+        dev.close()
+
+
+def test_pair_count_lattice_with_r_hi_equal_to_the_cell_side(torch_cuda, oracle_lib):
+    """Lattice data with r_hi = L/m (spacing = shell edge = what floor(L/r_hi) cells per axis would give as cell side):
+    neighbours at one spacing have r^2 within an ulp or two of r_hi^2, some below (counted), and their cell indices,
+    computed from rounded products, can differ by two when the cell side equals r_hi up to rounding.  The cell list must
+    keep its side strictly above r_hi; the count stays bit-exact against the O(n^2) definition."""
+    rng = np.random.default_rng(5)
+    for m, P in ((8, (2, 2, 2)), (12, (1, 1, 1)), (10, (2, 1, 2))):
+        h = L / m
+        g = np.arange(m) * h
+        X = np.stack(np.meshgrid(g, g, g, indexing="ij")).reshape(3, -1).copy()
+        n = X.shape[1]
+        for _ in range(2):                                   # a few ulps of jitter, both directions
+            up = rng.random((3, n)) < 0.3
+            dn = rng.random((3, n)) < 0.3
+            X = np.where(up, np.nextafter(X, 10.0), X)
+            X = np.where(dn, np.nextafter(X, -1.0), X)
+        X = np.clip(X, 0.0, np.nextafter(L, 0.0))
+        parts = {"x": X[0], "y": X[1], "z": X[2], "vx": np.zeros(n), "vy": np.zeros(n), "vz": np.zeros(n),
+                 "d": np.full(n, 1.0), "id": np.arange(n, dtype=np.int64)}
+        z = np.zeros(16 ** 3) if P != (1, 1, 1) else np.zeros(8 ** 3)
+        N = 16 if P != (1, 1, 1) else 8
+        o, dev, rc = make_pair(torch_cuda, oracle_lib, N, P, 2 * n, (z, z, z), parts)
+        assert rc == 0
+        counted = []
+        for r_lo, r_hi in ((0.0, h), (0.0, float(np.nextafter(h, 10.0))), (0.0, float(np.nextafter(h, 0.0))),
+                           (0.5 * h, h * (1 + 1e-15)), (0.0, h * (1 + 1e-13)), (0.99 * h, 1.01 * h), (0.0, 0.999 * h)):
+            want = o.pair_count(r_lo, r_hi)
+            assert int(dev.pair_count(r_lo, r_hi).item()) == want, (m, P, r_lo, r_hi)
+            counted.append(want)
+        assert 0 < counted[0] < 3 * n and counted[5] == 3 * n and counted[6] == 0     # the edge really splits the neighbours
         dev.close()
 
 
@@ -553,6 +621,50 @@ def _recipe_pair(torch, oracle_lib, name, n, N, **override):
     return cfg, o, dev
 
 
+@pytest.mark.parametrize("name,n,N,steps", [("Tiny", None, None, 8), ("Medium", 180000 + 13, 64, 6)])
+def test_fluid_refresh_before_every_step(torch_cuda, oracle_lib, name, n, N, steps):
+    """SURVEY 8(f) NEXT #4, first half: the carrier field changes every time step (section 2.1) and the
+    particles interpolate the CURRENT one.  One handle, lcs_set_fluid before every step with a field that
+    differs each time (a rotating mix of two generated fields, the same bytes to both sides), fused and unfused steps in
+    turn: a brick or halo cell left over from the previous field would show as a state mismatch.  ids / order / counts
+    exact, state 0 ulp, every step; the last refresh reuses the first field's arrays in another order."""
+    from workloads import gen
+    if n is None:
+        cfg = gen.get_config(name)
+        wl = gen.make_workload(cfg, device="cuda")
+        fluidA = [wl[k].cpu().numpy() for k in "uvw"]
+        parts = {k: v.cpu().numpy() for k, v in wl["particles"].items()}
+        o, dev, rc = make_pair(torch_cuda, oracle_lib, cfg["N"], cfg["P"], cfg["capacity"], fluidA, parts, g=cfg["g"])
+        assert rc == 0
+    else:
+        cfg, o, dev = _recipe_pair(torch_cuda, oracle_lib, name, n=n, N=N)
+        fluidA = [t.cpu().numpy() for t in gen.make_fluid(cfg, device="cuda")[:3]]
+    other = dict(cfg, index=cfg["index"] + 50)                 # other modes, same spectrum and rms
+    fluidB = [t.cpu().numpy() for t in gen.make_fluid(other, device="cuda")[:3]]
+    seen = []
+    for step in range(steps):
+        th = 0.7 * (step + 1)
+        if step == steps - 1:
+            field = [fluidA[2], fluidA[0], fluidA[1]]
+        else:
+            field = [np.ascontiguousarray(np.cos(th) * a + np.sin(th) * b) for a, b in zip(fluidA, fluidB)]
+        seen.append(float(field[0][5]))
+        o.set_fluid(*field)
+        dfield = [torch_cuda.from_numpy(f).cuda() for f in field]
+        dev.set_fluid(*dfield)
+        del dfield                                             # the library copied it: the caller may drop or reuse it
+        if step % 2 == 0:
+            dev.step_fused(cfg["dt"])
+        else:
+            dev.particle_step(cfg["dt"])
+            dev.migrate()
+        assert o.step(cfg["dt"]) == 0
+        assert dev.get_status() == (0, cfg["n"], o.n_migrated_last), step
+        compare_packed(dev, o, f"{name} refresh step {step}")
+    assert len(set(seen)) == steps                             # the fields really differed
+    dev.close()
+
+
 def test_clustered_shape_sample(torch_cuda, oracle_lib):
     """Clustered's recipe (Gaussian clumps, sigma = 2 cells, wide radius distribution): strongly non-uniform
     slab and migrant counts, ragged tiles everywhere."""
@@ -651,10 +763,19 @@ def test_full_size_free_running_P2_then_last_step_lockstep_P1(torch_cuda, oracle
         assert not np.array_equal(tail, np.sort(tail)), "the evolved state should no longer be in id order"
         del st
         gc.collect()
+        # the last step runs on a REFRESHED field: every brick and halo of a handle that has
+        # stepped K-1 times is rewritten (the reversed flow, negated in place: still divergence-free, so the slabs keep
+        # their occupancy in the steps that follow; the oracle borrows these arrays)
+        for f in fluid:
+            np.negative(f, out=f)
+        o.set_fluid(*fluid)
+        df = [torch_cuda.from_numpy(f).cuda() for f in fluid]
+        dev.set_fluid(*df)
+        del df
         assert o.step(dt) == 0
         dev.step_fused(dt)
         assert dev.get_status() == (0, n, o.n_migrated_last)
-        compare_packed(dev, o, f"{name}, step {K} in lock step")
+        compare_packed(dev, o, f"{name}, step {K} in lock step on a refreshed field")
     if name == "Large":
         # (3a) unfused push + axis-by-axis sweeps
         assert o.push(dt) == 0
