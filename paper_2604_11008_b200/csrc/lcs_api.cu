@@ -196,7 +196,6 @@ int enqueue_tile_pass(lcs_t* h, int mode, double dt, const Slabs* grp = nullptr,
     cudaEvent_t* ev = rec ? h->prof->data() + 4 * h->prof_steps : nullptr;
     if (rec) cudaEventRecord(ev[0], h->stream);
     const size_t smem = tile_pass_smem(G.P);
-    cudaMemsetAsync(h->T.gacc, 0, h->gacc_bytes, h->stream);
     const bool big = G.P > kTableSmemMax;
     const bool fused = mode != 0;
     const bool sn = fused && G.drag_model == 1;            // the unfused pass carries no push: one instantiation
@@ -218,7 +217,7 @@ int enqueue_tile_pass(lcs_t* h, int mode, double dt, const Slabs* grp = nullptr,
     k_table<<<(G.P + 7) / 8, 256, 0, h->stream>>>(G, h->T);
     if (rec) cudaEventRecord(ev[2], h->stream);
     k_unpack<<<dim3((G.chunks_per_sub + kUnpackWarps - 1) / kUnpackWarps, G.P), 32 * kUnpackWarps, 0, h->stream>>>(G, S, h->Snd, h->T, nf);
-    k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, commit ? 1 : 0);     // (also resets the tile ticket for the next round)
+    k_tile_index<<<1, 1024, 0, h->stream>>>(G, h->T, commit ? 1 : 0);     // (also resets the tile ticket and the look-back accumulators for the next round)
     if (rec) { cudaEventRecord(ev[3], h->stream); ++h->prof_steps; }
     if (commit) h->pushed = false;
     return check_launch(h, 5);

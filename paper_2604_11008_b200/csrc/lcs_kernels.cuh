@@ -17,24 +17,11 @@
 
 namespace lcs {
 
-#ifndef LCS_BLOCK
-#define LCS_BLOCK 384
-#endif
-#ifndef LCS_MIN_BLOCKS
-#define LCS_MIN_BLOCKS 1
-#endif
-constexpr int kBlock = LCS_BLOCK;            // threads per CTA of the tile pass
-constexpr int kMinBlocks = LCS_MIN_BLOCKS;   // CTAs per SM the tile pass is compiled for
+constexpr int kBlock = 384;                  // threads per CTA of the tile pass
+constexpr int kMinBlocks = 1;                // CTAs per SM the tile pass is compiled for
 constexpr int kWarps = kBlock / 32;
-#ifdef LCS_MAXREG
-#define LCS_TP_BOUNDS __maxnreg__(LCS_MAXREG)
-#else
 #define LCS_TP_BOUNDS __launch_bounds__(kBlock, kMinBlocks)
-#endif
-#ifndef LCS_ROWS
-#define LCS_ROWS 2
-#endif
-constexpr int kRows = LCS_ROWS;              // rows (particles per lane) of a warp tile
+constexpr int kRows = 2;                     // rows (particles per lane) of a warp tile
 constexpr int kTile = 32 * kRows;            // particles per tile
 static_assert(kRows >= 1 && kRows <= 4, "row masks and the unfused pass's code bytes are packed four rows to a word");
 constexpr int kStay = 13;
@@ -44,7 +31,7 @@ constexpr int kChunk = 256;                  // migrants of one send region hand
 
 // Look-back words (all 64-bit): [ count:24 | migrants:20 | stayers:20 ]
 //   desc[tile]   count = epoch of the launch that wrote it (1 .. 2^24-1); written once by the tile's push
-//   gacc[group]  count = tiles of the group of 32 that have published; zeroed per launch, accumulated by atomics
+//   gacc[group]  count = tiles of the group of 32 that have published; zeroed by k_tile_index after every round, accumulated by atomics
 constexpr unsigned long long kField20 = 0xfffffull;
 
 struct Geom {
@@ -72,7 +59,7 @@ struct Tables {
     uint32_t* recv_off;                // [P*32] slot in the receiver slab where segment (s,c) starts
     uint32_t* new_count;               // [P]
     uint64_t* desc;                    // [P*tiles_per_sub] tile aggregates
-    unsigned long long* gacc;          // [P*lbgroups_per_sub] accumulators of groups of 32 tiles (zeroed per launch)
+    unsigned long long* gacc;          // [P*lbgroups_per_sub] accumulators of groups of 32 tiles (zero between rounds: k_tile_index)
     uint32_t* tile_start;              // [P+1] compact prefix of non-empty tiles per subdomain
     uint32_t* send_count;              // [P] migrants in each send region after the tile pass
     uint32_t* chunk_excl;              // [P*chunks_per_sub*32] per-code count of each chunk, then its exclusive prefix over the chunks
@@ -387,10 +374,7 @@ k_repack_fluid(Geom G, const double* __restrict__ u, const double* __restrict__ 
 //   float reciprocals (prefetch shares); the ticket -> (s,t) map is an incremental search from the
 //   previous subdomain; particle slots are 32-bit indices (P*cap < 2^31 is checked at lcs_create).
 // ---------------------------------------------------------------------------------------------
-#ifndef LCS_NBUF
-#define LCS_NBUF 3
-#endif
-constexpr int kNBuf = LCS_NBUF;                     // tile buffers per warp: loading / being pushed / awaiting resolve
+constexpr int kNBuf = 3;                     // tile buffers per warp: loading / being pushed / awaiting resolve
 constexpr int kTableSmemMax = 1024;          // tile_start[] and the subdomain coordinates are mirrored in shared memory up to this P
 
 struct alignas(128) TileBuf {
@@ -1220,6 +1204,10 @@ k_tile_index(Geom G, Tables T, int commit)
         __syncthreads();
     }
     if (threadIdx.x == 0) { T.tile_start[G.P] = s_run; *T.ticket = 0u; }
+    // the group accumulators of the look-back start every tile pass at zero: cleared here, at the end of the round that
+    // used them (k_send_scan has read them by now), instead of a memset in front of every pass
+    const size_t ng = (size_t)G.P * (size_t)G.lbgroups_per_sub;
+    for (size_t i = threadIdx.x; i < ng; i += 1024) T.gacc[i] = 0ull;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1270,10 +1258,7 @@ k_table(Geom G, Tables T)
 // sorted by code in shared memory, so that the copy that follows writes runs: consecutive lanes, consecutive slots of one
 // receiver.  The reads from the send region are scattered only inside the chunk's 2 KB per array.
 // ---------------------------------------------------------------------------------------------
-#ifndef LCS_UNPACK_WARPS
-#define LCS_UNPACK_WARPS 4
-#endif
-constexpr int kUnpackWarps = LCS_UNPACK_WARPS;
+constexpr int kUnpackWarps = 4;
 
 __global__ void __launch_bounds__(32 * kUnpackWarps)
 k_unpack(Geom G, Slabs S, Slabs Snd, Tables T, int nf)

@@ -44,12 +44,12 @@ def assert_state_close(got, want, tag=""):
 
 
 def make_pair(torch, oracle_lib, N, P, cap, fluid, parts, g=(0.0, 0.0, 0.0), rho=1000.0, send_capacity=0, drag_model=0,
-              rk2=False):
+              rk2=False, nu=1.5e-5):
     from paper_2604_11008_b200 import LCS
-    o = oracle_lib.Oracle(N, *P, cap, g=g, rho_ratio=rho, drag_model=drag_model)
+    o = oracle_lib.Oracle(N, *P, cap, g=g, rho_ratio=rho, drag_model=drag_model, nu=nu)
     o.set_fluid(*fluid)
     rc = o.set_particles(*(parts[k] for k in F8))
-    dev = LCS(N, *P, cap, g=g, rho_ratio=rho, send_capacity=send_capacity, drag_model=drag_model, rk2=rk2)
+    dev = LCS(N, *P, cap, g=g, rho_ratio=rho, send_capacity=send_capacity, drag_model=drag_model, rk2=rk2, nu=nu)
     df = [torch.from_numpy(np.ascontiguousarray(f, dtype=np.float64)).cuda() for f in fluid]
     dev.set_fluid(*df)
     dp = to_dev(torch, parts)
@@ -665,6 +665,77 @@ def test_fluid_refresh_before_every_step(torch_cuda, oracle_lib, name, n, N, ste
     dev.close()
 
 
+@pytest.mark.parametrize("rho,nu,drag_model", [(843.0, 1.5e-5, 0), (843.0, 1.5e-5, 1), (1000.0, 1.0e-5, 0), (843.0, 1.8e-5, 1)])
+def test_paper_density_ratio_and_other_viscosities(torch_cuda, oracle_lib, rho, nu, drag_model):
+    """rho_p / rho = 843 is the paper's own value (BASELINE.json's configs say 1000) and nu enters tau_p and
+    Re_p: both reach the kernels only as the host-computed K_tau = rho_ratio / (18 nu) and 1 / nu, which the default
+    parameters of the other tests never vary.  Tiny's recipe, fused and unfused steps, lock-step, 0 ulp."""
+    from workloads import gen
+    cfg = gen.get_config("Tiny")
+    wl = gen.make_workload(cfg, device="cuda")
+    fluid = [wl[k].cpu().numpy() for k in "uvw"]
+    parts = {k: v.cpu().numpy() for k, v in wl["particles"].items()}
+    o, dev, rc = make_pair(torch_cuda, oracle_lib, cfg["N"], cfg["P"], cfg["capacity"], fluid, parts, g=(0.0, 0.0, -9.81),
+                           rho=rho, nu=nu, drag_model=drag_model)
+    assert rc == 0
+    for step in range(4):
+        if step % 2 == 0:
+            dev.step_fused(cfg["dt"])
+        else:
+            dev.particle_step(cfg["dt"])
+            dev.migrate()
+        assert o.step(cfg["dt"]) == 0
+        assert dev.get_status() == (0, cfg["n"], o.n_migrated_last)
+        compare_packed(dev, o, f"rho {rho} nu {nu} drag {drag_model} step {step}")
+    dev.close()
+
+
+def test_two_thousand_steps_fused_against_unfused(torch_cuda):
+    """A long run as a detector for a rare ordering bug in the look-back / in-place compaction protocol (PAPER.md:118:
+    "no data race occurs"), which the 10-100 step oracle comparisons cannot see: 2,000 fused steps of Medium (2^21
+    particles, 4x4x4, 64 subdomains x 640 tiles per pass) on one handle, the same 2,000 steps as lcs_particle_step +
+    lcs_migrate (other kernels, specified to give the same bits) on a second one.  Every 200 steps: every id exactly
+    once, every particle inside the subdomain of its slab, counts and all eight arrays identical between the two
+    handles.  Properties and GPU-vs-GPU identity only: the oracle pins the first 100 steps of this configuration
+    elsewhere."""
+    from workloads import gen
+    from paper_2604_11008_b200 import LCS
+    torch = torch_cuda
+    cfg = gen.get_config("Medium")
+    wl = gen.make_workload(cfg, device="cuda")
+    n, N, P = cfg["n"], cfg["N"], cfg["P"]
+    nP = P[0] * P[1] * P[2]
+    cap = 2 * cfg["capacity"]                                   # room for 2,000 steps of drift in the occupancy
+    devs = [LCS(N, *P, cap, g=cfg["g"], send_capacity=cfg["capacity"] // 2) for _ in range(2)]
+    for d in devs:
+        d.set_fluid(wl["u"], wl["v"], wl["w"])
+        d.set_particles(*(wl["particles"][k] for k in F8))
+    inv_dx = N / L
+    for block in range(10):
+        for _ in range(200):
+            devs[0].step_fused(cfg["dt"])
+            devs[1].particle_step(cfg["dt"])
+            devs[1].migrate()
+        st = [d.get_status() for d in devs]
+        assert st[0][:2] == (0, n) and st[1] == st[0], (block, st)
+        a, b = devs[0].get_particles(n), devs[1].get_particles(n)
+        for k in ("counts",) + F8:
+            assert torch.equal(a[k], b[k]), (block, k)
+        hit = torch.zeros(n, dtype=torch.bool, device="cuda")
+        assert int(a["id"].min()) >= 0 and int(a["id"].max()) < n
+        hit[a["id"]] = True
+        assert bool(hit.all()), block
+        own = None
+        for k, Pk, mul in (("x", P[0], 1), ("y", P[1], P[0]), ("z", P[2], P[0] * P[1])):
+            c = torch.clamp(torch.floor(a[k] * inv_dx).to(torch.int64), 0, N - 1) // (N // Pk) * mul
+            own = c if own is None else own + c
+        slab = torch.repeat_interleave(torch.arange(nP, dtype=torch.int64, device="cuda"), a["counts"])
+        assert slab.numel() == n and int((own != slab).sum()) == 0, block
+        del a, b, hit, own, slab
+    for d in devs:
+        d.close()
+
+
 def test_clustered_shape_sample(torch_cuda, oracle_lib):
     """Clustered's recipe (Gaussian clumps, sigma = 2 cells, wide radius distribution): strongly non-uniform
     slab and migrant counts, ragged tiles everywhere."""
@@ -699,6 +770,15 @@ def test_stress_shape_sample(torch_cuda, oracle_lib):
     dev.close()
 
 
+def _skip_or_fail(why):
+    """A full-size case that cannot run must not pass for one that did: on a box that should hold it (the B200 pool)
+    a shortage is a failure; LCS_ALLOW_SKIP=1 turns it into a skip on smaller machines."""
+    import os
+    if os.environ.get("LCS_ALLOW_SKIP") == "1":
+        pytest.skip(why)
+    pytest.fail(why + " (set LCS_ALLOW_SKIP=1 to skip on a smaller box)")
+
+
 def _reload_oracle_from_gpu(o, dev):
     """Protocol P1: the oracle takes over the GPU's current packed state (all codes = stay)."""
     st = to_np(dev.get_particles())
@@ -726,7 +806,7 @@ def test_full_size_free_running_P2_then_last_step_lockstep_P1(torch_cuda, oracle
     import psutil
     cfg = gen.get_config(name)
     if psutil.virtual_memory().available < 400 * cfg["n"] + 3 * 24 * cfg["N"] ** 3:
-        pytest.skip(f"{name} at full size needs more host memory for the oracle")
+        _skip_or_fail(f"{name} at full size needs more host memory for the oracle")
     K = cfg["steps"] if last is None else last
     first = K if first is None else first
     gc.collect()
@@ -734,7 +814,7 @@ def test_full_size_free_running_P2_then_last_step_lockstep_P1(torch_cuda, oracle
     nP = cfg["P"][0] * cfg["P"][1] * cfg["P"][2]
     need_dev = 97 * nP * cfg["capacity"] + 56 * cfg["N"] ** 3 + 80 * cfg["n"]
     if torch_cuda.cuda.mem_get_info()[0] < need_dev:
-        pytest.skip(f"{name} at full size needs {need_dev / 2**30:.0f} GiB of free device memory")
+        _skip_or_fail(f"{name} at full size needs {need_dev / 2**30:.0f} GiB of free device memory")
     wl = gen.make_workload(cfg, device="cuda")
     fluid = [wl[k].cpu().numpy() for k in "uvw"]
     parts = {k: v.cpu().numpy() for k, v in wl["particles"].items()}
@@ -831,7 +911,7 @@ def test_full_size_properties(torch_cuda, oracle_lib, name):
     torch.cuda.empty_cache()                           # the cached blocks of earlier tests count against this one
     need_dev = 97 * nP * cfg["capacity"] + 56 * N ** 3 + 144 * n      # workspace + input field + particle copies
     if torch.cuda.mem_get_info()[0] < need_dev or psutil.virtual_memory().available < 3 * 24 * N ** 3:
-        pytest.skip(f"{name} at full size needs {need_dev / 2**30:.0f} GiB of free device memory")
+        _skip_or_fail(f"{name} at full size needs {need_dev / 2**30:.0f} GiB of free device memory")
     wl = gen.make_workload(cfg, device="cuda")
     dev = LCS(N, *P, cfg["capacity"], g=cfg["g"], send_capacity=cfg["capacity"] // 2)
     dev.set_fluid(wl["u"], wl["v"], wl["w"])
