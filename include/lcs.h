@@ -230,7 +230,8 @@ int lcs_step_fused_host(lcs_t* h, double dt, int64_t n, const void* const h_in[8
 int lcs_profile_begin(lcs_t* h, int max_steps);
 int lcs_profile_end(lcs_t* h, double* ms_tile_pass, double* ms_table, double* ms_unpack, int* n_steps);
 
-/* Measurement aid for the roofline of the gather (a1): runs, alone on the handle's stream, a kernel in which every
+/* (The only export that is not part of the path: a measurement aid, used by bench.py's roofline.l2_to_sm.)
+ * Measurement aid for the roofline of the gather (a1): runs, alone on the handle's stream, a kernel in which every
  * lane issues eight independent 32-byte record loads per iteration (the gather's own load instruction, 12 warps per
  * SM) at pseudo-random records inside the first window_mb megabytes of the repacked fluid field, `iters` times, and
  * times it with CUDA events (synchronises).  *h_ms: duration in milliseconds, *h_bytes: sector bytes requested (host

@@ -140,7 +140,7 @@ class LCS:
     def set_fluid(self, u, v, w):
         for t in (u, v, w):
             assert t.is_cuda and t.dtype == self._torch.float64 and t.is_contiguous() and t.numel() == self.N ** 3
-        self._fluid = (u, v, w)   # borrowed by the library: keep alive
+        self._fluid = (u, v, w)   # (the library copies the field at call time, in stream order; kept only so that they outlive the enqueued repack)
         self._chk("lcs_set_fluid", self._L.lcs_set_fluid(self._h, _ptr(u), _ptr(v), _ptr(w)))
 
     def set_particles(self, x, y, z, vx, vy, vz, d, id):

@@ -1,7 +1,7 @@
 """One call of every timed entry point between cudaProfilerStart/Stop, for ncu captures of single kernels.
 
     ncu --set full --clock-control none --import-source on --profile-from-start off -o out \\
-        python -m paper_2604_11008_b200.profile_run --workload Large
+        python profile_run.py --workload Large
 
 Warm-up steps run first (unprofiled), so the profiled launches see the evolved state `bench.py` times.  The order of
 the profiled calls is: lcs_step_fused, lcs_particle_step, lcs_migrate, lcs_step_rk2 (with --rk2), lcs_set_fluid,
@@ -14,7 +14,7 @@ import argparse
 import os
 import sys
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
